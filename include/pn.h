@@ -1,0 +1,149 @@
+/*
+ * pn.h -- C ABI of libpn_b200: batched integration of post-Newtonian precessing circular-inspiral
+ * ODE systems on one NVIDIA B200 (sm_100a), after arXiv:0908.3889.
+ *
+ * What is computed (citations are lines of the paper text, PAPER.md, and sections of DESIGN.md):
+ *   - every system has the 10 state variables  y = (omega, S1x,S1y,S1z, S2x,S2y,S2z, Lx,Ly,Lz)
+ *      and two parameters (m1, m2); its right-hand side is Eq. (1) for omega
+ *     (PAPER.md:45), Eq. (2) with Omega_i of Eq. (4) for the spins and
+ *     Eq. (3) for L^, with the readings of DESIGN.md section 3;
+ *   - each system is integrated in time from its initial state until omega = omega_f
+ *      by an adaptive Dormand-Prince 5(4) stepper with per-system
+ *     error control; the last step lands on omega_f to a relative tau (R12);
+ *   - pn_histogram bins the unit-vector dot products S1^.S2^, S1^.L^, S2^.L^ of the final
+ *     states.
+ *
+ * Conventions
+ *   - Every function returns a pn_status.  Nothing throws.  Every CUDA call and kernel launch is
+ *     checked (unchecked kernels fail silently).
+ *   - Pointers are DEVICE pointers (cudaMalloc'ed, this process, current device) unless
+ *     pn_options.host_buffers != 0, in which case ALL array arguments of that call are HOST
+ *     pointers and the library stages them through its own device scratch (H2D before, D2H after).
+ *   - The caller owns every buffer.  The library keeps a small cached device scratch (SoA staging
+ *     arrays, work counter, status word) that pn_shutdown() frees.
+ *   - Calls are synchronous: on return the outputs are complete (the stream has been synchronised).
+ *     If pn_options.async != 0 and device pointers are used, the call only enqueues on
+ *     pn_options.stream and the per-call status is collected by pn_stream_status().
+ *   - N = 0 is a successful no-op.  Not thread-safe: one caller thread per process.
+ */
+#ifndef PN_B200_H
+#define PN_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { PN_FP64 = 0, PN_FP32 = 1 } pn_precision;
+
+typedef enum {
+    PN_OK = 0,
+    PN_EINVAL = 1,         /* bad argument (N < 0, null pointer, rtol <= 0, bins < 1, omega_f <= omega_0, m_i <= 0) */
+    PN_ECUDA = 2,          /* a CUDA call or launch failed; outputs unspecified; see pn_last_cuda_error() */
+    PN_ENOTCONVERGED = 3,  /* some system hit max_steps, step-size underflow or failed to land on omega_f */
+    PN_ENONFINITE = 4      /* some system produced a non-finite error norm */
+} pn_status;
+
+/* Per-system failure codes, written to out_steps[i] (which is otherwise the positive trial-step count). */
+#define PN_FAIL_MAXSTEPS   (-1)
+#define PN_FAIL_HUNDERFLOW (-2)
+#define PN_FAIL_NONFINITE  (-3)
+#define PN_FAIL_LANDING    (-4)
+#define PN_FAIL_BADINPUT   (-5)   /* m_i <= 0 or omega_0 >= omega_f for that system */
+
+/*
+ * pn_integrate -- adaptive DP5(4) integration of N independent systems to omega_f.
+ *   init_states [N][10] row-major doubles, order (omega, S1, S2, L^).  Read only.
+ *   masses      [N][2]  (m1, m2), any M = m1+m2 > 0 (the paper fixes M = 1).
+ *   omega0      consistency check only (the state is authoritative): if > 0, every
+ *               init_states[i][0] must equal it to 1e-12 relative, else PN_EINVAL.  <= 0: ignored.
+ *   omegaf      termination frequency, must exceed every initial omega.
+ *   rtol, atol  error control: a trial step is accepted when
+ *               sqrt(mean_j (err_j / (atol*N_j + rtol*max(|y_j|,|ynew_j|)))^2) <= 1, with N_j = 1 for
+ *               omega and L^, |S_i(0)| for the components of S_i (R6-R7).
+ *   precision   PN_FP64: all arithmetic in double.  PN_FP32: state, slopes, RHS and error norm in
+ *               float; time accumulation, step counters and all arrays of this interface in double.
+ *   out_final   [N][10] final states (the omega slot holds the landed omega, within tau of omega_f).
+ *   out_steps   [N] trial steps taken (accepted + rejected + discarded landing trials), or a
+ *               negative PN_FAIL_* code.  RHS evaluations of a system = 6*steps + 1.
+ * Returns PN_OK, or the worst status over all systems; the other systems still complete.
+ */
+int pn_integrate(const double* init_states, const double* masses, long long N,
+                 double omega0, double omegaf, double rtol, double atol, int precision,
+                 double* out_final, int* out_steps);
+
+typedef struct pn_options {
+    int size;              /* = sizeof(pn_options); checked */
+    int fixed_steps;       /* > 0: fixed-step mode: exactly this many DP5 steps of size h0, no error
+                              control, no omega_f stop (omegaf, rtol, atol ignored) */
+    double h0;             /* first step (adaptive) or the step (fixed); <= 0: 10*M */
+    int max_steps;         /* per system; <= 0: 10,000,000 */
+    unsigned term_mask;    /* tests only.  bit k (0..7) keeps the (M omega)^{k/3} term of the brace of
+                              Eq. (1); bit 16 keeps the spin terms of Eq. (1).  0: everything */
+    double tau_land;       /* landing tolerance |omega - omega_f| <= tau*omega_f; <= 0: 1e-13 (FP64), 3e-7 (FP32) */
+    int layout;            /* 0: AoS [N][10] / [N][2] as above.  1: SoA [10][N] / [2][N] for
+                              init_states, masses and out_final (no staging pass) */
+    int host_buffers;      /* != 0: every array argument is a HOST pointer (see Conventions) */
+    int async;             /* != 0: enqueue only (device pointers only) */
+    int sort_by_cost;      /* != 0: systems are issued to the work queue longest-expected-first
+                              (cost model in DESIGN.md 7); results are unaffected */
+    double* out_time;      /* [N] or NULL: time t_f at which omega_f was reached */
+    int* out_rejected;     /* [N] or NULL: rejected trial steps */
+    void* stream;          /* cudaStream_t, or NULL for the default stream */
+    int block_threads;     /* tuning: threads per block of the integrator (0: default) */
+    int grid_blocks;       /* tuning: blocks of the persistent grid (0: SMs x resident blocks) */
+} pn_options;
+
+/* Same as pn_integrate with explicit options (opt == NULL: defaults). */
+int pn_integrate_ex(const double* init_states, const double* masses, long long N,
+                    double omega0, double omegaf, double rtol, double atol, int precision,
+                    double* out_final, int* out_steps, const pn_options* opt);
+
+/*
+ * pn_histogram -- three histograms of the final configuration (R14).
+ *   final_states [N][10] (device, or host with the _ex variant), as written by pn_integrate.
+ *   bins         >= 1 equal-width bins over [-1, 1]; d = +1 falls in the last bin.
+ *   counts       [3][bins] unsigned 64-bit, overwritten: rows are S1^.S2^, S1^.L^, S2^.L^, where
+ *                A^.B^ = (A.B)/(|A||B|) with the norms taken from the state itself.
+ *   n_skipped    [3] or NULL: systems left out of each histogram because a norm is zero or the
+ *                quotient is not finite.
+ */
+int pn_histogram(const double* final_states, long long N, int bins,
+                 unsigned long long* counts, unsigned long long* n_skipped);
+
+/* As pn_histogram; layout/host_buffers/stream of opt are honoured (opt == NULL: defaults). */
+int pn_histogram_ex(const double* final_states, long long N, int bins,
+                    unsigned long long* counts, unsigned long long* n_skipped, const pn_options* opt);
+
+/* Worst pn_status of the async calls enqueued on `stream` since the last pn_stream_status; synchronises it. */
+int pn_stream_status(void* stream);
+
+/*
+ * pn_measure_fma_peak -- measured FMA throughput of this device at its current clocks: every thread
+ * runs `chains` independent dependent-FMA chains (no memory traffic) for about `seconds`.
+ * Writes achieved TFLOP/s (2 flops per FMA) and, if not NULL, the SM clock in MHz estimated from
+ * clock64() over the run.  The denominator of the reported roofline fraction.
+ */
+int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz);
+
+/* Device-side counters of the last synchronous pn_integrate* call: total trial steps, rejected
+ * steps, discarded landing trials, systems that failed.  Any pointer may be NULL. */
+int pn_last_counters(unsigned long long* trial_steps, unsigned long long* rejected,
+                     unsigned long long* landing_trials, unsigned long long* failed);
+
+/* Duration in milliseconds of the kernels of the last synchronous pn_integrate* / pn_histogram* call,
+ * measured with CUDA events on the call's stream: [0] stage-in, [1] integrator, [2] stage-out,
+ * [3] histogram.  Entries a call did not run are left unchanged. */
+int pn_last_kernel_ms(float ms[4]);
+
+/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
+unsigned long long pn_launch_count(void);
+
+const char* pn_strerror(int status);
+const char* pn_last_cuda_error(void);   /* text of the last failing CUDA call, "" if none */
+int pn_shutdown(void);                  /* frees cached scratch; the library stays usable */
+int pn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PN_B200_H */
