@@ -1,0 +1,277 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (pn_integrate + pn_histogram) on N B200s of one node.
+
+One "step" = one pass of the whole hot path over one batch of synthetic inspirals of the workload
+(default: C2 of BASELINE.json, 2^20 equal-mass maximally spinning inspirals, FP64, omega 0.005->0.05,
+rtol 1e-10): stage-in, persistent DP5(4) integrator, stage-out, histogram kernel.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+
+Prints ONE JSON line (see DESIGN.md 6 for every field).  Multi-GPU: the batch dimension is sharded
+(every rank integrates its own seeded batch of the same size: weak scaling); the only exchange is the
+all-reduce of the 3 x bins histogram counters.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_0908_3889_b200 import workloads as W  # noqa: E402
+
+# Algorithmic work per unit, counted on a constants-hoisted form of Eqs. (1)-(4) and the DP5(4) step
+# (every add, mul, div, sqrt, cbrt, log, pow = 1 flop, an FMA = 2):
+F_RHS = 109          # one right-hand-side evaluation
+F_STEP = 1240        # one trial step = 6 RHS + stage sums (400) + error vector (120) + norm/controller (~66)
+FP64_LANES_PER_SM = 64
+FP32_LANES_PER_SM = 128
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.check_output(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                               "-i", str(self.index)], timeout=5).decode().strip()
+                self.samples.append([t.strip() for t in out.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm, mx, reasons, pw = [], [], set(), []
+        for s in self.samples:
+            try:
+                sm.append(float(s[0])); mx.append(float(s[1])); pw.append(float(s[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), s[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_throughput(cfg, target_seconds=15.0, n_threads=0):
+    """Times the CPU oracle, as it stands, on a bounded seeded sample of the workload."""
+    from oracle import pn_oracle
+
+    pn_oracle.build()
+    y0, m = W.generate(W.with_size(cfg, min(cfg.n, 1 << 16)))
+    probe = min(256, y0.shape[0])
+    t0 = time.perf_counter()
+    pn_oracle.integrate(y0[:probe], m[:probe], cfg.omegaf, 1e-10, 1e-12, n_threads=n_threads)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    k = int(min(y0.shape[0], max(probe, probe * target_seconds / dt)))
+    t0 = time.perf_counter()
+    r = pn_oracle.integrate(y0[:k], m[:k], cfg.omegaf, 1e-10, 1e-12, n_threads=n_threads)
+    pn_oracle.histogram(r["final"], cfg.bins)
+    dt = time.perf_counter() - t0
+    cores = n_threads if n_threads > 0 else pn_oracle.num_threads()
+    return {"value": k / dt, "unit": "inspirals/s", "cores": cores, "kind": "oracle",
+            "sample": f"first {k} systems of the seeded {cfg.name} batch (FP64 oracle, rtol 1e-10, atol 1e-12), "
+                      f"{dt:.1f} s wall on {cores} threads, {os.cpu_count()} logical CPUs",
+            "rhs_evals_per_s": float((6 * r["steps"].astype(np.int64) + 1).sum() / dt), "seconds": dt,
+            "mean_steps": float(r["steps"].mean())}
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    per_step = []
+    last = None
+    for i in range(args.warmup + args.steps):
+        last = oracle_throughput(cfg, target_seconds=8.0 if i >= args.warmup else 2.0)
+        if i >= args.warmup:
+            per_step.append(last)
+    value = float(np.mean([p["value"] for p in per_step]))
+    line = {"impl": "reference", "metric": "inspirals_per_sec", "value": value, "unit": "inspirals/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([p["seconds"] for p in per_step])),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "n_inspirals": cfg.n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
+                       "rtol": 1e-10, "atol": 1e-12, "note": "each step is a bounded sample of the workload"},
+            "cpu_baseline": {k: last[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": value, "unit": "inspirals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "rhs_evals_per_sec": float(np.mean([p["rhs_evals_per_s"] for p in per_step])), "gpu_launches": 0}
+    line["cpu_baseline"]["value"] = value
+    print(json.dumps(line))
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    import paper_0908_3889_b200 as pn
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    prec = pn.PN_FP32 if cfg.precision == "fp32" else pn.PN_FP64
+
+    # every rank integrates its own seeded batch of the full workload size (weak scaling)
+    from dataclasses import replace
+    y0, m = W.generate(replace(cfg, seed=cfg.seed + 1000 * rank))
+    n = cfg.n
+    h_y0 = torch.from_numpy(y0).pin_memory(); h_m = torch.from_numpy(m).pin_memory()
+    d_y0, d_m = h_y0.to(dev), h_m.to(dev)
+    d_yf = torch.empty_like(d_y0)
+    d_steps = torch.empty(n, dtype=torch.int32, device=dev)
+    d_counts = torch.zeros(3, cfg.bins, dtype=torch.int64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        pn.pn_integrate(d_y0, d_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, d_yf, d_steps)
+        pn.pn_histogram(d_yf, cfg.bins, d_counts)
+        if world > 1:
+            dist.all_reduce(d_counts)        # the one exchange step of the sharded path
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(); flush.zero_()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    launches0 = pn.pn_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kern_ms, hist_ms, trial_steps = [], [], []
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+        k = pn.pn_last_kernel_ms(); kern_ms.append(k["integrate"]); hist_ms.append(k["histogram"])
+        trial_steps.append(pn.pn_last_counters()["trial_steps"])
+        flush.zero_()
+    ev1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = pn.pn_launch_count() - launches0
+    ms_total = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    counters = pn.pn_last_counters()
+
+    # end to end through the C ABI with HOST buffers: H2D of inputs and D2H of results inside the timed region
+    h_yf = torch.empty(n, 10, dtype=torch.float64).pin_memory()
+    h_steps = torch.empty(n, dtype=torch.int32).pin_memory()
+    h_counts = np.zeros((3, cfg.bins), dtype=np.uint64)
+    e2e_steps = max(1, min(args.steps, 3))
+
+    def e2e_step():
+        pn.pn_integrate(h_y0, h_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, h_yf, h_steps)
+        pn.pn_histogram(h_yf, cfg.bins, h_counts)
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_s = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    h2d = (10 + 2) * 8 * n + 10 * 8 * n          # states + masses for pn_integrate, final states for pn_histogram
+    d2h = 10 * 8 * n + 4 * n + 3 * cfg.bins * 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # roofline of the dominant kernel (the integrator): algorithmic flops / CUDA-event duration
+    lanes = FP32_LANES_PER_SM if prec == pn.PN_FP32 else FP64_LANES_PER_SM
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    peak_nominal = sms * lanes * 2 * sm_max * 1e6 / 1e12
+    peak_meas, peak_mhz = pn.pn_measure_fma_peak(prec, 0.5)
+    flops_launch = float(np.mean(trial_steps)) * F_STEP + n * F_RHS
+    k_ms = float(np.mean(kern_ms))
+    achieved = flops_launch / (k_ms * 1e-3) / 1e12
+    total_inspirals = n * world
+    line = {
+        "metric": "inspirals_per_sec", "value": total_inspirals / (ms_step * 1e-3), "unit": "inspirals/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if prec == pn.PN_FP32 else "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_inspirals_per_gpu": n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
+                   "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "parallelism": f"batch-sharded x{world}",
+                   "l2": "256 MiB memset between steps, inside the timed region (<0.1 % of a step)"},
+        "rhs_evals_per_sec": world * (6 * float(np.mean(trial_steps)) + n) / (ms_step * 1e-3),
+        "trial_steps_per_inspiral": float(np.mean(trial_steps)) / n,
+        "counters_last_step": counters,
+        "kernel_ms": {"integrate": k_ms, "histogram": float(np.mean(hist_ms))},
+        "roofline": {"bound": "alu", "kernel": "pn_integrate_adaptive_kernel", "achieved": achieved, "peak": peak_nominal,
+                     "unit": "TFLOP/s", "frac": achieved / peak_nominal, "traffic": None,
+                     "peak_source": f"nominal {sms} SMs x {lanes} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md 6.3)",
+                     "peak_measured_fma": peak_meas, "peak_measured_sm_mhz": peak_mhz,
+                     "frac_of_measured_fma": achieved / peak_meas if peak_meas > 0 else None,
+                     "flops_per_trial_step": F_STEP, "flops_per_rhs": F_RHS},
+        "e2e": {"value": total_inspirals / float(e2e_s.item()), "unit": "inspirals/s", "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cb = oracle_throughput(cfg, target_seconds=args.cpu_seconds)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"]["rhs_evals_per_s"] = cb["rhs_evals_per_s"]
+        line["paper_context"] = "paper: 0.057 inspirals/ms on 1 Xeon E5410 core (double) vs 2.7 inspirals/ms on 1 Tesla S1070 GPU (single), 'factor 50' (PAPER.md:86-96)"
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C2", choices=sorted(W.CONFIGS))
+    ap.add_argument("--n", type=int, default=0, help="override the batch size (not a bench line)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    cfg = W.CONFIGS[args.workload]
+    if args.n > 0:
+        cfg = W.with_size(cfg, args.n)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

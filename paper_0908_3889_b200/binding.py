@@ -1,0 +1,164 @@
+"""Thin ctypes binding of libpn_b200.so (C ABI in include/pn.h).  Argument marshalling only: every
+step of the path runs in the CUDA kernels.  torch is used for device memory and streams.
+
+There is NO CPU fallback: if the shared library is missing or no CUDA device is present, the calls
+raise.  This module never imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpn_b200.so")
+
+PN_FP64, PN_FP32 = 0, 1
+PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
+FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
+
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_stream_status",
+           "pn_measure_fma_peak", "pn_last_counters", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
+           "pn_last_cuda_error", "pn_shutdown", "pn_version"]
+
+
+class PnOptions(C.Structure):
+    _fields_ = [("size", C.c_int), ("fixed_steps", C.c_int), ("h0", C.c_double), ("max_steps", C.c_int),
+                ("term_mask", C.c_uint), ("tau_land", C.c_double), ("layout", C.c_int), ("host_buffers", C.c_int),
+                ("async_", C.c_int), ("sort_by_cost", C.c_int), ("out_time", C.c_void_p), ("out_rejected", C.c_void_p),
+                ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int)]
+
+
+class PnError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(msg)
+        self.status = status
+
+
+_lib = None
+
+
+def load():
+    """Loads the library; raises (loudly) if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_0908_3889_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        vp, d, ll, i = C.c_void_p, C.c_double, C.c_longlong, C.c_int
+        lib.pn_integrate.argtypes = [vp, vp, ll, d, d, d, d, i, vp, vp]
+        lib.pn_integrate_ex.argtypes = [vp, vp, ll, d, d, d, d, i, vp, vp, C.POINTER(PnOptions)]
+        lib.pn_histogram.argtypes = [vp, ll, i, vp, vp]
+        lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
+        lib.pn_stream_status.argtypes = [vp]
+        lib.pn_measure_fma_peak.argtypes = [i, d, C.POINTER(d), C.POINTER(d)]
+        lib.pn_last_counters.argtypes = [C.POINTER(C.c_ulonglong)] * 4
+        lib.pn_last_kernel_ms.argtypes = [C.POINTER(C.c_float)]
+        lib.pn_launch_count.restype = C.c_ulonglong
+        lib.pn_strerror.argtypes = [i]
+        lib.pn_strerror.restype = C.c_char_p
+        lib.pn_last_cuda_error.restype = C.c_char_p
+        _lib = lib
+    return _lib
+
+
+def _check(st, allow=()):
+    if st != PN_OK and st not in allow:
+        lib = load()
+        msg = lib.pn_strerror(st).decode()
+        if st == PN_ECUDA:
+            msg += ": " + lib.pn_last_cuda_error().decode()
+        raise PnError(st, f"pn status {st}: {msg}")
+    return st
+
+
+def _ptr(a):
+    """Address of a torch tensor (device or host) or a numpy array; None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return a.data_ptr()
+
+
+def _is_host(a) -> bool:
+    return isinstance(a, np.ndarray) or (hasattr(a, "is_cuda") and not a.is_cuda)
+
+
+def make_options(*, fixed_steps=0, h0=0.0, max_steps=0, term_mask=0, tau_land=0.0, layout=0, host_buffers=False,
+                 async_=False, sort_by_cost=False, out_time=None, out_rejected=None, stream=None, block_threads=0,
+                 grid_blocks=0) -> PnOptions:
+    o = PnOptions()
+    o.size = C.sizeof(PnOptions)
+    o.fixed_steps, o.h0, o.max_steps, o.term_mask, o.tau_land = int(fixed_steps), float(h0), int(max_steps), int(term_mask), float(tau_land)
+    o.layout, o.host_buffers, o.async_, o.sort_by_cost = int(layout), int(bool(host_buffers)), int(bool(async_)), int(bool(sort_by_cost))
+    o.out_time, o.out_rejected = _ptr(out_time), _ptr(out_rejected)
+    o.stream = None if stream is None else int(getattr(stream, "cuda_stream", stream))
+    o.block_threads, o.grid_blocks = int(block_threads), int(grid_blocks)
+    return o
+
+
+def pn_integrate(init_states, masses, omega0, omegaf, rtol, atol, precision, out_final, out_steps, *,
+                 allow_failures=False, **opts):
+    """pn_integrate_ex of include/pn.h.  Arrays are torch CUDA tensors (float64 / int32, contiguous), or
+    numpy / CPU tensors when every array is on the host (host_buffers is then set automatically).
+    Returns the pn_status (raises PnError unless it is PN_OK, or a per-system failure with allow_failures)."""
+    lib = load()
+    n = int(out_steps.shape[0])
+    host = _is_host(init_states)
+    for a in (masses, out_final, out_steps, opts.get("out_time"), opts.get("out_rejected")):
+        if a is not None and _is_host(a) != host:
+            raise ValueError("all arrays of one call must live on the same side (host or device)")
+    if host:
+        opts["host_buffers"] = True
+    o = make_options(**opts)
+    st = lib.pn_integrate_ex(_ptr(init_states), _ptr(masses), n, float(omega0), float(omegaf), float(rtol),
+                             float(atol), int(precision), _ptr(out_final), _ptr(out_steps), C.byref(o))
+    return _check(st, allow=(PN_ENOTCONVERGED, PN_ENONFINITE, PN_EINVAL) if allow_failures else ())
+
+
+def pn_histogram(final_states, bins, counts, n_skipped=None, *, n=None, **opts):
+    """pn_histogram_ex of include/pn.h: counts[3, bins] uint64 (torch int64 storage is accepted)."""
+    lib = load()
+    if n is None:
+        n = int(final_states.shape[1] if opts.get("layout", 0) == 1 else final_states.shape[0])
+    if _is_host(final_states):
+        opts["host_buffers"] = True
+    o = make_options(**opts)
+    return _check(lib.pn_histogram_ex(_ptr(final_states), int(n), int(bins), _ptr(counts), _ptr(n_skipped), C.byref(o)))
+
+
+def pn_stream_status(stream=None):
+    return load().pn_stream_status(None if stream is None else int(getattr(stream, "cuda_stream", stream)))
+
+
+def pn_measure_fma_peak(precision=PN_FP64, seconds=0.25):
+    t, mhz = C.c_double(0), C.c_double(0)
+    _check(load().pn_measure_fma_peak(int(precision), float(seconds), C.byref(t), C.byref(mhz)))
+    return t.value, mhz.value
+
+
+def pn_last_counters():
+    v = [C.c_ulonglong(0) for _ in range(4)]
+    load().pn_last_counters(*[C.byref(x) for x in v])
+    return dict(trial_steps=v[0].value, rejected=v[1].value, landing_trials=v[2].value, failed=v[3].value)
+
+
+def pn_last_kernel_ms():
+    ms = (C.c_float * 4)()
+    load().pn_last_kernel_ms(ms)
+    return dict(stage_in=ms[0], integrate=ms[1], stage_out=ms[2], histogram=ms[3])
+
+
+def pn_launch_count() -> int:
+    return int(load().pn_launch_count())
+
+
+def pn_shutdown():
+    return load().pn_shutdown()
+
+
+def pn_version() -> int:
+    return int(load().pn_version())

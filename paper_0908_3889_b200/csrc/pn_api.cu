@@ -1,0 +1,287 @@
+// pn_api.cu -- the C ABI of libpn_b200 (include/pn.h): argument checks, scratch management, staging,
+// launches, status collection.  Every CUDA call is checked.
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include "../../include/pn.h"
+#include "pn_internal.h"
+
+#define PN_VERSION 100
+
+static std::string g_last_err;
+#define CK(call)                                                                                     \
+    do {                                                                                             \
+        cudaError_t _e = (call);                                                                     \
+        if (_e != cudaSuccess) {                                                                     \
+            char _b[512];                                                                            \
+            snprintf(_b, sizeof _b, "%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(_e)); \
+            g_last_err = _b;                                                                         \
+            return PN_ECUDA;                                                                         \
+        }                                                                                            \
+    } while (0)
+
+// ---- cached device scratch ------------------------------------------------------------------------
+struct Buf {
+    void* p = nullptr;
+    size_t cap = 0;
+    int ensure(size_t bytes)
+    {
+        if (bytes <= cap) return PN_OK;
+        if (p) { CK(cudaFree(p)); p = nullptr; cap = 0; }
+        CK(cudaMalloc(&p, bytes));
+        cap = bytes;
+        return PN_OK;
+    }
+    int release()
+    {
+        if (p) { cudaError_t e = cudaFree(p); p = nullptr; cap = 0; if (e != cudaSuccess) return PN_ECUDA; }
+        return PN_OK;
+    }
+};
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
+static cudaEvent_t g_ev[5];
+static bool g_ev_ok = false;
+static float g_ms[4] = {0, 0, 0, 0};
+static unsigned long long g_counters[4] = {0, 0, 0, 0};
+static std::map<void*, int> g_stream_status;
+
+// layout of g_small: [0..3] counters (u64), then queue (u32), status (i32)
+struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned long long skipped[3]; };
+
+static int ensure_events()
+{
+    if (!g_ev_ok) {
+        for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&g_ev[i]));
+        g_ev_ok = true;
+    }
+    return PN_OK;
+}
+
+static void default_options(pn_options* o)
+{
+    memset(o, 0, sizeof *o);
+    o->size = (int)sizeof *o;
+}
+
+extern "C" int pn_integrate_ex(const double* init_states, const double* masses, long long N, double omega0,
+                               double omegaf, double rtol, double atol, int precision, double* out_final,
+                               int* out_steps, const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (N < 0 || N > 0x7fffffffLL / 16) return PN_EINVAL;
+    if (N == 0) return PN_OK;
+    if (!init_states || !masses || !out_final || !out_steps) return PN_EINVAL;
+    if (precision != PN_FP64 && precision != PN_FP32) return PN_EINVAL;
+    const bool fixed = o.fixed_steps > 0;
+    if (!fixed) {
+        if (!(rtol > 0.0) || !(atol >= 0.0) || !(omegaf > 0.0)) return PN_EINVAL;
+        if (omega0 > 0.0 && !(omega0 < omegaf)) return PN_EINVAL;
+    }
+    if (o.async && o.host_buffers) return PN_EINVAL;
+    if (o.block_threads != 0 && o.block_threads != 128 && o.block_threads != 256) return PN_EINVAL;
+    cudaStream_t s = (cudaStream_t)o.stream;
+    const int n = (int)N;
+    int rc;
+    if ((rc = ensure_events()) != PN_OK) return rc;
+
+    // ---- host buffers: stage through device scratch ----
+    const double* d_init = init_states;
+    const double* d_m = masses;
+    double* d_final = out_final;
+    int* d_steps = out_steps;
+    double* d_time = o.out_time;
+    int* d_rej = o.out_rejected;
+    if (o.host_buffers) {
+        if ((rc = g_h_init.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_h_m.ensure(sizeof(double) * 2 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_h_final.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_h_steps.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+        if (o.out_time && (rc = g_h_time.ensure(sizeof(double) * (size_t)n)) != PN_OK) return rc;
+        if (o.out_rejected && (rc = g_h_rej.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+        CK(cudaMemcpyAsync(g_h_init.p, init_states, sizeof(double) * 10 * (size_t)n, cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(g_h_m.p, masses, sizeof(double) * 2 * (size_t)n, cudaMemcpyHostToDevice, s));
+        d_init = (const double*)g_h_init.p; d_m = (const double*)g_h_m.p;
+        d_final = (double*)g_h_final.p; d_steps = (int*)g_h_steps.p;
+        d_time = o.out_time ? (double*)g_h_time.p : nullptr;
+        d_rej = o.out_rejected ? (int*)g_h_rej.p : nullptr;
+    }
+
+    // ---- SoA staging ----
+    if ((rc = g_small.ensure(sizeof(Small))) != PN_OK) return rc;
+    Small* small = (Small*)g_small.p;
+    CK(cudaMemsetAsync(small, 0, sizeof(Small), s));
+    PnKernelParams p;
+    memset(&p, 0, sizeof p);
+    CK(cudaEventRecord(g_ev[0], s));
+    if (o.layout == 0) {
+        if ((rc = g_soa_in.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_soa_m.ensure(sizeof(double) * 2 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_soa_out.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        CK(pn_launch_aos_to_soa(d_init, (double*)g_soa_in.p, n, 10, s));
+        CK(pn_launch_aos_to_soa(d_m, (double*)g_soa_m.p, n, 2, s));
+        p.y0 = (const double*)g_soa_in.p; p.masses = (const double*)g_soa_m.p; p.yf = (double*)g_soa_out.p;
+    } else {
+        p.y0 = d_init; p.masses = d_m; p.yf = d_final;
+    }
+    CK(cudaEventRecord(g_ev[1], s));
+    p.steps = d_steps; p.time = d_time; p.rejected = d_rej; p.order = nullptr;
+    p.n = n;
+    p.omega0 = omega0; p.omegaf = omegaf; p.rtol = rtol; p.atol = atol; p.h0 = o.h0;
+    p.tau = o.tau_land > 0.0 ? o.tau_land : (precision == PN_FP64 ? 1e-13 : 3e-7);
+    p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
+    p.fixed_steps = fixed ? o.fixed_steps : 0;
+    p.mask = o.term_mask;
+    p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
+    CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s));
+    CK(cudaEventRecord(g_ev[2], s));
+    if (o.layout == 0) CK(pn_launch_soa_to_aos((const double*)g_soa_out.p, d_final, n, 10, s));
+    CK(cudaEventRecord(g_ev[3], s));
+
+    if (o.async) {
+        // status is collected by pn_stream_status(); the Small block must stay untouched until then
+        g_stream_status[o.stream] = PN_OK;
+        return PN_OK;
+    }
+    if (o.host_buffers) {
+        CK(cudaMemcpyAsync(out_final, d_final, sizeof(double) * 10 * (size_t)n, cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(out_steps, d_steps, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, s));
+        if (o.out_time) CK(cudaMemcpyAsync(o.out_time, d_time, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, s));
+        if (o.out_rejected) CK(cudaMemcpyAsync(o.out_rejected, d_rej, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, s));
+    }
+    Small hs;
+    CK(cudaMemcpyAsync(&hs, small, sizeof hs, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&g_ms[i], g_ev[i], g_ev[i + 1]));
+    memcpy(g_counters, hs.counters, sizeof g_counters);
+    return hs.status;
+}
+
+extern "C" int pn_integrate(const double* init_states, const double* masses, long long N, double omega0,
+                            double omegaf, double rtol, double atol, int precision, double* out_final,
+                            int* out_steps)
+{
+    return pn_integrate_ex(init_states, masses, N, omega0, omegaf, rtol, atol, precision, out_final, out_steps, nullptr);
+}
+
+extern "C" int pn_histogram_ex(const double* final_states, long long N, int bins, unsigned long long* counts,
+                               unsigned long long* n_skipped, const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (N < 0 || bins < 1 || bins > (1 << 24) || !counts) return PN_EINVAL;
+    if (N > 0 && !final_states) return PN_EINVAL;
+    if (o.async && o.host_buffers) return PN_EINVAL;
+    cudaStream_t s = (cudaStream_t)o.stream;
+    int rc;
+    if ((rc = ensure_events()) != PN_OK) return rc;
+    const double* d_st = final_states;
+    unsigned long long* d_counts = counts;
+    unsigned long long* d_skip = n_skipped;
+    if (o.host_buffers) {
+        if (N > 0) {
+            if ((rc = g_h_final.ensure(sizeof(double) * 10 * (size_t)N)) != PN_OK) return rc;
+            CK(cudaMemcpyAsync(g_h_final.p, final_states, sizeof(double) * 10 * (size_t)N, cudaMemcpyHostToDevice, s));
+            d_st = (const double*)g_h_final.p;
+        }
+        if ((rc = g_h_counts.ensure(sizeof(unsigned long long) * (3 * (size_t)bins + 3))) != PN_OK) return rc;
+        d_counts = (unsigned long long*)g_h_counts.p;
+        d_skip = d_counts + 3 * (size_t)bins;
+    }
+    CK(cudaEventRecord(g_ev[3], s));
+    CK(pn_launch_histogram(d_st, o.layout, N, bins, d_counts, d_skip, s));
+    CK(cudaEventRecord(g_ev[4], s));
+    if (o.async) return PN_OK;
+    if (o.host_buffers) {
+        CK(cudaMemcpyAsync(counts, d_counts, sizeof(unsigned long long) * 3 * (size_t)bins, cudaMemcpyDeviceToHost, s));
+        if (n_skipped) CK(cudaMemcpyAsync(n_skipped, d_skip, sizeof(unsigned long long) * 3, cudaMemcpyDeviceToHost, s));
+    }
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    CK(cudaEventElapsedTime(&g_ms[3], g_ev[3], g_ev[4]));
+    return PN_OK;
+}
+
+extern "C" int pn_histogram(const double* final_states, long long N, int bins, unsigned long long* counts,
+                            unsigned long long* n_skipped)
+{
+    return pn_histogram_ex(final_states, N, bins, counts, n_skipped, nullptr);
+}
+
+extern "C" int pn_stream_status(void* stream)
+{
+    cudaStream_t s = (cudaStream_t)stream;
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    int st = PN_OK;
+    if (g_small.p && g_stream_status.count(stream)) {
+        Small hs;
+        CK(cudaMemcpy(&hs, g_small.p, sizeof hs, cudaMemcpyDeviceToHost));
+        memcpy(g_counters, hs.counters, sizeof g_counters);
+        st = hs.status;
+        g_stream_status.erase(stream);
+    }
+    return st;
+}
+
+extern "C" int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz)
+{
+    if (!tflops || (precision != PN_FP64 && precision != PN_FP32)) return PN_EINVAL;
+    CK(pn_run_fma_peak(precision, seconds, tflops, sm_mhz));
+    return PN_OK;
+}
+
+extern "C" int pn_last_counters(unsigned long long* trial_steps, unsigned long long* rejected,
+                                unsigned long long* landing_trials, unsigned long long* failed)
+{
+    if (trial_steps) *trial_steps = g_counters[0];
+    if (rejected) *rejected = g_counters[1];
+    if (landing_trials) *landing_trials = g_counters[2];
+    if (failed) *failed = g_counters[3];
+    return PN_OK;
+}
+
+extern "C" int pn_last_kernel_ms(float ms[4])
+{
+    if (!ms) return PN_EINVAL;
+    memcpy(ms, g_ms, sizeof g_ms);
+    return PN_OK;
+}
+
+extern "C" unsigned long long pn_launch_count(void) { return g_pn_launches; }
+
+extern "C" const char* pn_strerror(int st)
+{
+    switch (st) {
+        case PN_OK: return "ok";
+        case PN_EINVAL: return "invalid argument or input system";
+        case PN_ECUDA: return "CUDA call or kernel launch failed";
+        case PN_ENOTCONVERGED: return "a system hit max_steps, step-size underflow or failed to land on omega_f";
+        case PN_ENONFINITE: return "a system produced a non-finite error norm";
+        default: return "unknown status";
+    }
+}
+
+extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
+
+extern "C" int pn_shutdown(void)
+{
+    int rc = PN_OK;
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
+    for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
+    if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
+    g_stream_status.clear();
+    return rc;
+}
+
+extern "C" int pn_version(void) { return PN_VERSION; }

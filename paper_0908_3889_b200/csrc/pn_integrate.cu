@@ -1,0 +1,274 @@
+// pn_integrate.cu -- persistent-grid adaptive Dormand-Prince 5(4) integrator for sm_100a.
+//
+// One inspiral per lane.  Every warp iteration is one DP5 trial step executed by all 32 lanes in
+// lock-step (accept / reject / landing are per-lane selects, not branches around the RHS); a lane
+// whose inspiral has reached omega_f stores its result and immediately pulls the next system off a
+// global atomic work queue (warp-aggregated atomicAdd), so adaptive-step and termination divergence
+// cost only the short refill section.  All state (y, k1..k7, per-system constants) lives in
+// registers; global memory is touched only at refill and at finish.  (DESIGN.md 2, 7.)
+#include <cfloat>
+#include "pn_dp5.cuh"
+#include "pn_internal.h"
+
+#define PN_ST_EINVAL 1
+#define PN_ST_ENOTCONVERGED 3
+#define PN_ST_ENONFINITE 4
+#define PN_F_MAXSTEPS (-1)
+#define PN_F_HUNDERFLOW (-2)
+#define PN_F_NONFINITE (-3)
+#define PN_F_LANDING (-4)
+#define PN_F_BADINPUT (-5)
+
+template <typename real> struct PnLimits;
+template <> struct PnLimits<double> { static __device__ double tiny() { return 1e-300; } static __device__ double huge() { return DBL_MAX; } };
+template <> struct PnLimits<float> { static __device__ float tiny() { return 1e-30f; } static __device__ float huge() { return FLT_MAX; } };
+
+// 0.9 * E^{-1/5} (controller, DESIGN.md 3 R8).  Evaluated with the FP32 special-function unit in both
+// precisions: the factor only sets the next trial's step size, 1e-6 relative accuracy is ample and
+// it keeps ~100 instructions per trial step off the FP64 pipe.
+__device__ __forceinline__ float pn_ctrl_factor(float E) { return 0.9f * exp2f(-0.2f * __log2f(E)); }
+
+template <typename real>
+__device__ __forceinline__ void pn_store_result(const PnKernelParams& p, int idx, const real (&y)[10], int code,
+                                                double t, int nrej)
+{
+#pragma unroll
+    for (int i = 0; i < 10; ++i) p.yf[(size_t)i * p.n + idx] = (double)y[i];
+    p.steps[idx] = code;
+    if (p.time) p.time[idx] = t;
+    if (p.rejected) p.rejected[idx] = nrej;
+}
+
+template <typename real, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+
+    // lane state; idle lanes carry a benign dummy system so that the lock-step arithmetic stays finite
+    real y[10], k1[10];
+    PnConsts<real> c;
+    pn_make_consts<real>(0.5, 0.5, 0u, c);
+#pragma unroll
+    for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; }
+    y[0] = (real)0.01; y[9] = (real)1;
+    real h = (real)1, atS1 = (real)p.atol, atS2 = (real)p.atol;
+    double t = 0.0;
+    int idx = -1, steps = 0, nrej = 0, nland = 0;
+    bool after_reject = false, landing = false;
+    bool queue_empty = false;   // warp-uniform
+    unsigned tot_steps = 0, tot_rej = 0, tot_land = 0, tot_fail = 0;
+
+    const real omegaf = (real)p.omegaf;
+    const real om_hi = (real)(p.omegaf * (1.0 + p.tau));
+    const real om_tol = (real)(p.tau * p.omegaf);
+    const real rtol = (real)p.rtol, atol1 = (real)p.atol;
+
+    for (;;) {
+        // ---------------- refill: lanes without a system pull the next queue entries ----------------
+        if (!queue_empty) {
+            const unsigned wm = __ballot_sync(FULL, idx < 0);
+            if (wm) {
+                const int leader = __ffs(wm) - 1;
+                unsigned base = 0;
+                if (lane == leader) base = atomicAdd(p.queue, (unsigned)__popc(wm));
+                base = __shfl_sync(FULL, base, leader);
+                if (base + (unsigned)__popc(wm) >= (unsigned)p.n) queue_empty = true;
+                if (idx < 0) {
+                    const unsigned q = base + (unsigned)__popc(wm & ((1u << lane) - 1u));
+                    if (q < (unsigned)p.n) {
+                        const int i = p.order ? p.order[q] : (int)q;
+                        double y0[10];
+#pragma unroll
+                        for (int j = 0; j < 10; ++j) y0[j] = __ldg(p.y0 + (size_t)j * p.n + i);
+                        const double m1 = __ldg(p.masses + i), m2 = __ldg(p.masses + (size_t)p.n + i);
+#pragma unroll
+                        for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
+                        t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
+                        if (!(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
+                            (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0))) {
+                            pn_store_result(p, i, y, PN_F_BADINPUT, 0.0, 0);
+                            atomicMax(p.status, PN_ST_EINVAL);
+                            ++tot_fail;
+                            y[0] = (real)0.01;   // keep the dummy arithmetic benign
+                        } else {
+                            idx = i;
+                            pn_make_consts<real>(m1, m2, p.mask, c);
+                            pn_rhs(y, c, k1);
+                            h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
+                            // atol scaled by the conserved spin norms (R7)
+                            double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
+                            double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
+                            atS1 = (real)(p.atol * (s1 > 0.0 ? s1 : 1.0));
+                            atS2 = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
+                        }
+                    }
+                }
+            }
+        }
+        if (__all_sync(FULL, idx < 0)) break;
+
+        // ---------------- pre-trial guards (per lane) ----------------
+        if (idx >= 0) {
+            int code = 0;
+            if (steps >= p.max_steps) code = PN_F_MAXSTEPS;
+            else if (!(pn_abs(h) > PnLimits<real>::tiny()) || t + (double)h == t) code = PN_F_HUNDERFLOW;
+            if (code) {
+                pn_store_result(p, idx, y, code, t, nrej);
+                atomicMax(p.status, PN_ST_ENOTCONVERGED);
+                ++tot_fail; idx = -1; h = (real)1;
+            }
+        }
+
+        // ---------------- one DP5(4) trial step, all lanes ----------------
+        real ynew[10], k7[10], err[10];
+        pn_dp5_trial(y, k1, h, c, ynew, k7, err);
+
+        // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|)
+        real sum = (real)0;
+#pragma unroll
+        for (int i = 0; i < 10; ++i) {
+            const real at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
+            const real sc = pn_fma(rtol, pn_max(pn_abs(y[i]), pn_abs(ynew[i])), at);
+            const real q = err[i] / sc;
+            sum = pn_fma(q, q, sum);
+        }
+        real E = sqrt(sum * (real)0.1);
+
+        if (idx >= 0) {
+            ++steps; ++tot_steps;
+            if (!(E <= PnLimits<real>::huge())) {       // NaN or inf
+                pn_store_result(p, idx, y, PN_F_NONFINITE, t, nrej);
+                atomicMax(p.status, PN_ST_ENONFINITE);
+                ++tot_fail; idx = -1; h = (real)1;
+            } else {
+                const float fac = pn_ctrl_factor(fmaxf((float)E, 1e-30f));
+                if (E <= (real)1) {
+                    const real om_new = ynew[0];
+                    if (om_new > om_hi) {
+                        // passes error control but overshoots omega_f: discard, Newton update of h
+                        // from the same state with d(omega_new)/dh ~ k7[0] (R12)
+                        ++tot_land; landing = true;
+                        if (++nland > 50) {
+                            pn_store_result(p, idx, y, PN_F_LANDING, t, nrej);
+                            atomicMax(p.status, PN_ST_ENOTCONVERGED);
+                            ++tot_fail; idx = -1; h = (real)1;
+                        } else {
+                            const real hn = h - (om_new - omegaf) / k7[0];
+                            h = pn_max(hn, (real)0.1 * h);
+                        }
+                    } else {
+                        // accept
+                        t += (double)h;
+#pragma unroll
+                        for (int i = 0; i < 10; ++i) { y[i] = ynew[i]; k1[i] = k7[i]; }
+                        nland = 0;
+                        if (pn_abs(om_new - omegaf) <= om_tol) {
+                            pn_store_result(p, idx, y, steps, t, nrej);
+                            idx = -1; h = (real)1;
+                        } else if (landing) {
+                            h = pn_min(h, (omegaf - y[0]) / k1[0]);
+                        } else {
+                            h = h * (real)fminf(fmaxf(fac, 0.2f), after_reject ? 1.0f : 5.0f);
+                        }
+                        after_reject = false;
+                    }
+                } else {
+                    ++nrej; ++tot_rej;
+                    h = h * (real)fminf(fmaxf(fac, 0.2f), 1.0f);
+                    after_reject = true;
+                }
+            }
+        }
+    }
+
+    // ---------------- per-launch counters: warp reduce, one atomic per warp ----------------
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        tot_steps += __shfl_xor_sync(FULL, tot_steps, o);
+        tot_rej += __shfl_xor_sync(FULL, tot_rej, o);
+        tot_land += __shfl_xor_sync(FULL, tot_land, o);
+        tot_fail += __shfl_xor_sync(FULL, tot_fail, o);
+    }
+    if (lane == 0) {
+        atomicAdd(p.counters + 0, (unsigned long long)tot_steps);
+        atomicAdd(p.counters + 1, (unsigned long long)tot_rej);
+        atomicAdd(p.counters + 2, (unsigned long long)tot_land);
+        atomicAdd(p.counters + 3, (unsigned long long)tot_fail);
+    }
+}
+
+// Fixed-step mode (tests, R15): exactly fixed_steps DP5 steps of size h0, y <- y_new.
+template <typename real, int BLOCK>
+__global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKernelParams p)
+{
+    const int i = blockIdx.x * BLOCK + threadIdx.x;
+    if (i >= p.n) return;
+    double y0[10];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) y0[j] = p.y0[(size_t)j * p.n + i];
+    const double m1 = p.masses[i], m2 = p.masses[(size_t)p.n + i];
+    real y[10], k1[10];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
+    if (!(m1 > 0.0) || !(m2 > 0.0)) {
+        pn_store_result(p, i, y, PN_F_BADINPUT, 0.0, 0);
+        atomicMax(p.status, PN_ST_EINVAL);
+        return;
+    }
+    PnConsts<real> c;
+    pn_make_consts<real>(m1, m2, p.mask, c);
+    pn_rhs(y, c, k1);
+    const real h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
+    double t = 0.0;
+    for (int s = 0; s < p.fixed_steps; ++s) {
+        real ynew[10], k7[10], err[10];
+        pn_dp5_trial(y, k1, h, c, ynew, k7, err);
+#pragma unroll
+        for (int j = 0; j < 10; ++j) { y[j] = ynew[j]; k1[j] = k7[j]; }
+        t += (double)h;
+    }
+    pn_store_result(p, i, y, p.fixed_steps, t, 0);
+    if (threadIdx.x == 0) atomicAdd(p.counters, 0ull);
+}
+
+unsigned long long g_pn_launches = 0;
+
+template <typename real, int BLOCK, int MINB>
+static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
+{
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pn_integrate_adaptive_kernel<real, BLOCK, MINB>,
+                                                           BLOCK, 0)) != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    int grid = grid_blocks > 0 ? grid_blocks : sms * per_sm;
+    const long long need = ((long long)p.n + BLOCK - 1) / BLOCK;
+    if (need < grid) grid = (int)need;
+    if (grid < 1) grid = 1;
+    pn_integrate_adaptive_kernel<real, BLOCK, MINB><<<grid, BLOCK, 0, s>>>(p);
+    ++g_pn_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int block_threads, int grid_blocks,
+                                cudaStream_t s)
+{
+    if (p.n <= 0) return cudaSuccess;
+    if (p.fixed_steps > 0) {
+        const int B = 128;
+        const int grid = (p.n + B - 1) / B;
+        if (precision == 0) pn_integrate_fixed_kernel<double, B><<<grid, B, 0, s>>>(p);
+        else pn_integrate_fixed_kernel<float, B><<<grid, B, 0, s>>>(p);
+        ++g_pn_launches;
+        return cudaGetLastError();
+    }
+    if (precision == 0) {
+        if (block_threads == 256) return launch_adaptive<double, 256, 1>(p, grid_blocks, s);
+        return launch_adaptive<double, 128, 2>(p, grid_blocks, s);
+    }
+    if (block_threads == 128) return launch_adaptive<float, 128, 4>(p, grid_blocks, s);
+    return launch_adaptive<float, 256, 2>(p, grid_blocks, s);
+}

@@ -1,0 +1,39 @@
+// pn_internal.h -- declarations shared by the translation units of libpn_b200 (host side only).
+#pragma once
+#include <cuda_runtime.h>
+
+// Arguments of the integrator kernels.  All arrays are DEVICE pointers in SoA layout with stride n:
+// y0[c*n + i], masses[j*n + i], yf[c*n + i].
+struct PnKernelParams {
+    const double* y0;
+    const double* masses;
+    double* yf;
+    int* steps;
+    double* time;        // may be null
+    int* rejected;       // may be null
+    const int* order;    // may be null: queue position -> system index
+    int n;
+    double omega0;       // > 0: every initial omega must match it to 1e-12 relative
+    double omegaf, rtol, atol, h0, tau;
+    int max_steps;
+    int fixed_steps;
+    unsigned mask;
+    unsigned int* queue;            // global work counter (zeroed before launch)
+    unsigned long long* counters;   // [0] trial steps [1] rejected [2] landing trials [3] failed systems
+    int* status;                    // worst pn_status seen on the device (atomicMax)
+};
+
+// launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults
+cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int block_threads, int grid_blocks,
+                                cudaStream_t s);
+// staging + histogram + peak (pn_aux.cu)
+cudaError_t pn_launch_aos_to_soa(const double* aos, double* soa, int n, int width, cudaStream_t s);
+cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int width, cudaStream_t s);
+cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long n, int bins,
+                                unsigned long long* counts /*[3][bins]*/, unsigned long long* skipped /*[3]*/,
+                                cudaStream_t s);
+cudaError_t pn_launch_cost_keys(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys,
+                                int* idx, cudaStream_t s);
+cudaError_t pn_run_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz);
+
+extern unsigned long long g_pn_launches;

@@ -1,0 +1,146 @@
+// pn_rhs.cuh -- register-resident right-hand side of the precessing PN inspiral ODEs for sm_100a.
+//
+// Eqs. (1)-(4) of arXiv:0908.3889 rewritten for the device:
+//   x = M omega, v = x^{1/3};  everything that depends only on (m1, m2) is folded once per system into
+//   PnConsts, the brace of Eq. (1) becomes a Horner polynomial in v whose v^3, v^4 and v^6 coefficients
+//   carry the spin-orbit, spin-spin and log terms, and the three cross products L x S1, L x S2, S2 x S1
+//   are shared between Eq. (2) and Eq. (3):
+//     S1_dot = alpha1 (L x S1) + beta (S2 x S1),   alpha_i = A_i v^5 - 3 beta (L.S_j),  beta = x^2/(2 M^3)
+//     S2_dot = alpha2 (L x S2) - beta (S2 x S1)
+//     L_dot  = -v/(eta M^2) [alpha1 (L x S1) + alpha2 (L x S2)]      (the beta pieces cancel in the sum)
+// This file shares nothing with oracle/ (which evaluates the equations as printed).
+#pragma once
+#include <cuda_runtime.h>
+
+#define PN_MASK_ALL 0x100FFu
+#define PN_MASK_SPIN (1u << 16)
+
+// ---- scalar helpers, one overload per precision -------------------------------------------------
+__device__ __forceinline__ double pn_fma(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float pn_fma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double pn_abs(double a) { return fabs(a); }
+__device__ __forceinline__ float pn_abs(float a) { return fabsf(a); }
+__device__ __forceinline__ double pn_max(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ float pn_max(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ double pn_min(double a, double b) { return fmin(a, b); }
+__device__ __forceinline__ float pn_min(float a, float b) { return fminf(a, b); }
+
+// Per-system constants.  Computed in double from (m1, m2, term_mask), stored in `real`.
+template <typename real>
+struct PnConsts {
+    real M;        // m1 + m2
+    real c0, c2, c3, c4, c5, c6, c7;  // spin-independent coefficients of v^k in the brace of Eq. (1)
+    real cl;       // coefficient of ln(x) inside the v^6 term: -(856/105)(2/3)
+    real p1, p2;   // spin-orbit: v^3 coefficient += p1 (L.S1) + p2 (L.S2)
+    real q1, q2;   // spin-spin:  v^4 coefficient += q1 (S1.S2) + q2 (L.S1)(L.S2)
+    real K0;       // omega_dot = K0 v^11 brace,  K0 = 96 eta / (5 M^2)
+    real A1, A2;   // A_i = eta (4 + 3 m_j/m_i) / (2M)
+    real Bc;       // beta = Bc x^2,  Bc = 1/(2 M^3)
+    real G;        // L_dot prefactor: -1/(eta M^2), times v
+};
+
+template <typename real>
+__device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned mask, PnConsts<real>& c)
+{
+    if (mask == 0) mask = PN_MASK_ALL;
+    const double pi = 3.14159265358979323846, gammaE = 0.5772156649015329;
+    const double M = m1 + m2, M2 = M * M;
+    const double eta = m1 * m2 / M2;
+    const double spin = (mask & PN_MASK_SPIN) ? 1.0 : 0.0;
+    auto on = [&](int k) { return (mask >> k) & 1u ? 1.0 : 0.0; };
+    c.M = (real)M;
+    c.c0 = (real)on(0);
+    c.c2 = (real)(on(2) * (-(743.0 + 924.0 * eta) / 336.0));
+    c.c3 = (real)(on(3) * (4.0 * pi));
+    c.c4 = (real)(on(4) * (34103.0 / 18144.0 + (13661.0 / 2016.0) * eta + (59.0 / 18.0) * eta * eta));
+    c.c5 = (real)(on(5) * (-(4159.0 + 15876.0 * eta) * pi / 672.0));
+    // theta^ enters linearly in eta (R1); ln(16 x^{2/3}) = ln 16 + (2/3) ln x, natural log (R2)
+    const double theta = 1039.0 / 4620.0;
+    c.c6 = (real)(on(6) * (16447322263.0 / 139708800.0 - (1712.0 / 105.0) * gammaE + (16.0 / 3.0) * pi * pi +
+                           (-273811877.0 / 1088640.0 + (451.0 / 48.0) * pi * pi - (88.0 / 3.0) * theta) * eta +
+                           (541.0 / 896.0) * eta * eta - (5605.0 / 2592.0) * eta * eta * eta -
+                           (856.0 / 105.0) * 2.772588722239781237669 /* ln 16 */));
+    c.cl = (real)(on(6) * (-(856.0 / 105.0) * (2.0 / 3.0)));
+    c.c7 = (real)(on(7) * ((-4415.0 / 4032.0 + (358675.0 / 6048.0) * eta + (91495.0 / 1512.0) * eta * eta) * pi));
+    const double w1 = 113.0 * m1 * m1 / M2 + 75.0 * eta, w2 = 113.0 * m2 * m2 / M2 + 75.0 * eta;
+    c.p1 = (real)(-on(3) * spin * w1 / (12.0 * m1 * m1));
+    c.p2 = (real)(-on(3) * spin * w2 / (12.0 * m2 * m2));
+    const double mm = (m1 * m1) * (m2 * m2);
+    c.q1 = (real)(-on(4) * spin * 247.0 * eta / (48.0 * mm));
+    c.q2 = (real)(on(4) * spin * 721.0 * eta / (48.0 * mm));
+    c.K0 = (real)(96.0 * eta / (5.0 * M2));
+    c.A1 = (real)(eta * (4.0 + 3.0 * m2 / m1) / (2.0 * M));
+    c.A2 = (real)(eta * (4.0 + 3.0 * m1 / m2) / (2.0 * M));
+    c.Bc = (real)(1.0 / (2.0 * M2 * M));
+    c.G = (real)(-1.0 / (eta * M2));
+}
+
+// v = x^{1/3} and ln x.  First version: the CUDA math library; FP32 uses the hardware approximations
+// (MUFU lg2) for the log, whose absolute error ~1e-6 enters B(v) scaled by (856/105)(2/3) x^2 <= 1.4e-2.
+__device__ __forceinline__ void pn_cbrt_log(double x, double& v, double& lnx)
+{
+    v = cbrt(x);
+    lnx = log(x);
+}
+__device__ __forceinline__ void pn_cbrt_log(float x, float& v, float& lnx)
+{
+    v = cbrtf(x);
+    lnx = __logf(x);
+}
+
+// f = RHS(y).  ~75 FMA-pipe instructions plus the cube root and the logarithm; no memory traffic.
+template <typename real>
+__device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, real (&f)[10])
+{
+    const real x = c.M * y[0];
+    real v, lnx;
+    pn_cbrt_log(x, v, lnx);
+    const real v2 = v * v, v4 = v2 * v2, v5 = v4 * v, x2 = x * x;
+
+    const real S1x = y[1], S1y = y[2], S1z = y[3];
+    const real S2x = y[4], S2y = y[5], S2z = y[6];
+    const real Lx = y[7], Ly = y[8], Lz = y[9];
+
+    const real LS1 = pn_fma(Lx, S1x, pn_fma(Ly, S1y, Lz * S1z));
+    const real LS2 = pn_fma(Lx, S2x, pn_fma(Ly, S2y, Lz * S2z));
+    const real S12 = pn_fma(S1x, S2x, pn_fma(S1y, S2y, S1z * S2z));
+
+    // Eq. (1): Horner in v; coefficients of v^3, v^4, v^6 carry the spin-orbit, spin-spin, log pieces
+    const real k3 = pn_fma(c.p1, LS1, pn_fma(c.p2, LS2, c.c3));
+    const real k4 = pn_fma(c.q1, S12, pn_fma(c.q2 * LS1, LS2, c.c4));
+    const real k6 = pn_fma(c.cl, lnx, c.c6);
+    real B = pn_fma(c.c7, v, k6);
+    B = pn_fma(B, v, c.c5);
+    B = pn_fma(B, v, k4);
+    B = pn_fma(B, v, k3);
+    B = pn_fma(B, v, c.c2);
+    B = pn_fma(B, v2, c.c0);
+    f[0] = (c.K0 * (v5 * x2)) * B;
+
+    // Eq. (4),(2): shared cross products
+    const real beta = c.Bc * x2;
+    const real b3 = (real)3.0 * beta;
+    const real al1 = pn_fma(-b3, LS2, c.A1 * v5);
+    const real al2 = pn_fma(-b3, LS1, c.A2 * v5);
+    // u1 = alpha1 (L x S1), u2 = alpha2 (L x S2), w = beta (S2 x S1)
+    const real u1x = al1 * pn_fma(Ly, S1z, -(Lz * S1y));
+    const real u1y = al1 * pn_fma(Lz, S1x, -(Lx * S1z));
+    const real u1z = al1 * pn_fma(Lx, S1y, -(Ly * S1x));
+    const real u2x = al2 * pn_fma(Ly, S2z, -(Lz * S2y));
+    const real u2y = al2 * pn_fma(Lz, S2x, -(Lx * S2z));
+    const real u2z = al2 * pn_fma(Lx, S2y, -(Ly * S2x));
+    const real wx = pn_fma(S2y, S1z, -(S2z * S1y));
+    const real wy = pn_fma(S2z, S1x, -(S2x * S1z));
+    const real wz = pn_fma(S2x, S1y, -(S2y * S1x));
+    f[1] = pn_fma(beta, wx, u1x);
+    f[2] = pn_fma(beta, wy, u1y);
+    f[3] = pn_fma(beta, wz, u1z);
+    f[4] = pn_fma(-beta, wx, u2x);
+    f[5] = pn_fma(-beta, wy, u2y);
+    f[6] = pn_fma(-beta, wz, u2z);
+    // Eq. (3)
+    const real g = c.G * v;
+    f[7] = g * (u1x + u2x);
+    f[8] = g * (u1y + u2y);
+    f[9] = g * (u1z + u2z);
+}

@@ -1,0 +1,146 @@
+"""GPU edge cases of the boundary: empty / tiny / ragged batches, failure codes, layouts, host buffers,
+determinism, and the full-size launch configuration checked on sampled systems."""
+import numpy as np
+import pytest
+
+from paper_0908_3889_b200 import workloads as W
+from test_gpu_parity import check_adaptive, dots_of, gpu_integrate, pn  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def test_empty_and_tiny(pn, oracle):
+    dev = "cuda:0"
+    e10 = torch.empty(0, 10, dtype=torch.float64, device=dev)
+    e2 = torch.empty(0, 2, dtype=torch.float64, device=dev)
+    es = torch.empty(0, dtype=torch.int32, device=dev)
+    assert pn.pn_integrate(e10, e2, 0.0, 0.05, 1e-10, 1e-12, 0, e10, es) == 0
+    counts = torch.ones(3, 7, dtype=torch.int64, device=dev)
+    pn.pn_histogram(e10, 7, counts, n=0)
+    assert counts.sum().item() == 0
+    for n in (1, 31, 33, 257):
+        cfg = W.with_size(W.CONFIGS["C1"], n)
+        y0, m = W.generate(cfg)
+        check_adaptive(pn, oracle, cfg, y0, m)
+
+
+def test_invalid_arguments(pn):
+    from paper_0908_3889_b200 import PnError
+
+    cfg = W.with_size(W.CONFIGS["C1"], 64)
+    y0, m = W.generate(cfg)
+    with pytest.raises(PnError) as e:
+        gpu_integrate(pn, y0, m, cfg, rtol=0.0)
+    assert e.value.status == 1
+    with pytest.raises(PnError):
+        gpu_integrate(pn, y0, m, cfg, omega0=0.06)            # omega0 >= omega_f
+    with pytest.raises(PnError):
+        gpu_integrate(pn, y0, m, cfg, precision=7)
+    with pytest.raises(PnError):
+        pn.pn_histogram(torch.zeros(4, 10, dtype=torch.float64, device="cuda:0"), 0,
+                        torch.zeros(3, 1, dtype=torch.int64, device="cuda:0"))
+    # wrong omega0 for one system -> that system is flagged, the call reports EINVAL, others complete
+    y1 = y0.copy(); y1[5, 0] = 0.021
+    g = gpu_integrate(pn, y1, m, cfg, omega0=0.02, allow_failures=True)
+    assert g["status"] == 1 and g["steps"][5] == -5 and np.all(np.delete(g["steps"], 5) > 0)
+
+
+def test_per_system_failures_do_not_stop_the_batch(pn):
+    cfg = W.with_size(W.CONFIGS["C1"], 100)
+    y0, m = W.generate(cfg)
+    m[3, 1] = -0.5                      # bad mass
+    y0[7, 0] = 0.07                     # already beyond omega_f
+    g = gpu_integrate(pn, y0, m, cfg, allow_failures=True)
+    assert g["status"] == 1
+    assert g["steps"][3] == -5 and g["steps"][7] == -5
+    good = np.ones(100, bool); good[[3, 7]] = False
+    assert np.all(g["steps"][good] > 0)
+    assert np.array_equal(g["final"][3], y0[3])
+    # max_steps
+    g = gpu_integrate(pn, y0[good], m[good], cfg, max_steps=20, allow_failures=True)
+    assert g["status"] == 3 and np.all(g["steps"] == -1)
+    c = pn.pn_last_counters()
+    assert c["failed"] == good.sum() and c["trial_steps"] == 20 * good.sum()
+    # non-finite state
+    y2 = y0[good].copy(); y2[0, 2] = np.nan
+    g = gpu_integrate(pn, y2, m[good], cfg, allow_failures=True)
+    assert g["status"] == 4 and g["steps"][0] == -3 and np.all(g["steps"][1:] > 0)
+
+
+def test_zero_spin_and_aligned_systems(pn, oracle):
+    """Degenerate cases of the method: chi = 0 (no division by |S|), aligned spins (no precession)."""
+    cfg = W.with_size(W.CONFIGS["C2"], 6)
+    y0, m = W.generate(cfg)
+    y0[0, 1:7] = 0.0
+    y0[1, 1:4] = 0.0
+    y0[2, 1:4] = [0, 0, 0.25]; y0[2, 4:7] = [0, 0, -0.25]
+    g, r = check_adaptive(pn, oracle, cfg, y0, m)
+    assert np.array_equal(g["final"][0, 1:], y0[0, 1:]) and np.array_equal(g["final"][2, 1:], y0[2, 1:])
+    counts = torch.zeros(3, 10, dtype=torch.int64, device="cuda:0")
+    skipped = torch.zeros(3, dtype=torch.int64, device="cuda:0")
+    pn.pn_histogram(g["d_final"], 10, counts, skipped)
+    assert skipped.cpu().tolist() == [2, 2, 1]
+
+
+def test_layouts_host_buffers_and_determinism(pn, oracle):
+    cfg = W.with_size(W.CONFIGS["C3"], 1000)
+    y0, m = W.generate(cfg)
+    a = gpu_integrate(pn, y0, m, cfg)
+    b = gpu_integrate(pn, y0, m, cfg)
+    assert np.array_equal(a["final"], b["final"]) and np.array_equal(a["steps"], b["steps"])   # queue order is irrelevant
+    # SoA layout
+    dev = "cuda:0"
+    d_y0 = torch.from_numpy(y0.T.copy()).to(dev); d_m = torch.from_numpy(m.T.copy()).to(dev)
+    d_yf = torch.empty_like(d_y0); d_steps = torch.empty(cfg.n, dtype=torch.int32, device=dev)
+    pn.pn_integrate(d_y0, d_m, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, d_yf, d_steps, layout=1)
+    assert np.array_equal(d_yf.cpu().numpy().T, a["final"]) and np.array_equal(d_steps.cpu().numpy(), a["steps"])
+    # host buffers (numpy in, numpy out)
+    h_yf = np.empty_like(y0); h_steps = np.empty(cfg.n, dtype=np.int32); h_t = np.empty(cfg.n)
+    pn.pn_integrate(y0, m, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, h_yf, h_steps, out_time=h_t)
+    assert np.array_equal(h_yf, a["final"]) and np.array_equal(h_steps, a["steps"]) and np.array_equal(h_t, a["time"])
+    # both block shapes agree bit for bit
+    c = gpu_integrate(pn, y0, m, cfg, block_threads=256)
+    assert np.array_equal(c["final"], a["final"])
+    # a stream from torch, async enqueue, status collected afterwards
+    s = torch.cuda.Stream()
+    d_y0a = torch.from_numpy(y0).to(dev); d_ma = torch.from_numpy(m).to(dev)
+    d_yfa = torch.empty_like(d_y0a); s.wait_stream(torch.cuda.current_stream())
+    pn.pn_integrate(d_y0a, d_ma, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, d_yfa, d_steps, stream=s, async_=True)
+    assert pn.pn_stream_status(s) == 0
+    assert np.array_equal(d_yfa.cpu().numpy(), a["final"])
+
+
+@pytest.mark.parametrize("name,nsample", [("C2", 768), ("C3", 768), ("C4", 1024), ("C5", 192)])
+def test_full_size_launch_configuration_sampled(pn, oracle, name, nsample):
+    """BASELINE.json's full sizes in the launch configuration bench.py times; outputs compared on a
+    seeded sample the oracle can compute one by one, plus properties that hold at any size."""
+    cfg = W.CONFIGS[name]
+    y0, m = W.generate(cfg)
+    idx = W.sample_indices(cfg.n, nsample)
+    g, r = check_adaptive(pn, oracle, cfg, y0, m, idx=idx)
+    f = g["final"]
+    assert np.abs(f[:, 0] - cfg.omegaf).max() <= 1.01e-13 * cfg.omegaf
+    for s in (slice(1, 4), slice(4, 7), slice(7, 10)):
+        n0 = np.linalg.norm(y0[:, s], axis=1); n1 = np.linalg.norm(f[:, s], axis=1)
+        ok = n0 > 0
+        assert np.abs(n1[ok] / n0[ok] - 1).max() < 1e-7
+    c = pn.pn_last_counters()
+    assert c["trial_steps"] == g["steps"].sum() and c["failed"] == 0
+    counts = torch.zeros(3, cfg.bins, dtype=torch.int64, device="cuda:0")
+    skipped = torch.zeros(3, dtype=torch.int64, device="cuda:0")
+    pn.pn_histogram(g["d_final"], cfg.bins, counts, skipped)
+    c_ref = oracle.histogram(f, cfg.bins)[0].astype(np.int64)
+    assert np.abs(counts.cpu().numpy() - c_ref).sum() <= 8
+    assert counts.sum().item() + skipped.sum().item() == 3 * cfg.n
+
+
+def test_fp32_full_size_C4_histograms(pn, oracle):
+    cfg64, cfg32 = W.CONFIGS["C4"], W.CONFIGS["C4f"]
+    y0, m = W.generate(cfg64)
+    a = gpu_integrate(pn, y0, m, cfg64)
+    b = gpu_integrate(pn, y0, m, cfg32, precision=1)
+    da, db = dots_of(oracle, a["final"]), dots_of(oracle, b["final"])
+    assert np.abs(da - db).max() <= 2e-3
+    ca = oracle.histogram(a["final"], 50)[0].astype(np.int64); cb = oracle.histogram(b["final"], 50)[0].astype(np.int64)
+    assert np.all(np.abs(ca - cb) <= 5 * np.sqrt(ca + cb + 1))
