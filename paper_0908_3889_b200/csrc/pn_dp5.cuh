@@ -41,34 +41,35 @@
 // estimate err = h sum_s e_s k_s.  6 RHS evaluations, 200 + 60 FMAs, 26 coefficient multiplies.
 template <typename real>
 __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&k1)[10], real h,
-                                             const PnConsts<real>& c, real (&ynew)[10], real (&k7)[10],
-                                             real (&err)[10])
+                                             const PnConsts<real>& c, const PnBase<real>& base, real (&ynew)[10],
+                                             real (&k7)[10], real (&err)[10], PnBase<real>& base_new)
 {
     real k2[10], k3[10], k4[10], k5[10], k6[10], ys[10];
+    real r_tmp, l_tmp;
     {
         const real a1 = h * (real)DP_A21;
 #pragma unroll
         for (int i = 0; i < 10; ++i) ys[i] = pn_fma(a1, k1[i], y[i]);
-        pn_rhs(ys, c, k2);
+        pn_rhs(ys, c, base, k2, r_tmp, l_tmp);
     }
     {
         const real a1 = h * (real)DP_A31, a2 = h * (real)DP_A32;
 #pragma unroll
         for (int i = 0; i < 10; ++i) ys[i] = pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i]));
-        pn_rhs(ys, c, k3);
+        pn_rhs(ys, c, base, k3, r_tmp, l_tmp);
     }
     {
         const real a1 = h * (real)DP_A41, a2 = h * (real)DP_A42, a3 = h * (real)DP_A43;
 #pragma unroll
         for (int i = 0; i < 10; ++i) ys[i] = pn_fma(a3, k3[i], pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i])));
-        pn_rhs(ys, c, k4);
+        pn_rhs(ys, c, base, k4, r_tmp, l_tmp);
     }
     {
         const real a1 = h * (real)DP_A51, a2 = h * (real)DP_A52, a3 = h * (real)DP_A53, a4 = h * (real)DP_A54;
 #pragma unroll
         for (int i = 0; i < 10; ++i)
             ys[i] = pn_fma(a4, k4[i], pn_fma(a3, k3[i], pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i]))));
-        pn_rhs(ys, c, k5);
+        pn_rhs(ys, c, base, k5, r_tmp, l_tmp);
     }
     {
         const real a1 = h * (real)DP_A61, a2 = h * (real)DP_A62, a3 = h * (real)DP_A63, a4 = h * (real)DP_A64,
@@ -77,7 +78,7 @@ __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&k
         for (int i = 0; i < 10; ++i)
             ys[i] = pn_fma(a5, k5[i],
                            pn_fma(a4, k4[i], pn_fma(a3, k3[i], pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i])))));
-        pn_rhs(ys, c, k6);
+        pn_rhs(ys, c, base, k6, r_tmp, l_tmp);
     }
     {
         const real b1 = h * (real)DP_B1, b3 = h * (real)DP_B3, b4 = h * (real)DP_B4, b5 = h * (real)DP_B5,
@@ -89,7 +90,8 @@ __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&k
             ynew[i] = pn_fma(b6, k6[i], pn_fma(b5, k5[i], pn_fma(b4, k4[i], pn_fma(b3, k3[i], pn_fma(b1, k1[i], y[i])))));
             err[i] = pn_fma(e6, k6[i], pn_fma(e5, k5[i], pn_fma(e4, k4[i], pn_fma(e3, k3[i], e1 * k1[i]))));
         }
-        pn_rhs(ynew, c, k7);
+        pn_rhs(ynew, c, base, k7, r_tmp, l_tmp);
+        base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
         const real e7 = h * (real)DP_E7;
 #pragma unroll
         for (int i = 0; i < 10; ++i) err[i] = pn_fma(e7, k7[i], err[i]);

@@ -26,7 +26,19 @@ template <> struct PnLimits<float> { static __device__ float tiny() { return 1e-
 // 0.9 * E^{-1/5} (controller, DESIGN.md 3 R8).  Evaluated with the FP32 special-function unit in both
 // precisions: the factor only sets the next trial's step size, 1e-6 relative accuracy is ample and
 // it keeps ~100 instructions per trial step off the FP64 pipe.
-__device__ __forceinline__ float pn_ctrl_factor(float E) { return 0.9f * exp2f(-0.2f * __log2f(E)); }
+// argument: E^2 = mean_j (err_j/sc_j)^2, so the factor is 0.9 (E^2)^{-1/10}; no square root needed.
+__device__ __forceinline__ float pn_ctrl_factor(float E2) { return 0.9f * exp2f(-0.1f * __log2f(E2)); }
+
+// err/sc for the error norm: MUFU reciprocal seed (rcp.approx.ftz.f64, ~2^-23) + one Newton step gives
+// ~1.4e-14 relative accuracy with 3 FP64-pipe instructions and no slow-path branch (an IEEE divide is ~10).
+__device__ __forceinline__ double pn_ratio(double a, double b)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+    r = fma(fma(-b, r, 1.0), r, r);
+    return a * r;
+}
+__device__ __forceinline__ float pn_ratio(float a, float b) { return __fdividef(a, b); }
 
 template <typename real>
 __device__ __forceinline__ void pn_store_result(const PnKernelParams& p, int idx, const real (&y)[10], int code,
@@ -48,10 +60,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     // lane state; idle lanes carry a benign dummy system so that the lock-step arithmetic stays finite
     real y[10], k1[10];
     PnConsts<real> c;
+    PnBase<real> base;
     pn_make_consts<real>(0.5, 0.5, 0u, c);
 #pragma unroll
     for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; }
     y[0] = (real)0.01; y[9] = (real)1;
+    pn_base_init(c.M * y[0], base);
     real h = (real)1, atS1 = (real)p.atol, atS2 = (real)p.atol;
     double t = 0.0;
     int idx = -1, steps = 0, nrej = 0, nland = 0;
@@ -70,12 +84,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
             const unsigned wm = __ballot_sync(FULL, idx < 0);
             if (wm) {
                 const int leader = __ffs(wm) - 1;
-                unsigned base = 0;
-                if (lane == leader) base = atomicAdd(p.queue, (unsigned)__popc(wm));
-                base = __shfl_sync(FULL, base, leader);
-                if (base + (unsigned)__popc(wm) >= (unsigned)p.n) queue_empty = true;
+                unsigned qbase = 0;
+                if (lane == leader) qbase = atomicAdd(p.queue, (unsigned)__popc(wm));
+                qbase = __shfl_sync(FULL, qbase, leader);
+                if (qbase + (unsigned)__popc(wm) >= (unsigned)p.n) queue_empty = true;
                 if (idx < 0) {
-                    const unsigned q = base + (unsigned)__popc(wm & ((1u << lane) - 1u));
+                    const unsigned q = qbase + (unsigned)__popc(wm & ((1u << lane) - 1u));
                     if (q < (unsigned)p.n) {
                         const int i = p.order ? p.order[q] : (int)q;
                         double y0[10];
@@ -91,10 +105,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                             atomicMax(p.status, PN_ST_EINVAL);
                             ++tot_fail;
                             y[0] = (real)0.01;   // keep the dummy arithmetic benign
+                            pn_base_init(c.M * y[0], base);
                         } else {
                             idx = i;
                             pn_make_consts<real>(m1, m2, p.mask, c);
-                            pn_rhs(y, c, k1);
+                            pn_base_init(c.M * y[0], base);
+                            real r_tmp, l_tmp;
+                            pn_rhs(y, c, base, k1, r_tmp, l_tmp);
                             h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
                             // atol scaled by the conserved spin norms (R7)
                             double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
@@ -122,7 +139,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
 
         // ---------------- one DP5(4) trial step, all lanes ----------------
         real ynew[10], k7[10], err[10];
-        pn_dp5_trial(y, k1, h, c, ynew, k7, err);
+        PnBase<real> base_new;
+        pn_dp5_trial(y, k1, h, c, base, ynew, k7, err, base_new);
 
         // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|)
         real sum = (real)0;
@@ -130,20 +148,20 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         for (int i = 0; i < 10; ++i) {
             const real at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
             const real sc = pn_fma(rtol, pn_max(pn_abs(y[i]), pn_abs(ynew[i])), at);
-            const real q = err[i] / sc;
+            const real q = pn_ratio(err[i], sc);
             sum = pn_fma(q, q, sum);
         }
-        real E = sqrt(sum * (real)0.1);
+        const real E2 = sum * (real)0.1;      // E^2; accept iff E^2 <= 1
 
         if (idx >= 0) {
             ++steps; ++tot_steps;
-            if (!(E <= PnLimits<real>::huge())) {       // NaN or inf
+            if (!(E2 <= PnLimits<real>::huge())) {       // NaN or inf
                 pn_store_result(p, idx, y, PN_F_NONFINITE, t, nrej);
                 atomicMax(p.status, PN_ST_ENONFINITE);
                 ++tot_fail; idx = -1; h = (real)1;
             } else {
-                const float fac = pn_ctrl_factor(fmaxf((float)E, 1e-30f));
-                if (E <= (real)1) {
+                const float fac = pn_ctrl_factor(fmaxf((float)E2, 1e-37f));
+                if (E2 <= (real)1) {
                     const real om_new = ynew[0];
                     if (om_new > om_hi) {
                         // passes error control but overshoots omega_f: discard, Newton update of h
@@ -162,6 +180,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                         t += (double)h;
 #pragma unroll
                         for (int i = 0; i < 10; ++i) { y[i] = ynew[i]; k1[i] = k7[i]; }
+                        base = base_new;
                         nland = 0;
                         if (pn_abs(om_new - omegaf) <= om_tol) {
                             pn_store_result(p, idx, y, steps, t, nrej);
@@ -218,12 +237,16 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
     }
     PnConsts<real> c;
     pn_make_consts<real>(m1, m2, p.mask, c);
-    pn_rhs(y, c, k1);
+    PnBase<real> base, base_new;
+    pn_base_init(c.M * y[0], base);
+    real r_tmp, l_tmp;
+    pn_rhs(y, c, base, k1, r_tmp, l_tmp);
     const real h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
     double t = 0.0;
     for (int s = 0; s < p.fixed_steps; ++s) {
         real ynew[10], k7[10], err[10];
-        pn_dp5_trial(y, k1, h, c, ynew, k7, err);
+        pn_dp5_trial(y, k1, h, c, base, ynew, k7, err, base_new);
+        base = base_new;
 #pragma unroll
         for (int j = 0; j < 10; ++j) { y[j] = ynew[j]; k1[j] = k7[j]; }
         t += (double)h;

@@ -75,26 +75,73 @@ __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned ma
     c.G = (real)(-1.0 / (eta * M2));
 }
 
-// v = x^{1/3} and ln x.  First version: the CUDA math library; FP32 uses the hardware approximations
-// (MUFU lg2) for the log, whose absolute error ~1e-6 enters B(v) scaled by (856/105)(2/3) x^2 <= 1.4e-2.
-__device__ __forceinline__ void pn_cbrt_log(double x, double& v, double& lnx)
+// ---- v = x^{1/3} and ln x, once per stage ------------------------------------------------------------
+// FP64: the library cbrt + log cost ~50 FP64-pipe instructions per stage, almost as much as the rest of
+// the RHS.  Within one trial step omega moves by a fraction of a percent, so both are expanded about the
+// step's base point x0 (the accepted state), for which r0 = x0^{-1/3} and l0 = ln x0 are carried:
+//     e = 1 - x r0^3            (= 1 - x/x0, one FMA)
+//     x^{-1/3} = r0 (1-e)^{-1/3} = r0 (1 + e/3 + 2e^2/9 + 14e^3/81 + ...)
+//     ln x     = l0 + log1p(-e)  = l0 - e (1 + e/2 + e^2/3 + ...)
+// The first expansion is self-correcting (it is exact in r0 whatever r0's own rounding error), so nothing
+// accumulates in r; l0 is chained once per accepted step with a truncation error < 3e-15 at the switch
+// point |e| = 0.03, beyond which the library functions are used (rare, divergent).  ~22 FMA-pipe
+// instructions per stage.  FP32 uses cbrtf and the MUFU log directly.
+template <typename real> struct PnBase { real r0, r03, l0; };
+
+__device__ __forceinline__ void pn_base_init(double x, PnBase<double>& b)
 {
-    v = cbrt(x);
-    lnx = log(x);
+    b.r0 = rcbrt(x);
+    b.r03 = b.r0 * b.r0 * b.r0;
+    b.l0 = log(x);
 }
-__device__ __forceinline__ void pn_cbrt_log(float x, float& v, float& lnx)
+__device__ __forceinline__ void pn_base_init(float, PnBase<float>& b) { b.r0 = b.r03 = b.l0 = 0.0f; }
+
+// r = x^{-1/3}, lnx = ln x  ->  returned so that an accepted step can adopt them as the next base
+__device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, double& v, double& lnx, double& r)
+{
+    const double e = fma(-x, b.r03, 1.0);
+    if (fabs(e) > 0.03) {
+        r = rcbrt(x);
+        lnx = log(x);
+    } else {
+        // (1-e)^{-1/3} = 1 + e S(e),  S = sum_{k=1..9} s_k e^{k-1},  s_k = prod_{j<k}(1/3 + j)/k!
+        // log1p(-e)    =   - e Q(e),  Q = sum_{k=1..9} e^{k-1}/k
+        // truncation < 6.1e-17 for |e| <= 0.03.  Even/odd split in e halves the dependent FMA chains.
+        const double e2 = e * e;
+        double Sa = 135850.0 / 1594323.0, Sb = 5434.0 / 59049.0;   // s9 | s8
+        Sa = fma(Sa, e2, 1976.0 / 19683.0);  Sb = fma(Sb, e2, 728.0 / 6561.0);   // s7 | s6
+        Sa = fma(Sa, e2, 91.0 / 729.0);      Sb = fma(Sb, e2, 35.0 / 243.0);     // s5 | s4
+        Sa = fma(Sa, e2, 14.0 / 81.0);       Sb = fma(Sb, e2, 2.0 / 9.0);        // s3 | s2
+        Sa = fma(Sa, e2, 1.0 / 3.0);                                             // s1
+        const double S = fma(Sb, e, Sa);
+        double Qa = 1.0 / 9.0, Qb = 1.0 / 8.0;
+        Qa = fma(Qa, e2, 1.0 / 7.0);  Qb = fma(Qb, e2, 1.0 / 6.0);
+        Qa = fma(Qa, e2, 1.0 / 5.0);  Qb = fma(Qb, e2, 1.0 / 4.0);
+        Qa = fma(Qa, e2, 1.0 / 3.0);  Qb = fma(Qb, e2, 1.0 / 2.0);
+        Qa = fma(Qa, e2, 1.0);
+        const double Q = fma(Qb, e, Qa);
+        r = fma(b.r0 * e, S, b.r0);
+        lnx = fma(-e, Q, b.l0);
+    }
+    v = x * (r * r);
+}
+__device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float& v, float& lnx, float& r)
 {
     v = cbrtf(x);
     lnx = __logf(x);
+    r = 0.0f;
 }
 
-// f = RHS(y).  ~75 FMA-pipe instructions plus the cube root and the logarithm; no memory traffic.
+// f = RHS(y).  ~75 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and
+// lnx_out = ln x of this evaluation are handed back for the base update of an accepted step.
 template <typename real>
-__device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, real (&f)[10])
+__device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, const PnBase<real>& base,
+                                       real (&f)[10], real& r_out, real& lnx_out)
 {
     const real x = c.M * y[0];
-    real v, lnx;
-    pn_cbrt_log(x, v, lnx);
+    real v, lnx, r;
+    pn_powers(x, base, v, lnx, r);
+    r_out = r; lnx_out = lnx;
     const real v2 = v * v, v4 = v2 * v2, v5 = v4 * v, x2 = x * x;
 
     const real S1x = y[1], S1y = y[2], S1z = y[3];
