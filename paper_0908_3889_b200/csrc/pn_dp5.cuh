@@ -1,7 +1,7 @@
 // pn_dp5.cuh -- one Dormand-Prince 5(4) trial step in registers (PAPER.md:66 names the method; the
 // tableau is the standard 7-stage FSAL pair, R5).  Written for register economy:
-//   - the step size is folded into the coefficients once per stage (h*a_sj), so a stage argument costs
-//     (s-1) FMAs per component;
+//   - the step size is folded into the slopes (K_s = h k_s), so a stage argument costs (s-1) FMAs per
+//     component with constant coefficients;
 //   - after k6 the 5th-order solution y_new and the partial error sum are formed together, so that
 //     k2..k6 are dead while the seventh RHS is evaluated; only y, k1 (kept for a rejected step), y_new
 //     and the error partial stay live.
@@ -37,63 +37,50 @@
 #define DP_E6 (22.0 / 525.0)
 #define DP_E7 (-1.0 / 40.0)
 
-// Trial step from (y, k1 = f(y)) with step h.  Outputs y_new (5th order), k7 = f(y_new) and the error
-// estimate err = h sum_s e_s k_s.  6 RHS evaluations, 200 + 60 FMAs, 26 coefficient multiplies.
+// Trial step from (y, K1 = h f(y)) with step h.  All slopes are "scaled" (K_s = h k_s, see pn_rhs.cuh), so
+// every coefficient below is a compile-time constant.  Outputs y_new (5th order), K7 = h f(y_new) and the
+// error estimate err = sum_s e_s K_s.  6 RHS evaluations, 200 + 60 FMAs.
 template <typename real>
-__device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&k1)[10], real h,
-                                             const PnConsts<real>& c, const PnBase<real>& base, real (&ynew)[10],
-                                             real (&k7)[10], real (&err)[10], PnBase<real>& base_new)
+__device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K1)[10], real h,
+                                             const PnConsts<real>& c, const PnUni<real>& u, const PnBase<real>& base,
+                                             real (&ynew)[10], real (&K7)[10], real (&err)[10], PnBase<real>& base_new)
 {
-    real k2[10], k3[10], k4[10], k5[10], k6[10], ys[10];
+    real K2[10], K3[10], K4[10], K5[10], K6[10], ys[10];
     real r_tmp, l_tmp;
-    {
-        const real a1 = h * (real)DP_A21;
+    PnScaled<real> sc;
+    pn_make_scaled(c, h, sc);
 #pragma unroll
-        for (int i = 0; i < 10; ++i) ys[i] = pn_fma(a1, k1[i], y[i]);
-        pn_rhs(ys, c, base, k2, r_tmp, l_tmp);
+    for (int i = 0; i < 10; ++i) ys[i] = pn_fma((real)DP_A21, K1[i], y[i]);
+    pn_rhs(ys, c, u, sc, base, K2, r_tmp, l_tmp);
+#pragma unroll
+    for (int i = 0; i < 10; ++i) ys[i] = pn_fma((real)DP_A32, K2[i], pn_fma((real)DP_A31, K1[i], y[i]));
+    pn_rhs(ys, c, u, sc, base, K3, r_tmp, l_tmp);
+#pragma unroll
+    for (int i = 0; i < 10; ++i)
+        ys[i] = pn_fma((real)DP_A43, K3[i], pn_fma((real)DP_A42, K2[i], pn_fma((real)DP_A41, K1[i], y[i])));
+    pn_rhs(ys, c, u, sc, base, K4, r_tmp, l_tmp);
+#pragma unroll
+    for (int i = 0; i < 10; ++i)
+        ys[i] = pn_fma((real)DP_A54, K4[i],
+                       pn_fma((real)DP_A53, K3[i], pn_fma((real)DP_A52, K2[i], pn_fma((real)DP_A51, K1[i], y[i]))));
+    pn_rhs(ys, c, u, sc, base, K5, r_tmp, l_tmp);
+#pragma unroll
+    for (int i = 0; i < 10; ++i)
+        ys[i] = pn_fma((real)DP_A65, K5[i],
+                       pn_fma((real)DP_A64, K4[i],
+                              pn_fma((real)DP_A63, K3[i], pn_fma((real)DP_A62, K2[i], pn_fma((real)DP_A61, K1[i], y[i])))));
+    pn_rhs(ys, c, u, sc, base, K6, r_tmp, l_tmp);
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        ynew[i] = pn_fma((real)DP_B6, K6[i],
+                         pn_fma((real)DP_B5, K5[i],
+                                pn_fma((real)DP_B4, K4[i], pn_fma((real)DP_B3, K3[i], pn_fma((real)DP_B1, K1[i], y[i])))));
+        err[i] = pn_fma((real)DP_E6, K6[i],
+                        pn_fma((real)DP_E5, K5[i],
+                               pn_fma((real)DP_E4, K4[i], pn_fma((real)DP_E3, K3[i], (real)DP_E1 * K1[i]))));
     }
-    {
-        const real a1 = h * (real)DP_A31, a2 = h * (real)DP_A32;
+    pn_rhs(ynew, c, u, sc, base, K7, r_tmp, l_tmp);
+    base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
 #pragma unroll
-        for (int i = 0; i < 10; ++i) ys[i] = pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i]));
-        pn_rhs(ys, c, base, k3, r_tmp, l_tmp);
-    }
-    {
-        const real a1 = h * (real)DP_A41, a2 = h * (real)DP_A42, a3 = h * (real)DP_A43;
-#pragma unroll
-        for (int i = 0; i < 10; ++i) ys[i] = pn_fma(a3, k3[i], pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i])));
-        pn_rhs(ys, c, base, k4, r_tmp, l_tmp);
-    }
-    {
-        const real a1 = h * (real)DP_A51, a2 = h * (real)DP_A52, a3 = h * (real)DP_A53, a4 = h * (real)DP_A54;
-#pragma unroll
-        for (int i = 0; i < 10; ++i)
-            ys[i] = pn_fma(a4, k4[i], pn_fma(a3, k3[i], pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i]))));
-        pn_rhs(ys, c, base, k5, r_tmp, l_tmp);
-    }
-    {
-        const real a1 = h * (real)DP_A61, a2 = h * (real)DP_A62, a3 = h * (real)DP_A63, a4 = h * (real)DP_A64,
-                   a5 = h * (real)DP_A65;
-#pragma unroll
-        for (int i = 0; i < 10; ++i)
-            ys[i] = pn_fma(a5, k5[i],
-                           pn_fma(a4, k4[i], pn_fma(a3, k3[i], pn_fma(a2, k2[i], pn_fma(a1, k1[i], y[i])))));
-        pn_rhs(ys, c, base, k6, r_tmp, l_tmp);
-    }
-    {
-        const real b1 = h * (real)DP_B1, b3 = h * (real)DP_B3, b4 = h * (real)DP_B4, b5 = h * (real)DP_B5,
-                   b6 = h * (real)DP_B6;
-        const real e1 = h * (real)DP_E1, e3 = h * (real)DP_E3, e4 = h * (real)DP_E4, e5 = h * (real)DP_E5,
-                   e6 = h * (real)DP_E6;
-#pragma unroll
-        for (int i = 0; i < 10; ++i) {
-            ynew[i] = pn_fma(b6, k6[i], pn_fma(b5, k5[i], pn_fma(b4, k4[i], pn_fma(b3, k3[i], pn_fma(b1, k1[i], y[i])))));
-            err[i] = pn_fma(e6, k6[i], pn_fma(e5, k5[i], pn_fma(e4, k4[i], pn_fma(e3, k3[i], e1 * k1[i]))));
-        }
-        pn_rhs(ynew, c, base, k7, r_tmp, l_tmp);
-        base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
-        const real e7 = h * (real)DP_E7;
-#pragma unroll
-        for (int i = 0; i < 10; ++i) err[i] = pn_fma(e7, k7[i], err[i]);
-    }
+    for (int i = 0; i < 10; ++i) err[i] = pn_fma((real)DP_E7, K7[i], err[i]);
 }

@@ -7,7 +7,8 @@
 // cost only the short refill section.  All state (y, k1..k7, per-system constants) lives in
 // registers; global memory is touched only at refill and at finish.  (DESIGN.md 2, 7.)
 #include <cfloat>
-#include "pn_dp5.cuh"
+#include <cstdlib>
+#include "pn_dp5_smem.cuh"
 #include "pn_internal.h"
 
 #define PN_ST_EINVAL 1
@@ -51,22 +52,29 @@ __device__ __forceinline__ void pn_store_result(const PnKernelParams& p, int idx
     if (p.rejected) p.rejected[idx] = nrej;
 }
 
-template <typename real, int BLOCK, int MINB>
+// SMEM = true (FP64 only): k2..k5 and the error partial live in dynamic shared memory (pn_dp5_smem.cuh)
+template <typename real, int BLOCK, int MINB, bool SMEM>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
 {
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+    extern __shared__ double pn_dyn_smem[];
+    PnSmem<BLOCK> sm;
+    sm.addr = SMEM ? (unsigned)__cvta_generic_to_shared(pn_dyn_smem) + threadIdx.x * 8u : 0u;
 
     // lane state; idle lanes carry a benign dummy system so that the lock-step arithmetic stays finite
     real y[10], k1[10];
     PnConsts<real> c;
     PnBase<real> base;
+    PnUni<real> u;
+    pn_make_uni<real>(p.mask, u);
     pn_make_consts<real>(0.5, 0.5, 0u, c);
 #pragma unroll
     for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; }
     y[0] = (real)0.01; y[9] = (real)1;
     pn_base_init(c.M * y[0], base);
-    real h = (real)1, atS1 = (real)p.atol, atS2 = (real)p.atol;
+    real h = (real)0;
+    float atS1 = (float)p.atol, atS2 = (float)p.atol;
     double t = 0.0;
     int idx = -1, steps = 0, nrej = 0, nland = 0;
     bool after_reject = false, landing = false;
@@ -76,7 +84,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     const real omegaf = (real)p.omegaf;
     const real om_hi = (real)(p.omegaf * (1.0 + p.tau));
     const real om_tol = (real)(p.tau * p.omegaf);
-    const real rtol = (real)p.rtol, atol1 = (real)p.atol;
+    const float rtol = (float)p.rtol, atol1 = (float)p.atol;
 
     for (;;) {
         // ---------------- refill: lanes without a system pull the next queue entries ----------------
@@ -106,18 +114,23 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                             ++tot_fail;
                             y[0] = (real)0.01;   // keep the dummy arithmetic benign
                             pn_base_init(c.M * y[0], base);
+                            h = (real)0;
+#pragma unroll
+                            for (int j = 0; j < 10; ++j) k1[j] = (real)0;
                         } else {
                             idx = i;
                             pn_make_consts<real>(m1, m2, p.mask, c);
                             pn_base_init(c.M * y[0], base);
-                            real r_tmp, l_tmp;
-                            pn_rhs(y, c, base, k1, r_tmp, l_tmp);
                             h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
+                            real r_tmp, l_tmp;
+                            PnScaled<real> sc;
+                            pn_make_scaled(c, h, sc);
+                            pn_rhs(y, c, u, sc, base, k1, r_tmp, l_tmp);      // K1 = h f(y0)
                             // atol scaled by the conserved spin norms (R7)
                             double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
                             double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
-                            atS1 = (real)(p.atol * (s1 > 0.0 ? s1 : 1.0));
-                            atS2 = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
+                            atS1 = (float)(p.atol * (s1 > 0.0 ? s1 : 1.0));
+                            atS2 = (float)(p.atol * (s2 > 0.0 ? s2 : 1.0));
                         }
                     }
                 }
@@ -133,72 +146,85 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
             if (code) {
                 pn_store_result(p, idx, y, code, t, nrej);
                 atomicMax(p.status, PN_ST_ENOTCONVERGED);
-                ++tot_fail; idx = -1; h = (real)1;
+                ++tot_fail; idx = -1; h = (real)0;
+#pragma unroll
+                for (int i = 0; i < 10; ++i) k1[i] = (real)0;
             }
         }
 
-        // ---------------- one DP5(4) trial step, all lanes ----------------
+        // ---------------- one DP5(4) trial step, all lanes (k1, k7 hold the SCALED slopes h*f) ----------------
         real ynew[10], k7[10], err[10];
         PnBase<real> base_new;
-        pn_dp5_trial(y, k1, h, c, base, ynew, k7, err, base_new);
+        if constexpr (SMEM) pn_dp5_trial_smem<BLOCK>(y, k1, h, c, u, base, sm, ynew, k7, err, base_new);
+        else pn_dp5_trial(y, k1, h, c, u, base, ynew, k7, err, base_new);
 
-        // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|)
-        real sum = (real)0;
+        // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|).
+        // Evaluated in FP32 in both precisions: it only decides accept/reject and the next step size, a
+        // relative accuracy of 1e-7 is ample, and the F64->F32 conversions run on the otherwise idle
+        // conversion unit instead of ~65 instructions on the FP64 pipe.
+        float sum = 0.0f;
 #pragma unroll
         for (int i = 0; i < 10; ++i) {
-            const real at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
-            const real sc = pn_fma(rtol, pn_max(pn_abs(y[i]), pn_abs(ynew[i])), at);
-            const real q = pn_ratio(err[i], sc);
-            sum = pn_fma(q, q, sum);
+            const float at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
+            const float scl = fmaxf(fmaf(rtol, fmaxf(fabsf((float)y[i]), fabsf((float)ynew[i])), at), 1e-37f);
+            const float q = __fdividef((float)err[i], scl);
+            sum = fmaf(q, q, sum);
         }
-        const real E2 = sum * (real)0.1;      // E^2; accept iff E^2 <= 1
+        const float E2 = sum * 0.1f;      // E^2; accept iff E^2 <= 1
 
+        // ---------------- per-lane decision: ratio = h_next / h, accept or keep ----------------
+        bool accept = false;
+        real ratio = (real)0;             // idle lanes are frozen: h = 0, K1 = 0
         if (idx >= 0) {
             ++steps; ++tot_steps;
-            if (!(E2 <= PnLimits<real>::huge())) {       // NaN or inf
+            if (!(E2 <= FLT_MAX)) {       // NaN or inf
                 pn_store_result(p, idx, y, PN_F_NONFINITE, t, nrej);
                 atomicMax(p.status, PN_ST_ENONFINITE);
-                ++tot_fail; idx = -1; h = (real)1;
+                ++tot_fail; idx = -1;
             } else {
-                const float fac = pn_ctrl_factor(fmaxf((float)E2, 1e-37f));
-                if (E2 <= (real)1) {
+                const float fac = pn_ctrl_factor(fmaxf(E2, 1e-37f));
+                if (E2 <= 1.0f) {
                     const real om_new = ynew[0];
                     if (om_new > om_hi) {
-                        // passes error control but overshoots omega_f: discard, Newton update of h
-                        // from the same state with d(omega_new)/dh ~ k7[0] (R12)
+                        // passes error control but overshoots omega_f: discard, Newton update of h from the
+                        // same state with d(omega_new)/dh ~ k7[0] = K7[0]/h (R12)
                         ++tot_land; landing = true;
                         if (++nland > 50) {
                             pn_store_result(p, idx, y, PN_F_LANDING, t, nrej);
                             atomicMax(p.status, PN_ST_ENOTCONVERGED);
-                            ++tot_fail; idx = -1; h = (real)1;
+                            ++tot_fail; idx = -1;
                         } else {
-                            const real hn = h - (om_new - omegaf) / k7[0];
-                            h = pn_max(hn, (real)0.1 * h);
+                            ratio = pn_max((real)1 - (om_new - omegaf) / k7[0], (real)0.1);
                         }
                     } else {
-                        // accept
+                        accept = true;
                         t += (double)h;
-#pragma unroll
-                        for (int i = 0; i < 10; ++i) { y[i] = ynew[i]; k1[i] = k7[i]; }
-                        base = base_new;
                         nland = 0;
                         if (pn_abs(om_new - omegaf) <= om_tol) {
-                            pn_store_result(p, idx, y, steps, t, nrej);
-                            idx = -1; h = (real)1;
+                            pn_store_result(p, idx, ynew, steps, t, nrej);
+                            idx = -1;
                         } else if (landing) {
-                            h = pn_min(h, (omegaf - y[0]) / k1[0]);
+                            ratio = pn_min((real)1, (omegaf - om_new) / k7[0]);
                         } else {
-                            h = h * (real)fminf(fmaxf(fac, 0.2f), after_reject ? 1.0f : 5.0f);
+                            ratio = (real)fminf(fmaxf(fac, 0.2f), after_reject ? 1.0f : 5.0f);
                         }
                         after_reject = false;
                     }
                 } else {
                     ++nrej; ++tot_rej;
-                    h = h * (real)fminf(fmaxf(fac, 0.2f), 1.0f);
+                    ratio = (real)fminf(fmaxf(fac, 0.2f), 1.0f);
                     after_reject = true;
                 }
             }
         }
+        // unified update: the kept slope vector is rescaled to the next step size (K1 <- (h'/h) K)
+#pragma unroll
+        for (int i = 0; i < 10; ++i) {
+            k1[i] = ratio * (accept ? k7[i] : k1[i]);
+            y[i] = accept ? ynew[i] : y[i];
+        }
+        if (accept) base = base_new;
+        h *= ratio;
     }
 
     // ---------------- per-launch counters: warp reduce, one atomic per warp ----------------
@@ -238,14 +264,18 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
     PnConsts<real> c;
     pn_make_consts<real>(m1, m2, p.mask, c);
     PnBase<real> base, base_new;
+    PnUni<real> u;
+    pn_make_uni<real>(p.mask, u);
     pn_base_init(c.M * y[0], base);
-    real r_tmp, l_tmp;
-    pn_rhs(y, c, base, k1, r_tmp, l_tmp);
     const real h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
+    real r_tmp, l_tmp;
+    PnScaled<real> sc;
+    pn_make_scaled(c, h, sc);
+    pn_rhs(y, c, u, sc, base, k1, r_tmp, l_tmp);
     double t = 0.0;
     for (int s = 0; s < p.fixed_steps; ++s) {
         real ynew[10], k7[10], err[10];
-        pn_dp5_trial(y, k1, h, c, base, ynew, k7, err, base_new);
+        pn_dp5_trial(y, k1, h, c, u, base, ynew, k7, err, base_new);
         base = base_new;
 #pragma unroll
         for (int j = 0; j < 10; ++j) { y[j] = ynew[j]; k1[j] = k7[j]; }
@@ -257,21 +287,27 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
 
 unsigned long long g_pn_launches = 0;
 
-template <typename real, int BLOCK, int MINB>
+template <typename real, int BLOCK, int MINB, bool SMEM>
 static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
+    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM>;
+    const int shm = SMEM ? PN_SM_SLOTS * BLOCK * (int)sizeof(double) : 0;
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pn_integrate_adaptive_kernel<real, BLOCK, MINB>,
-                                                           BLOCK, 0)) != cudaSuccess) return e;
+    if (SMEM) {
+        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, shm)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                      cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
+    }
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BLOCK, shm)) != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     int grid = grid_blocks > 0 ? grid_blocks : sms * per_sm;
     const long long need = ((long long)p.n + BLOCK - 1) / BLOCK;
     if (need < grid) grid = (int)need;
     if (grid < 1) grid = 1;
-    pn_integrate_adaptive_kernel<real, BLOCK, MINB><<<grid, BLOCK, 0, s>>>(p);
+    kern<<<grid, BLOCK, shm, s>>>(p);
     ++g_pn_launches;
     return cudaGetLastError();
 }
@@ -289,9 +325,11 @@ cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int bloc
         return cudaGetLastError();
     }
     if (precision == 0) {
-        if (block_threads == 256) return launch_adaptive<double, 256, 1>(p, grid_blocks, s);
-        return launch_adaptive<double, 128, 2>(p, grid_blocks, s);
+        if (block_threads == 256) return launch_adaptive<double, 256, 1, false>(p, grid_blocks, s);
+        const char* v = getenv("PN_DEV_VARIANT");   // development switch, not part of the ABI
+        if (v && v[0] == 'r') return launch_adaptive<double, 128, 2, false>(p, grid_blocks, s);
+        return launch_adaptive<double, 128, 3, true>(p, grid_blocks, s);
     }
-    if (block_threads == 128) return launch_adaptive<float, 128, 4>(p, grid_blocks, s);
-    return launch_adaptive<float, 256, 2>(p, grid_blocks, s);
+    if (block_threads == 128) return launch_adaptive<float, 128, 4, false>(p, grid_blocks, s);
+    return launch_adaptive<float, 256, 2, false>(p, grid_blocks, s);
 }

@@ -3,11 +3,10 @@
 // Eqs. (1)-(4) of arXiv:0908.3889 rewritten for the device:
 //   x = M omega, v = x^{1/3};  everything that depends only on (m1, m2) is folded once per system into
 //   PnConsts, the brace of Eq. (1) becomes a Horner polynomial in v whose v^3, v^4 and v^6 coefficients
-//   carry the spin-orbit, spin-spin and log terms, and the three cross products L x S1, L x S2, S2 x S1
-//   are shared between Eq. (2) and Eq. (3):
-//     S1_dot = alpha1 (L x S1) + beta (S2 x S1),   alpha_i = A_i v^5 - 3 beta (L.S_j),  beta = x^2/(2 M^3)
-//     S2_dot = alpha2 (L x S2) - beta (S2 x S1)
-//     L_dot  = -v/(eta M^2) [alpha1 (L x S1) + alpha2 (L x S2)]      (the beta pieces cancel in the sum)
+//   carry the spin-orbit, spin-spin and log terms, and Eq. (4) collapses to
+//     Omega_1 = alpha1 L + beta S2,   alpha_i = A_i v^5 - 3 beta (L.S_j),  beta = x^2/(2 M^3)
+//     Omega_2 = alpha2 L + beta S1
+//   followed by the two cross products of Eq. (2) and L_dot = -v/(eta M^2) (S1_dot + S2_dot) of Eq. (3).
 // This file shares nothing with oracle/ (which evaluates the equations as printed).
 #pragma once
 #include <cuda_runtime.h>
@@ -29,8 +28,7 @@ __device__ __forceinline__ float pn_min(float a, float b) { return fminf(a, b); 
 template <typename real>
 struct PnConsts {
     real M;        // m1 + m2
-    real c0, c2, c3, c4, c5, c6, c7;  // spin-independent coefficients of v^k in the brace of Eq. (1)
-    real cl;       // coefficient of ln(x) inside the v^6 term: -(856/105)(2/3)
+    real c2, c4, c5, c6, c7;  // spin-independent, mass-dependent coefficients of v^k in the brace of Eq. (1)
     real p1, p2;   // spin-orbit: v^3 coefficient += p1 (L.S1) + p2 (L.S2)
     real q1, q2;   // spin-spin:  v^4 coefficient += q1 (S1.S2) + q2 (L.S1)(L.S2)
     real K0;       // omega_dot = K0 v^11 brace,  K0 = 96 eta / (5 M^2)
@@ -38,6 +36,23 @@ struct PnConsts {
     real Bc;       // beta = Bc x^2,  Bc = 1/(2 M^3)
     real G;        // L_dot prefactor: -1/(eta M^2), times v
 };
+
+// Coefficients that depend only on term_mask: the same for every system of a launch, so they stay out of the
+// per-lane register budget (warp-uniform values).
+template <typename real>
+struct PnUni {
+    real c0;   // the "1" of the brace
+    real c3;   // 4 pi, spin-independent part of the v^3 coefficient
+    real cl;   // coefficient of ln(x) inside the v^6 term: -(856/105)(2/3)
+};
+template <typename real>
+__device__ __forceinline__ void pn_make_uni(unsigned mask, PnUni<real>& u)
+{
+    if (mask == 0) mask = PN_MASK_ALL;
+    u.c0 = (real)((mask >> 0) & 1u ? 1.0 : 0.0);
+    u.c3 = (real)((mask >> 3) & 1u ? 4.0 * 3.14159265358979323846 : 0.0);
+    u.cl = (real)((mask >> 6) & 1u ? -(856.0 / 105.0) * (2.0 / 3.0) : 0.0);
+}
 
 template <typename real>
 __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned mask, PnConsts<real>& c)
@@ -49,9 +64,7 @@ __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned ma
     const double spin = (mask & PN_MASK_SPIN) ? 1.0 : 0.0;
     auto on = [&](int k) { return (mask >> k) & 1u ? 1.0 : 0.0; };
     c.M = (real)M;
-    c.c0 = (real)on(0);
     c.c2 = (real)(on(2) * (-(743.0 + 924.0 * eta) / 336.0));
-    c.c3 = (real)(on(3) * (4.0 * pi));
     c.c4 = (real)(on(4) * (34103.0 / 18144.0 + (13661.0 / 2016.0) * eta + (59.0 / 18.0) * eta * eta));
     c.c5 = (real)(on(5) * (-(4159.0 + 15876.0 * eta) * pi / 672.0));
     // theta^ enters linearly in eta (R1); ln(16 x^{2/3}) = ln 16 + (2/3) ln x, natural log (R2)
@@ -60,7 +73,6 @@ __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned ma
                            (-273811877.0 / 1088640.0 + (451.0 / 48.0) * pi * pi - (88.0 / 3.0) * theta) * eta +
                            (541.0 / 896.0) * eta * eta - (5605.0 / 2592.0) * eta * eta * eta -
                            (856.0 / 105.0) * 2.772588722239781237669 /* ln 16 */));
-    c.cl = (real)(on(6) * (-(856.0 / 105.0) * (2.0 / 3.0)));
     c.c7 = (real)(on(7) * ((-4415.0 / 4032.0 + (358675.0 / 6048.0) * eta + (91495.0 / 1512.0) * eta * eta) * pi));
     const double w1 = 113.0 * m1 * m1 / M2 + 75.0 * eta, w2 = 113.0 * m2 * m2 / M2 + 75.0 * eta;
     c.p1 = (real)(-on(3) * spin * w1 / (12.0 * m1 * m1));
@@ -132,10 +144,24 @@ __device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float& 
     r = 0.0f;
 }
 
-// f = RHS(y).  ~75 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and
+// The slopes are produced already multiplied by the step size h ("scaled slopes" K = h f): the four
+// prefactors that enter every output linearly are pre-multiplied by h once per trial step, which costs
+// nothing per evaluation and lets every stage sum of the stepper use compile-time tableau coefficients
+// (constant-bank operands) instead of per-lane h*a_sj registers.  This matters on sm_100a because a DFMA
+// with three distinct register sources issues every 3 cycles, one with two every 2 (measured,
+// DESIGN.md 7.2).
+template <typename real> struct PnScaled { real hK0, hA1, hA2, hBc; };
+template <typename real>
+__device__ __forceinline__ void pn_make_scaled(const PnConsts<real>& c, real h, PnScaled<real>& s)
+{
+    s.hK0 = h * c.K0; s.hA1 = h * c.A1; s.hA2 = h * c.A2; s.hBc = h * c.Bc;
+}
+
+// K = h f(y).  ~70 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and
 // lnx_out = ln x of this evaluation are handed back for the base update of an accepted step.
 template <typename real>
-__device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, const PnBase<real>& base,
+__device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, const PnUni<real>& u,
+                                       const PnScaled<real>& sc, const PnBase<real>& base,
                                        real (&f)[10], real& r_out, real& lnx_out)
 {
     const real x = c.M * y[0];
@@ -153,41 +179,34 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     const real S12 = pn_fma(S1x, S2x, pn_fma(S1y, S2y, S1z * S2z));
 
     // Eq. (1): Horner in v; coefficients of v^3, v^4, v^6 carry the spin-orbit, spin-spin, log pieces
-    const real k3 = pn_fma(c.p1, LS1, pn_fma(c.p2, LS2, c.c3));
+    const real k3 = pn_fma(c.p1, LS1, pn_fma(c.p2, LS2, u.c3));
     const real k4 = pn_fma(c.q1, S12, pn_fma(c.q2 * LS1, LS2, c.c4));
-    const real k6 = pn_fma(c.cl, lnx, c.c6);
+    const real k6 = pn_fma(u.cl, lnx, c.c6);
     real B = pn_fma(c.c7, v, k6);
     B = pn_fma(B, v, c.c5);
     B = pn_fma(B, v, k4);
     B = pn_fma(B, v, k3);
     B = pn_fma(B, v, c.c2);
-    B = pn_fma(B, v2, c.c0);
-    f[0] = (c.K0 * (v5 * x2)) * B;
+    B = pn_fma(B, v2, u.c0);
+    f[0] = (sc.hK0 * (v5 * x2)) * B;
 
-    // Eq. (4),(2): shared cross products
-    const real beta = c.Bc * x2;
+    // Eq. (4): h Omega_1 = al1 L + beta S2,  h Omega_2 = al2 L + beta S1
+    const real beta = sc.hBc * x2;
     const real b3 = (real)3.0 * beta;
-    const real al1 = pn_fma(-b3, LS2, c.A1 * v5);
-    const real al2 = pn_fma(-b3, LS1, c.A2 * v5);
-    // u1 = alpha1 (L x S1), u2 = alpha2 (L x S2), w = beta (S2 x S1)
-    const real u1x = al1 * pn_fma(Ly, S1z, -(Lz * S1y));
-    const real u1y = al1 * pn_fma(Lz, S1x, -(Lx * S1z));
-    const real u1z = al1 * pn_fma(Lx, S1y, -(Ly * S1x));
-    const real u2x = al2 * pn_fma(Ly, S2z, -(Lz * S2y));
-    const real u2y = al2 * pn_fma(Lz, S2x, -(Lx * S2z));
-    const real u2z = al2 * pn_fma(Lx, S2y, -(Ly * S2x));
-    const real wx = pn_fma(S2y, S1z, -(S2z * S1y));
-    const real wy = pn_fma(S2z, S1x, -(S2x * S1z));
-    const real wz = pn_fma(S2x, S1y, -(S2y * S1x));
-    f[1] = pn_fma(beta, wx, u1x);
-    f[2] = pn_fma(beta, wy, u1y);
-    f[3] = pn_fma(beta, wz, u1z);
-    f[4] = pn_fma(-beta, wx, u2x);
-    f[5] = pn_fma(-beta, wy, u2y);
-    f[6] = pn_fma(-beta, wz, u2z);
+    const real al1 = pn_fma(-b3, LS2, sc.hA1 * v5);
+    const real al2 = pn_fma(-b3, LS1, sc.hA2 * v5);
+    const real O1x = pn_fma(beta, S2x, al1 * Lx), O1y = pn_fma(beta, S2y, al1 * Ly), O1z = pn_fma(beta, S2z, al1 * Lz);
+    const real O2x = pn_fma(beta, S1x, al2 * Lx), O2y = pn_fma(beta, S1y, al2 * Ly), O2z = pn_fma(beta, S1z, al2 * Lz);
+    // Eq. (2): S_i_dot = Omega_i x S_i
+    f[1] = pn_fma(O1y, S1z, -(O1z * S1y));
+    f[2] = pn_fma(O1z, S1x, -(O1x * S1z));
+    f[3] = pn_fma(O1x, S1y, -(O1y * S1x));
+    f[4] = pn_fma(O2y, S2z, -(O2z * S2y));
+    f[5] = pn_fma(O2z, S2x, -(O2x * S2z));
+    f[6] = pn_fma(O2x, S2y, -(O2y * S2x));
     // Eq. (3)
     const real g = c.G * v;
-    f[7] = g * (u1x + u2x);
-    f[8] = g * (u1y + u2y);
-    f[9] = g * (u1z + u2z);
+    f[7] = g * (f[1] + f[4]);
+    f[8] = g * (f[2] + f[5]);
+    f[9] = g * (f[3] + f[6]);
 }
