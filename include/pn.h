@@ -130,6 +130,10 @@ int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* s
 int pn_last_counters(unsigned long long* trial_steps, unsigned long long* rejected,
                      unsigned long long* landing_trials, unsigned long long* failed);
 
+/* FP64 only: number of systems of the last synchronous pn_integrate* call that were re-integrated by the
+ * wide-range redo pass because one of their steps changed omega by more than 3 %. */
+unsigned long long pn_last_redo_count(void);
+
 /* Duration in milliseconds of the kernels of the last synchronous pn_integrate* / pn_histogram* call,
  * measured with CUDA events on the call's stream: [0] stage-in, [1] integrator, [2] stage-out,
  * [3] histogram.  Entries a call did not run are left unchanged. */

@@ -19,7 +19,7 @@ PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
 EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_stream_status",
-           "pn_measure_fma_peak", "pn_last_counters", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
+           "pn_measure_fma_peak", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
 
@@ -57,6 +57,7 @@ def load():
         lib.pn_last_counters.argtypes = [C.POINTER(C.c_ulonglong)] * 4
         lib.pn_last_kernel_ms.argtypes = [C.POINTER(C.c_float)]
         lib.pn_launch_count.restype = C.c_ulonglong
+        lib.pn_last_redo_count.restype = C.c_ulonglong
         lib.pn_strerror.argtypes = [i]
         lib.pn_strerror.restype = C.c_char_p
         lib.pn_last_cuda_error.restype = C.c_char_p
@@ -143,7 +144,8 @@ def pn_measure_fma_peak(precision=PN_FP64, seconds=0.25):
 def pn_last_counters():
     v = [C.c_ulonglong(0) for _ in range(4)]
     load().pn_last_counters(*[C.byref(x) for x in v])
-    return dict(trial_steps=v[0].value, rejected=v[1].value, landing_trials=v[2].value, failed=v[3].value)
+    return dict(trial_steps=v[0].value, rejected=v[1].value, landing_trials=v[2].value, failed=v[3].value,
+                redo=int(load().pn_last_redo_count()))
 
 
 def pn_last_kernel_ms():

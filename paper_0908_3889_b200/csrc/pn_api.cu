@@ -39,15 +39,16 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
 static cudaEvent_t g_ev[5];
 static bool g_ev_ok = false;
 static float g_ms[4] = {0, 0, 0, 0};
 static unsigned long long g_counters[4] = {0, 0, 0, 0};
+static unsigned g_redo_count = 0;   // systems that went through the redo pass in the last synchronous call
 static std::map<void*, int> g_stream_status;
 
 // layout of g_small: [0..3] counters (u64), then queue (u32), status (i32)
-struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned long long skipped[3]; };
+struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned int queue2; unsigned int redo_count; unsigned long long skipped[3]; };
 
 static int ensure_events()
 {
@@ -137,7 +138,9 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
     p.fixed_steps = fixed ? o.fixed_steps : 0;
     p.mask = o.term_mask;
+    if ((rc = g_redo.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
     p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
+    p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = (int*)g_redo.p;
     CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s));
     CK(cudaEventRecord(g_ev[2], s));
     if (o.layout == 0) CK(pn_launch_soa_to_aos((const double*)g_soa_out.p, d_final, n, 10, s));
@@ -160,6 +163,7 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     CK(cudaGetLastError());
     for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&g_ms[i], g_ev[i], g_ev[i + 1]));
     memcpy(g_counters, hs.counters, sizeof g_counters);
+    g_redo_count = hs.redo_count;
     return hs.status;
 }
 
@@ -251,6 +255,8 @@ extern "C" int pn_last_counters(unsigned long long* trial_steps, unsigned long l
     return PN_OK;
 }
 
+extern "C" unsigned long long pn_last_redo_count(void) { return g_redo_count; }
+
 extern "C" int pn_last_kernel_ms(float ms[4])
 {
     if (!ms) return PN_EINVAL;
@@ -277,7 +283,7 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
     for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
     if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
     g_stream_status.clear();

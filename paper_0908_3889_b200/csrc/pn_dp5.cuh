@@ -40,10 +40,10 @@
 // Trial step from (y, K1 = h f(y)) with step h.  All slopes are "scaled" (K_s = h k_s, see pn_rhs.cuh), so
 // every coefficient below is a compile-time constant.  Outputs y_new (5th order), K7 = h f(y_new) and the
 // error estimate err = sum_s e_s K_s.  6 RHS evaluations, 200 + 60 FMAs.
-template <typename real>
+template <bool SLOW, typename real>
 __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K1)[10], real h,
                                              const PnConsts<real>& c, const PnUni<real>& u, const PnBase<real>& base,
-                                             real (&ynew)[10], real (&K7)[10], real (&err)[10], PnBase<real>& base_new)
+                                             real (&ynew)[10], real (&K7)[10], real (&err)[10], PnBase<real>& base_new, bool& bad)
 {
     real K2[10], K3[10], K4[10], K5[10], K6[10], ys[10];
     real r_tmp, l_tmp;
@@ -51,25 +51,25 @@ __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K
     pn_make_scaled(c, h, sc);
 #pragma unroll
     for (int i = 0; i < 10; ++i) ys[i] = pn_fma((real)DP_A21, K1[i], y[i]);
-    pn_rhs(ys, c, u, sc, base, K2, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ys, c, u, sc, base, K2, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < 10; ++i) ys[i] = pn_fma((real)DP_A32, K2[i], pn_fma((real)DP_A31, K1[i], y[i]));
-    pn_rhs(ys, c, u, sc, base, K3, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ys, c, u, sc, base, K3, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < 10; ++i)
         ys[i] = pn_fma((real)DP_A43, K3[i], pn_fma((real)DP_A42, K2[i], pn_fma((real)DP_A41, K1[i], y[i])));
-    pn_rhs(ys, c, u, sc, base, K4, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ys, c, u, sc, base, K4, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < 10; ++i)
         ys[i] = pn_fma((real)DP_A54, K4[i],
                        pn_fma((real)DP_A53, K3[i], pn_fma((real)DP_A52, K2[i], pn_fma((real)DP_A51, K1[i], y[i]))));
-    pn_rhs(ys, c, u, sc, base, K5, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ys, c, u, sc, base, K5, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < 10; ++i)
         ys[i] = pn_fma((real)DP_A65, K5[i],
                        pn_fma((real)DP_A64, K4[i],
                               pn_fma((real)DP_A63, K3[i], pn_fma((real)DP_A62, K2[i], pn_fma((real)DP_A61, K1[i], y[i])))));
-    pn_rhs(ys, c, u, sc, base, K6, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ys, c, u, sc, base, K6, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         ynew[i] = pn_fma((real)DP_B6, K6[i],
@@ -79,7 +79,7 @@ __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K
                         pn_fma((real)DP_E5, K5[i],
                                pn_fma((real)DP_E4, K4[i], pn_fma((real)DP_E3, K3[i], (real)DP_E1 * K1[i]))));
     }
-    pn_rhs(ynew, c, u, sc, base, K7, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ynew, c, u, sc, base, K7, r_tmp, l_tmp, bad);
     base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
 #pragma unroll
     for (int i = 0; i < 10; ++i) err[i] = pn_fma((real)DP_E7, K7[i], err[i]);

@@ -34,11 +34,11 @@ struct PnSmem {
     }
 };
 
-template <int BLOCK>
+template <bool SLOW, int BLOCK>
 __device__ __forceinline__ void pn_dp5_trial_smem(const double (&y)[10], const double (&K1)[10], double h,
                                                   const PnConsts<double>& c, const PnUni<double>& u, const PnBase<double>& base,
                                                   const PnSmem<BLOCK>& sm, double (&ynew)[10], double (&K7)[10],
-                                                  double (&err)[10], PnBase<double>& base_new)
+                                                  double (&err)[10], PnBase<double>& base_new, bool& bad)
 {
     double ys[10], kf[10];   // stage argument, freshest (scaled) slope vector
     double r_tmp, l_tmp;
@@ -46,25 +46,25 @@ __device__ __forceinline__ void pn_dp5_trial_smem(const double (&y)[10], const d
     pn_make_scaled(c, h, sc);
 #pragma unroll
     for (int i = 0; i < 10; ++i) ys[i] = fma(DP_A21, K1[i], y[i]);
-    pn_rhs(ys, c, u, sc, base, kf, r_tmp, l_tmp);              // kf = K2
+    pn_rhs<SLOW>(ys, c, u, sc, base, kf, r_tmp, l_tmp, bad);              // kf = K2
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         sm.st(PN_SM_K2 + i, kf[i]);
         ys[i] = fma(DP_A32, kf[i], fma(DP_A31, K1[i], y[i]));
     }
-    pn_rhs(ys, c, u, sc, base, kf, r_tmp, l_tmp);              // kf = K3
+    pn_rhs<SLOW>(ys, c, u, sc, base, kf, r_tmp, l_tmp, bad);              // kf = K3
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         sm.st(PN_SM_K3 + i, kf[i]);
         ys[i] = fma(DP_A43, kf[i], fma(DP_A42, sm.ld(PN_SM_K2 + i), fma(DP_A41, K1[i], y[i])));
     }
-    pn_rhs(ys, c, u, sc, base, kf, r_tmp, l_tmp);              // kf = K4
+    pn_rhs<SLOW>(ys, c, u, sc, base, kf, r_tmp, l_tmp, bad);              // kf = K4
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         sm.st(PN_SM_K4 + i, kf[i]);
         ys[i] = fma(DP_A54, kf[i], fma(DP_A53, sm.ld(PN_SM_K3 + i), fma(DP_A52, sm.ld(PN_SM_K2 + i), fma(DP_A51, K1[i], y[i]))));
     }
-    pn_rhs(ys, c, u, sc, base, kf, r_tmp, l_tmp);              // kf = K5
+    pn_rhs<SLOW>(ys, c, u, sc, base, kf, r_tmp, l_tmp, bad);              // kf = K5
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         sm.st(PN_SM_K5 + i, kf[i]);
@@ -72,7 +72,7 @@ __device__ __forceinline__ void pn_dp5_trial_smem(const double (&y)[10], const d
                     fma(DP_A64, sm.ld(PN_SM_K4 + i),
                         fma(DP_A63, sm.ld(PN_SM_K3 + i), fma(DP_A62, sm.ld(PN_SM_K2 + i), fma(DP_A61, K1[i], y[i])))));
     }
-    pn_rhs(ys, c, u, sc, base, kf, r_tmp, l_tmp);              // kf = K6
+    pn_rhs<SLOW>(ys, c, u, sc, base, kf, r_tmp, l_tmp, bad);              // kf = K6
     // stage 7 = 5th-order solution; the error partial is parked while the last RHS runs
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
@@ -80,7 +80,7 @@ __device__ __forceinline__ void pn_dp5_trial_smem(const double (&y)[10], const d
         ynew[i] = fma(DP_B6, kf[i], fma(DP_B5, k5i, fma(DP_B4, k4i, fma(DP_B3, k3i, fma(DP_B1, K1[i], y[i])))));
         sm.st(PN_SM_ERR + i, fma(DP_E6, kf[i], fma(DP_E5, k5i, fma(DP_E4, k4i, fma(DP_E3, k3i, DP_E1 * K1[i])))));
     }
-    pn_rhs(ynew, c, u, sc, base, K7, r_tmp, l_tmp);
+    pn_rhs<SLOW>(ynew, c, u, sc, base, K7, r_tmp, l_tmp, bad);
     base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
 #pragma unroll
     for (int i = 0; i < 10; ++i) err[i] = fma(DP_E7, K7[i], sm.ld(PN_SM_ERR + i));

@@ -52,17 +52,28 @@ __device__ __forceinline__ void pn_store_result(const PnKernelParams& p, int idx
     if (p.rejected) p.rejected[idx] = nrej;
 }
 
+// FP32 helpers without the denormal-range fix-up code the CUDA intrinsics carry (inputs are clamped).
+__device__ __forceinline__ float pn_rcp_f(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ float pn_lg2_f(float a) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ float pn_ex2_f(float a) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+
 // SMEM = true (FP64 only): k2..k5 and the error partial live in dynamic shared memory (pn_dp5_smem.cuh)
-template <typename real, int BLOCK, int MINB, bool SMEM>
+// SLOW = true: the redo pass.  Systems whose step left the range of the cbrt/log series in the fast kernel
+// are re-integrated from their initial state with the wide-range evaluation (pn_rhs.cuh) in every stage.
+template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
 {
+    const unsigned n_queue = SLOW ? *p.redo_count : (unsigned)p.n;     // length of the work queue
+    const int* order = SLOW ? p.redo_list : p.order;
+    if (SLOW && n_queue == 0u) return;
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     extern __shared__ double pn_dyn_smem[];
     PnSmem<BLOCK> sm;
     sm.addr = SMEM ? (unsigned)__cvta_generic_to_shared(pn_dyn_smem) + threadIdx.x * 8u : 0u;
 
-    // lane state; idle lanes carry a benign dummy system so that the lock-step arithmetic stays finite
+    // lane state.  k1 holds the SCALED slope h*f(y).  Idle lanes are frozen (h = 0, k1 = 0) on a benign
+    // dummy state, so the lock-step arithmetic stays finite and never leaves the series' range.
     real y[10], k1[10];
     PnConsts<real> c;
     PnBase<real> base;
@@ -88,75 +99,70 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
 
     for (;;) {
         // ---------------- refill: lanes without a system pull the next queue entries ----------------
-        if (!queue_empty) {
+        if (!queue_empty && __any_sync(FULL, idx < 0)) {
             const unsigned wm = __ballot_sync(FULL, idx < 0);
-            if (wm) {
-                const int leader = __ffs(wm) - 1;
-                unsigned qbase = 0;
-                if (lane == leader) qbase = atomicAdd(p.queue, (unsigned)__popc(wm));
-                qbase = __shfl_sync(FULL, qbase, leader);
-                if (qbase + (unsigned)__popc(wm) >= (unsigned)p.n) queue_empty = true;
-                if (idx < 0) {
-                    const unsigned q = qbase + (unsigned)__popc(wm & ((1u << lane) - 1u));
-                    if (q < (unsigned)p.n) {
-                        const int i = p.order ? p.order[q] : (int)q;
-                        double y0[10];
+            const int leader = __ffs(wm) - 1;
+            unsigned qbase = 0;
+            if (lane == leader) qbase = atomicAdd(SLOW ? p.queue2 : p.queue, (unsigned)__popc(wm));
+            qbase = __shfl_sync(FULL, qbase, leader);
+            if (qbase + (unsigned)__popc(wm) >= n_queue) queue_empty = true;
+            if (idx < 0) {
+                const unsigned q = qbase + (unsigned)__popc(wm & ((1u << lane) - 1u));
+                if (q < n_queue) {
+                    const int i = order ? order[q] : (int)q;
+                    double y0[10];
 #pragma unroll
-                        for (int j = 0; j < 10; ++j) y0[j] = __ldg(p.y0 + (size_t)j * p.n + i);
-                        const double m1 = __ldg(p.masses + i), m2 = __ldg(p.masses + (size_t)p.n + i);
+                    for (int j = 0; j < 10; ++j) y0[j] = __ldg(p.y0 + (size_t)j * p.n + i);
+                    const double m1 = __ldg(p.masses + i), m2 = __ldg(p.masses + (size_t)p.n + i);
+                    if (!(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
+                        (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0))) {
+                        real ybad[10];
+#pragma unroll
+                        for (int j = 0; j < 10; ++j) ybad[j] = (real)y0[j];
+                        pn_store_result(p, i, ybad, PN_F_BADINPUT, 0.0, 0);
+                        atomicMax(p.status, PN_ST_EINVAL);
+                        ++tot_fail;          // the lane stays frozen and asks again next iteration
+                    } else {
 #pragma unroll
                         for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
                         t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
-                        if (!(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
-                            (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0))) {
-                            pn_store_result(p, i, y, PN_F_BADINPUT, 0.0, 0);
-                            atomicMax(p.status, PN_ST_EINVAL);
-                            ++tot_fail;
-                            y[0] = (real)0.01;   // keep the dummy arithmetic benign
-                            pn_base_init(c.M * y[0], base);
-                            h = (real)0;
-#pragma unroll
-                            for (int j = 0; j < 10; ++j) k1[j] = (real)0;
-                        } else {
-                            idx = i;
-                            pn_make_consts<real>(m1, m2, p.mask, c);
-                            pn_base_init(c.M * y[0], base);
-                            h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
-                            real r_tmp, l_tmp;
-                            PnScaled<real> sc;
-                            pn_make_scaled(c, h, sc);
-                            pn_rhs(y, c, u, sc, base, k1, r_tmp, l_tmp);      // K1 = h f(y0)
-                            // atol scaled by the conserved spin norms (R7)
-                            double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
-                            double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
-                            atS1 = (float)(p.atol * (s1 > 0.0 ? s1 : 1.0));
-                            atS2 = (float)(p.atol * (s2 > 0.0 ? s2 : 1.0));
-                        }
+                        idx = i;
+                        pn_make_consts<real>(m1, m2, p.mask, c);
+                        pn_base_init(c.M * y[0], base);
+                        h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
+                        real r_tmp, l_tmp;
+                        bool bad_tmp = false;
+                        PnScaled<real> sc;
+                        pn_make_scaled(c, h, sc);
+                        pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad_tmp);      // K1 = h f(y0)
+                        // atol scaled by the conserved spin norms (R7)
+                        double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
+                        double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
+                        atS1 = (float)(p.atol * (s1 > 0.0 ? s1 : 1.0));
+                        atS2 = (float)(p.atol * (s2 > 0.0 ? s2 : 1.0));
                     }
                 }
             }
         }
-        if (__all_sync(FULL, idx < 0)) break;
-
-        // ---------------- pre-trial guards (per lane) ----------------
-        if (idx >= 0) {
-            int code = 0;
-            if (steps >= p.max_steps) code = PN_F_MAXSTEPS;
-            else if (!(pn_abs(h) > PnLimits<real>::tiny()) || t + (double)h == t) code = PN_F_HUNDERFLOW;
-            if (code) {
-                pn_store_result(p, idx, y, code, t, nrej);
-                atomicMax(p.status, PN_ST_ENOTCONVERGED);
-                ++tot_fail; idx = -1; h = (real)0;
-#pragma unroll
-                for (int i = 0; i < 10; ++i) k1[i] = (real)0;
-            }
+        if (__all_sync(FULL, idx < 0)) {
+            if (queue_empty) break;
+            continue;                        // only bad-input lanes were drawn: ask again
         }
 
-        // ---------------- one DP5(4) trial step, all lanes (k1, k7 hold the SCALED slopes h*f) ----------------
+        // ---------------- one DP5(4) trial step, all lanes, one basic block ----------------
         real ynew[10], k7[10], err[10];
         PnBase<real> base_new;
-        if constexpr (SMEM) pn_dp5_trial_smem<BLOCK>(y, k1, h, c, u, base, sm, ynew, k7, err, base_new);
-        else pn_dp5_trial(y, k1, h, c, u, base, ynew, k7, err, base_new);
+        bool bad = false;
+        if constexpr (SMEM) pn_dp5_trial_smem<SLOW, BLOCK>(y, k1, h, c, u, base, sm, ynew, k7, err, base_new, bad);
+        else pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
+        // fast kernel: a lane whose step left the series' range (|1 - x/x0| > 0.03, only at very loose
+        // tolerances) hands its system to the redo pass and frees itself; redo kernel: `bad` means omega more
+        // than doubled inside one step, which is treated as a rejected step.
+        const bool force_reject = SLOW && bad;
+        if (!SLOW && idx >= 0 && bad) {
+            p.redo_list[atomicAdd(p.redo_count, 1u)] = idx;
+            idx = -1;
+        }
 
         // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|).
         // Evaluated in FP32 in both precisions: it only decides accept/reject and the next step size, a
@@ -166,56 +172,58 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
 #pragma unroll
         for (int i = 0; i < 10; ++i) {
             const float at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
-            const float scl = fmaxf(fmaf(rtol, fmaxf(fabsf((float)y[i]), fabsf((float)ynew[i])), at), 1e-37f);
-            const float q = __fdividef((float)err[i], scl);
+            const float scl = fmaxf(fmaf(rtol, fmaxf(fabsf((float)y[i]), fabsf((float)ynew[i])), at), 1e-30f);
+            const float q = (float)err[i] * pn_rcp_f(scl);
             sum = fmaf(q, q, sum);
         }
-        const float E2 = sum * 0.1f;      // E^2; accept iff E^2 <= 1
+        const float E2 = force_reject ? 1e30f : sum * 0.1f;      // E^2; accept iff E^2 <= 1
 
-        // ---------------- per-lane decision: ratio = h_next / h, accept or keep ----------------
-        bool accept = false;
-        real ratio = (real)0;             // idle lanes are frozen: h = 0, K1 = 0
-        if (idx >= 0) {
-            ++steps; ++tot_steps;
-            if (!(E2 <= FLT_MAX)) {       // NaN or inf
-                pn_store_result(p, idx, y, PN_F_NONFINITE, t, nrej);
-                atomicMax(p.status, PN_ST_ENONFINITE);
-                ++tot_fail; idx = -1;
-            } else {
-                const float fac = pn_ctrl_factor(fmaxf(E2, 1e-37f));
-                if (E2 <= 1.0f) {
-                    const real om_new = ynew[0];
-                    if (om_new > om_hi) {
-                        // passes error control but overshoots omega_f: discard, Newton update of h from the
-                        // same state with d(omega_new)/dh ~ k7[0] = K7[0]/h (R12)
-                        ++tot_land; landing = true;
-                        if (++nland > 50) {
-                            pn_store_result(p, idx, y, PN_F_LANDING, t, nrej);
-                            atomicMax(p.status, PN_ST_ENOTCONVERGED);
-                            ++tot_fail; idx = -1;
-                        } else {
-                            ratio = pn_max((real)1 - (om_new - omegaf) / k7[0], (real)0.1);
-                        }
-                    } else {
-                        accept = true;
-                        t += (double)h;
-                        nland = 0;
-                        if (pn_abs(om_new - omegaf) <= om_tol) {
-                            pn_store_result(p, idx, ynew, steps, t, nrej);
-                            idx = -1;
-                        } else if (landing) {
-                            ratio = pn_min((real)1, (omegaf - om_new) / k7[0]);
-                        } else {
-                            ratio = (real)fminf(fmaxf(fac, 0.2f), after_reject ? 1.0f : 5.0f);
-                        }
-                        after_reject = false;
-                    }
-                } else {
-                    ++nrej; ++tot_rej;
-                    ratio = (real)fminf(fmaxf(fac, 0.2f), 1.0f);
-                    after_reject = true;
-                }
+        // ---------------- per-lane decision as straight-line selects ----------------
+        // controller factor 0.9 (E^2)^{-1/10} on the FP32 special-function unit (R8)
+        const float fac = 0.9f * pn_ex2_f(-0.1f * pn_lg2_f(fminf(fmaxf(E2, 1e-30f), 1e30f)));
+        const bool active = idx >= 0;
+        const bool finite = E2 <= FLT_MAX;                 // false for NaN and inf
+        const bool ok = E2 <= 1.0f;
+        const real om_new = ynew[0];
+        const bool over = active && ok && (om_new > om_hi);            // passes error control, overshoots omega_f
+        const bool accept = active && ok && !over;
+        const bool landed = accept && (pn_abs(om_new - omegaf) <= om_tol);
+        const bool reject = active && finite && !ok;
+        real ratio = (real)fminf(fmaxf(fac, 0.2f), (after_reject || reject) ? 1.0f : 5.0f);   // h_next / h
+        if (!active) ratio = (real)0;                      // idle (or just handed to the redo pass): frozen
+        steps += active ? 1 : 0;
+        tot_steps += active ? 1u : 0u;
+        nrej += reject ? 1 : 0;
+        tot_rej += reject ? 1u : 0u;
+        if (accept) t += (double)h;
+        after_reject = reject || (after_reject && !accept);
+        if (over || (accept && landing)) {
+            // landing on omega_f (R12): Newton on h with d(omega_new)/dh ~ k7[0]/h.
+            // over: discard the step and retry from the same state; accepted-short: first guess from the new state
+            const real d = (over ? (om_new - omegaf) : (omegaf - om_new)) / k7[0];
+            ratio = over ? pn_max((real)1 - d, (real)0.1) : pn_min((real)1, d);
+            if (over) { ++tot_land; ++nland; landing = true; }
+        }
+        if (accept) nland = 0;
+        const real h_next = h * ratio;
+        // rare exits: finished, non-finite, landing failure, max_steps, step-size underflow
+        int code = 0;
+        if (active) {
+            if (!finite) code = PN_F_NONFINITE;
+            else if (landed) code = steps;
+            else if (nland > 50) code = PN_F_LANDING;
+            else if (steps >= p.max_steps) code = PN_F_MAXSTEPS;
+            else if (!(pn_abs(h_next) > PnLimits<real>::tiny()) || t + (double)h_next == t) code = PN_F_HUNDERFLOW;
+        }
+        if (code != 0) {
+            if (accept) pn_store_result(p, idx, ynew, code, t, nrej);
+            else pn_store_result(p, idx, y, code, t, nrej);
+            if (code < 0) {
+                atomicMax(p.status, code == PN_F_NONFINITE ? PN_ST_ENONFINITE : PN_ST_ENOTCONVERGED);
+                ++tot_fail;
             }
+            idx = -1;
+            ratio = (real)0;              // freeze the lane
         }
         // unified update: the kept slope vector is rescaled to the next step size (K1 <- (h'/h) K)
 #pragma unroll
@@ -223,7 +231,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
             k1[i] = ratio * (accept ? k7[i] : k1[i]);
             y[i] = accept ? ynew[i] : y[i];
         }
-        if (accept) base = base_new;
+        base.r0 = accept ? base_new.r0 : base.r0;
+        base.r03 = accept ? base_new.r03 : base.r03;
+        base.l0 = accept ? base_new.l0 : base.l0;
         h *= ratio;
     }
 
@@ -244,11 +254,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
 }
 
 // Fixed-step mode (tests, R15): exactly fixed_steps DP5 steps of size h0, y <- y_new.
-template <typename real, int BLOCK>
+// SLOW = true is the redo pass over the systems that left the series' range in the fast pass.
+template <typename real, int BLOCK, bool SLOW>
 __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKernelParams p)
 {
-    const int i = blockIdx.x * BLOCK + threadIdx.x;
-    if (i >= p.n) return;
+    const int q = blockIdx.x * BLOCK + threadIdx.x;
+    const int nq = SLOW ? (int)*p.redo_count : p.n;
+    if (q >= nq) return;
+    const int i = SLOW ? p.redo_list[q] : q;
     double y0[10];
 #pragma unroll
     for (int j = 0; j < 10; ++j) y0[j] = p.y0[(size_t)j * p.n + i];
@@ -271,11 +284,17 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
     real r_tmp, l_tmp;
     PnScaled<real> sc;
     pn_make_scaled(c, h, sc);
-    pn_rhs(y, c, u, sc, base, k1, r_tmp, l_tmp);
+    bool bad = false;
+    pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad);
     double t = 0.0;
     for (int s = 0; s < p.fixed_steps; ++s) {
         real ynew[10], k7[10], err[10];
-        pn_dp5_trial(y, k1, h, c, u, base, ynew, k7, err, base_new);
+        bad = false;
+        pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
+        if (!SLOW && bad) {
+            p.redo_list[atomicAdd(p.redo_count, 1u)] = i;
+            return;
+        }
         base = base_new;
 #pragma unroll
         for (int j = 0; j < 10; ++j) { y[j] = ynew[j]; k1[j] = k7[j]; }
@@ -287,10 +306,10 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
 
 unsigned long long g_pn_launches = 0;
 
-template <typename real, int BLOCK, int MINB, bool SMEM>
+template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW>
 static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
-    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM>;
+    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM, SLOW>;
     const int shm = SMEM ? PN_SM_SLOTS * BLOCK * (int)sizeof(double) : 0;
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t e;
@@ -319,17 +338,26 @@ cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int bloc
     if (p.fixed_steps > 0) {
         const int B = 128;
         const int grid = (p.n + B - 1) / B;
-        if (precision == 0) pn_integrate_fixed_kernel<double, B><<<grid, B, 0, s>>>(p);
-        else pn_integrate_fixed_kernel<float, B><<<grid, B, 0, s>>>(p);
+        if (precision == 0) {
+            pn_integrate_fixed_kernel<double, B, false><<<grid, B, 0, s>>>(p);
+            pn_integrate_fixed_kernel<double, B, true><<<grid, B, 0, s>>>(p);
+            ++g_pn_launches;
+        } else {
+            pn_integrate_fixed_kernel<float, B, false><<<grid, B, 0, s>>>(p);
+        }
         ++g_pn_launches;
         return cudaGetLastError();
     }
     if (precision == 0) {
-        if (block_threads == 256) return launch_adaptive<double, 256, 1, false>(p, grid_blocks, s);
+        cudaError_t e;
         const char* v = getenv("PN_DEV_VARIANT");   // development switch, not part of the ABI
-        if (v && v[0] == 'r') return launch_adaptive<double, 128, 2, false>(p, grid_blocks, s);
-        return launch_adaptive<double, 128, 3, true>(p, grid_blocks, s);
+        if (block_threads == 256) e = launch_adaptive<double, 256, 1, false, false>(p, grid_blocks, s);
+        else if (v && v[0] == 's') e = launch_adaptive<double, 128, 3, true, false>(p, grid_blocks, s);
+        else e = launch_adaptive<double, 128, 2, false, false>(p, grid_blocks, s);
+        if (e != cudaSuccess) return e;
+        // redo pass for systems that left the series' range; its queue length is read on the device
+        return launch_adaptive<double, 128, 2, false, true>(p, grid_blocks, s);
     }
-    if (block_threads == 128) return launch_adaptive<float, 128, 4, false>(p, grid_blocks, s);
-    return launch_adaptive<float, 256, 2, false>(p, grid_blocks, s);
+    if (block_threads == 128) return launch_adaptive<float, 128, 4, false, false>(p, grid_blocks, s);
+    return launch_adaptive<float, 256, 2, false, false>(p, grid_blocks, s);
 }

@@ -19,6 +19,9 @@ struct PnKernelParams {
     int fixed_steps;
     unsigned mask;
     unsigned int* queue;            // global work counter (zeroed before launch)
+    unsigned int* queue2;           // work counter of the redo pass
+    int* redo_list;                 // [n] systems handed to the redo pass (FP64 only)
+    unsigned int* redo_count;
     unsigned long long* counters;   // [0] trial steps [1] rejected [2] landing trials [3] failed systems
     int* status;                    // worst pn_status seen on the device (atomicMax)
 };

@@ -96,7 +96,7 @@ __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned ma
 //     ln x     = l0 + log1p(-e)  = l0 - e (1 + e/2 + e^2/3 + ...)
 // The first expansion is self-correcting (it is exact in r0 whatever r0's own rounding error), so nothing
 // accumulates in r; l0 is chained once per accepted step with a truncation error < 3e-15 at the switch
-// point |e| = 0.03, beyond which the library functions are used (rare, divergent).  ~22 FMA-pipe
+// point |e| = 0.03, beyond which the trial step is repeated with the library functions (rare).  ~22 FMA-pipe
 // instructions per stage.  FP32 uses cbrtf and the MUFU log directly.
 template <typename real> struct PnBase { real r0, r03, l0; };
 
@@ -108,14 +108,43 @@ __device__ __forceinline__ void pn_base_init(double x, PnBase<double>& b)
 }
 __device__ __forceinline__ void pn_base_init(float, PnBase<float>& b) { b.r0 = b.r03 = b.l0 = 0.0f; }
 
-// r = x^{-1/3}, lnx = ln x  ->  returned so that an accepted step can adopt them as the next base
-__device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, double& v, double& lnx, double& r)
+// r = x^{-1/3}, lnx = ln x  ->  returned so that an accepted step can adopt them as the next base.
+// SLOW = false: series only, branch-free; `bad` is raised when |e| is outside the series' range, and the
+// caller then repeats the whole trial step with SLOW = true (library rcbrt/log), so the hot loop stays one
+// basic block.
+template <bool SLOW>
+__device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, double& v, double& lnx, double& r, bool& bad)
 {
-    const double e = fma(-x, b.r03, 1.0);
-    if (fabs(e) > 0.03) {
-        r = rcbrt(x);
-        lnx = log(x);
+    if (SLOW) {
+        // wide-range, call-free evaluation about the same base, exact to rounding for x/x0 in [0.4, 2]:
+        //   x^{-1/3} = r0 u,  u = rho^{-1/3} by five cubically convergent iterations u <- u (1 + d/3 + 2 d^2/9),
+        //              d = 1 - rho u^3,  rho = x/x0 = 1 - e
+        //   ln x     = l0 + 2 atanh(w),  w = (rho - 1)/(rho + 1) = -e/(2 - e);  1/(2 - e) by Newton, no divide
+        // Outside that range (omega more than doubled or halved inside ONE step) e is clamped, the values are
+        // finite but wrong, and `bad` tells the caller to reject the step.
+        const double e_raw = fma(-x, b.r03, 1.0);
+        const double e = fmin(fmax(e_raw, -1.0), 0.6);
+        bad = bad || (e_raw < -1.0) || (e_raw > 0.6);
+        const double rho = 1.0 - e;
+        double uu = 1.0;
+#pragma unroll
+        for (int it = 0; it < 5; ++it) {
+            const double d = fma(-rho * uu, uu * uu, 1.0);
+            uu = fma(uu * d, fma(d, 2.0 / 9.0, 1.0 / 3.0), uu);
+        }
+        r = b.r0 * uu;
+        const double den = 2.0 - e;
+        double t = fma(e, fma(e, 0.125, 0.25), 0.5);
+#pragma unroll
+        for (int it = 0; it < 5; ++it) t = t * fma(-den, t, 2.0);
+        const double w = -e * t, w2 = w * w;
+        double A = 1.0 / 45.0;
+#pragma unroll
+        for (int k = 21; k >= 1; --k) A = fma(A, w2, 1.0 / (double)(2 * k + 1));
+        lnx = fma(2.0 * w, fma(A, w2, 1.0), b.l0);
     } else {
+        const double e = fma(-x, b.r03, 1.0);
+        bad = bad || (fabs(e) > 0.03);      // false for NaN: a non-finite state is reported as such, not redone
         // (1-e)^{-1/3} = 1 + e S(e),  S = sum_{k=1..9} s_k e^{k-1},  s_k = prod_{j<k}(1/3 + j)/k!
         // log1p(-e)    =   - e Q(e),  Q = sum_{k=1..9} e^{k-1}/k
         // truncation < 6.1e-17 for |e| <= 0.03.  Even/odd split in e halves the dependent FMA chains.
@@ -137,7 +166,8 @@ __device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, dou
     }
     v = x * (r * r);
 }
-__device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float& v, float& lnx, float& r)
+template <bool SLOW>
+__device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float& v, float& lnx, float& r, bool&)
 {
     v = cbrtf(x);
     lnx = __logf(x);
@@ -159,14 +189,14 @@ __device__ __forceinline__ void pn_make_scaled(const PnConsts<real>& c, real h, 
 
 // K = h f(y).  ~70 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and
 // lnx_out = ln x of this evaluation are handed back for the base update of an accepted step.
-template <typename real>
+template <bool SLOW, typename real>
 __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, const PnUni<real>& u,
                                        const PnScaled<real>& sc, const PnBase<real>& base,
-                                       real (&f)[10], real& r_out, real& lnx_out)
+                                       real (&f)[10], real& r_out, real& lnx_out, bool& bad)
 {
     const real x = c.M * y[0];
     real v, lnx, r;
-    pn_powers(x, base, v, lnx, r);
+    pn_powers<SLOW>(x, base, v, lnx, r, bad);
     r_out = r; lnx_out = lnx;
     const real v2 = v * v, v4 = v2 * v2, v5 = v4 * v, x2 = x * x;
 

@@ -144,3 +144,27 @@ def test_fp32_full_size_C4_histograms(pn, oracle):
     assert np.abs(da - db).max() <= 2e-3
     ca = oracle.histogram(a["final"], 50)[0].astype(np.int64); cb = oracle.histogram(b["final"], 50)[0].astype(np.int64)
     assert np.all(np.abs(ca - cb) <= 5 * np.sqrt(ca + cb + 1))
+
+
+def test_loose_tolerance_uses_the_redo_pass(pn, oracle):
+    """FP64 at a very loose tolerance: steps change omega by more than 3 %, which is outside the range of the
+    in-step cbrt/log series; such systems are re-integrated by the wide-range redo kernel.  The result
+    still tracks the oracle run with the same settings to tolerance level."""
+    cfg = W.with_size(W.CONFIGS["C1"], 300)
+    y0, m = W.generate(cfg)
+    g = gpu_integrate(pn, y0, m, cfg, rtol=1e-3, atol=1e-5)
+    assert g["status"] == 0 and np.all(g["steps"] > 0)
+    assert pn.pn_last_counters()["redo"] > 0
+    r = oracle.integrate(y0, m, cfg.omegaf, 1e-3, 1e-5)
+    ref = oracle.integrate(y0, m, cfg.omegaf, 1e-10, 1e-12)
+    dg, dr, dref = dots_of(oracle, g["final"]), dots_of(oracle, r["final"]), dots_of(oracle, ref["final"])
+    err_oracle = np.abs(dr - dref).max()
+    assert np.abs(dg - dref).max() <= 3 * err_oracle + 1e-6      # as accurate as the oracle at this tolerance
+    assert np.abs(g["final"][:, 0] - cfg.omegaf).max() <= 1.01e-13 * cfg.omegaf
+    assert abs(g["steps"].mean() / r["steps"].mean() - 1) < 0.1
+    # fixed-step mode with a huge step goes through the fixed-step redo kernel and still matches the oracle
+    g = gpu_integrate(pn, y0[:64], m[:64], cfg, fixed_steps=20, h0=100.0)
+    r = oracle.integrate(y0[:64], m[:64], 0, 0, 0, fixed_steps=20, h0=100.0)
+    assert pn.pn_last_counters()["redo"] > 0
+    from test_gpu_parity import comp_scale
+    assert (np.abs(g["final"] - r["final"]) / comp_scale(y0[:64])).max() <= 1e-11
