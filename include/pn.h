@@ -125,6 +125,13 @@ int pn_stream_status(void* stream);
  */
 int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz);
 
+/*
+ * pn_measure_fma_operands -- issue cost of an FMA as a function of how many DISTINCT register sources it
+ * reads (1, 2 or 3; the other operands are uniform): cycles per warp instruction per scheduler with 8 warps
+ * x 8 independent chains resident.  Evidence for the operand-port model of DESIGN.md 7.2.
+ */
+int pn_measure_fma_operands(int precision, int n_register_sources, double* cycles_per_warp_inst);
+
 /* Device-side counters of the last synchronous pn_integrate* call: total trial steps, rejected
  * steps, discarded landing trials, systems that failed.  Any pointer may be NULL. */
 int pn_last_counters(unsigned long long* trial_steps, unsigned long long* rejected,

@@ -19,7 +19,7 @@ PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
 EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_stream_status",
-           "pn_measure_fma_peak", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
+           "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
 
@@ -54,6 +54,7 @@ def load():
         lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_stream_status.argtypes = [vp]
         lib.pn_measure_fma_peak.argtypes = [i, d, C.POINTER(d), C.POINTER(d)]
+        lib.pn_measure_fma_operands.argtypes = [i, i, C.POINTER(d)]
         lib.pn_last_counters.argtypes = [C.POINTER(C.c_ulonglong)] * 4
         lib.pn_last_kernel_ms.argtypes = [C.POINTER(C.c_float)]
         lib.pn_launch_count.restype = C.c_ulonglong
@@ -139,6 +140,12 @@ def pn_measure_fma_peak(precision=PN_FP64, seconds=0.25):
     t, mhz = C.c_double(0), C.c_double(0)
     _check(load().pn_measure_fma_peak(int(precision), float(seconds), C.byref(t), C.byref(mhz)))
     return t.value, mhz.value
+
+
+def pn_measure_fma_operands(precision=PN_FP64, n_register_sources=3):
+    c = C.c_double(0)
+    _check(load().pn_measure_fma_operands(int(precision), int(n_register_sources), C.byref(c)))
+    return c.value
 
 
 def pn_last_counters():

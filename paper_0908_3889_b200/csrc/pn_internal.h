@@ -35,8 +35,7 @@ cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int widt
 cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long n, int bins,
                                 unsigned long long* counts /*[3][bins]*/, unsigned long long* skipped /*[3]*/,
                                 cudaStream_t s);
-cudaError_t pn_launch_cost_keys(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys,
-                                int* idx, cudaStream_t s);
-cudaError_t pn_run_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz);
+cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
+                            double* cycles_per_warp_inst);
 
 extern unsigned long long g_pn_launches;
