@@ -139,8 +139,8 @@ def run_ours(args, cfg):
     prec = pn.PN_FP32 if cfg.precision == "fp32" else pn.PN_FP64
 
     # every rank integrates its own seeded batch of the full workload size (weak scaling)
-    from dataclasses import replace
-    y0, m = W.generate(replace(cfg, seed=cfg.seed + 1000 * rank))
+    from paper_0908_3889_b200 import sharding
+    y0, m = W.generate(sharding.rank_config(cfg, rank))
     n = cfg.n
     h_y0 = torch.from_numpy(y0).pin_memory(); h_m = torch.from_numpy(m).pin_memory()
     d_y0, d_m = h_y0.to(dev), h_m.to(dev)
@@ -153,8 +153,7 @@ def run_ours(args, cfg):
     def step():
         pn.pn_integrate(d_y0, d_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, d_yf, d_steps)
         pn.pn_histogram(d_yf, cfg.bins, d_counts)
-        if world > 1:
-            dist.all_reduce(d_counts)        # the one exchange step of the sharded path
+        sharding.allreduce_counts(d_counts, dist if world > 1 else None)   # the one exchange step
 
     def barrier():
         if world > 1:
@@ -180,10 +179,7 @@ def run_ours(args, cfg):
     clocks = sampler.stop()
     launches = pn.pn_launch_count() - launches0
     ms_total = ev0.elapsed_time(ev1)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
+    ms_step = sharding.max_over_ranks(ms_total, dev, dist if world > 1 else None) / args.steps
     counters = pn.pn_last_counters()
 
     # end to end through the C ABI with HOST buffers: H2D of inputs and D2H of results inside the timed region
@@ -202,9 +198,7 @@ def run_ours(args, cfg):
     for _ in range(e2e_steps):
         e2e_step()
     barrier()
-    e2e_s = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_s = sharding.max_over_ranks((time.perf_counter() - t0) / e2e_steps, dev, dist if world > 1 else None)
     h2d = (10 + 2) * 8 * n + 10 * 8 * n          # states + masses for pn_integrate, final states for pn_histogram
     d2h = 10 * 8 * n + 4 * n + 3 * cfg.bins * 8
 
@@ -244,7 +238,7 @@ def run_ours(args, cfg):
                      "frac_with_oracle_as_printed_count": (float(np.mean(trial_steps)) * F_STEP_ORACLE + n * F_RHS_ORACLE)
                      / (k_ms * 1e-3) / 1e12 / peak_nominal,
                      "fma_issue_cycles_by_register_sources": {str(k): pn.pn_measure_fma_operands(prec, k) for k in (1, 2, 3)}},
-        "e2e": {"value": total_inspirals / float(e2e_s.item()), "unit": "inspirals/s", "h2d_bytes_per_step": h2d,
+        "e2e": {"value": total_inspirals / e2e_s, "unit": "inspirals/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,
     }

@@ -1,0 +1,35 @@
+"""Host-side plumbing of the multi-GPU path: the batch dimension is sharded, every rank
+runs its own persistent grid, and the only exchange is the sum of the 3 x bins histogram counters.
+Backend-agnostic (NCCL on GPUs, gloo in the CPU tests); holds no arithmetic of the method."""
+from __future__ import annotations
+
+from dataclasses import replace
+
+
+def rank_config(cfg, rank: int):
+    """Weak scaling: every rank integrates its own full-size batch with a rank-specific seed."""
+    return replace(cfg, seed=cfg.seed + 1000 * int(rank))
+
+
+def shard_range(n: int, rank: int, world: int):
+    """Strong scaling: contiguous, balanced [lo, hi) slice of a batch of n systems for this rank."""
+    base, rem = divmod(int(n), int(world))
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def allreduce_counts(counts, dist=None):
+    """In-place sum of the histogram counters over ranks (int64 tensor [3, bins]); no-op for one rank."""
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(counts)
+    return counts
+
+
+def max_over_ranks(value: float, device, dist=None) -> float:
+    """A timing is the max over ranks, reduced on the device."""
+    import torch
+
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())

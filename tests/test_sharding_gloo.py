@@ -1,0 +1,74 @@
+"""N > 1 host logic on CPU: world_size 2, gloo backend.  No GPU, no CUDA library call."""
+import os
+import socket
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist  # noqa: E402
+import torch.multiprocessing as mp  # noqa: E402
+
+from paper_0908_3889_b200 import sharding  # noqa: E402
+from paper_0908_3889_b200 import workloads as W  # noqa: E402
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        cfg = W.with_size(W.CONFIGS["C3"], 2000)
+        mine = sharding.rank_config(cfg, rank)
+        y0, m = W.generate(mine)
+        # stand-in for this rank's final dot products: something deterministic from ITS inputs
+        d = y0[:, 4] / np.linalg.norm(y0[:, 4:7], axis=1)
+        local = np.stack([np.histogram(d, bins=50, range=(-1, 1))[0]] * 3).astype(np.int64)
+        counts = torch.from_numpy(local.copy())
+        sharding.allreduce_counts(counts, dist)
+        tmax = sharding.max_over_ranks(10.0 + rank, torch.device("cpu"), dist)
+        lo, hi = sharding.shard_range(1001, rank, world)
+        out.put((rank, local, counts.numpy(), tmax, lo, hi, float(y0[:, 1].sum())))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_rank_sharding_and_count_allreduce():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted([q.get(timeout=120) for _ in range(world)], key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    total = res[0][1] + res[1][1]
+    for rank, local, reduced, tmax, lo, hi, chk in res:
+        assert np.array_equal(reduced, total)           # every rank holds the global histogram
+        assert reduced.sum() == 3 * 2000 * world
+        assert tmax == 11.0                             # max over ranks
+    assert (res[0][4], res[0][5], res[1][4], res[1][5]) == (0, 501, 501, 1001)   # disjoint, covering
+    assert res[0][6] != res[1][6]                       # ranks drew different batches
+
+
+def test_shard_range_partitions():
+    for n in (0, 1, 7, 1000, 1 << 20):
+        for world in (1, 2, 3, 8):
+            r = [sharding.shard_range(n, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == n
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+            sizes = [hi - lo for lo, hi in r]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def test_single_process_is_a_noop():
+    c = torch.ones(3, 5, dtype=torch.int64)
+    assert sharding.allreduce_counts(c, dist).sum().item() == 15
+    assert sharding.max_over_ranks(3.5, torch.device("cpu"), dist) == 3.5
