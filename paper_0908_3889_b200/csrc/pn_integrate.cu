@@ -57,6 +57,39 @@ __device__ __forceinline__ float pn_rcp_f(float a) { float r; asm("rcp.approx.ft
 __device__ __forceinline__ float pn_lg2_f(float a) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 __device__ __forceinline__ float pn_ex2_f(float a) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
 
+// E^2 of the scaled RMS error norm, returned in FP32 (see the call site).
+__device__ __forceinline__ float pn_err_norm2(const double (&y)[10], const double (&ynew)[10], const double (&err)[10],
+                                              float rtol, float atol1, float atS1, float atS2)
+{
+    const double rt = (double)rtol;
+    double sum = 0.0;
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const double at = (double)((i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1));
+        const unsigned ha = (unsigned)__double2hiint(y[i]) & 0x7fffffffu, hb = (unsigned)__double2hiint(ynew[i]) & 0x7fffffffu;
+        const double m = hb > ha ? ynew[i] : y[i];          // larger magnitude to ~1e-6 (high words only)
+        const double sc = fma(rt, fabs(m), at);
+        double r;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(sc));
+        const double q = err[i] * r;
+        sum = fma(q, q, sum);
+    }
+    return (float)(sum * 0.1);
+}
+__device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float (&ynew)[10], const float (&err)[10],
+                                              float rtol, float atol1, float atS1, float atS2)
+{
+    float sum = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const float at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
+        const float scl = fmaxf(fmaf(rtol, fmaxf(fabsf(y[i]), fabsf(ynew[i])), at), 1e-30f);
+        const float q = err[i] * pn_rcp_f(scl);
+        sum = fmaf(q, q, sum);
+    }
+    return sum * 0.1f;
+}
+
 // SMEM = true (FP64 only): k2..k5 and the error partial live in dynamic shared memory (pn_dp5_smem.cuh)
 // SLOW = true: the redo pass.  Systems whose step left the range of the cbrt/log series in the fast kernel
 // are re-integrated from their initial state with the wide-range evaluation (pn_rhs.cuh) in every stage.
@@ -164,19 +197,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
             idx = -1;
         }
 
-        // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|).
-        // Evaluated in FP32 in both precisions: it only decides accept/reject and the next step size, a
-        // relative accuracy of 1e-7 is ample, and the F64->F32 conversions run on the otherwise idle
-        // conversion unit instead of ~65 instructions on the FP64 pipe.
-        float sum = 0.0f;
-#pragma unroll
-        for (int i = 0; i < 10; ++i) {
-            const float at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
-            const float scl = fmaxf(fmaf(rtol, fmaxf(fabsf((float)y[i]), fabsf((float)ynew[i])), at), 1e-30f);
-            const float q = (float)err[i] * pn_rcp_f(scl);
-            sum = fmaf(q, q, sum);
-        }
-        const float E2 = force_reject ? 1e30f : sum * 0.1f;      // E^2; accept iff E^2 <= 1
+        // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|), E^2 = mean (err_j/sc_j)^2.
+        // It only decides accept/reject and the next step size, so ~1e-6 relative accuracy is ample:
+        // FP64: the larger magnitude is picked by comparing the high words (integer pipe), 1/sc_j is the raw
+        // MUFU seed (rcp.approx.ftz.f64, ~2^-23, no Newton step): 3 FP64 instructions per component and no
+        // F64<->F32 conversions (which issue at 1/8 rate and put a long serial tail at the end of the step).
+        const float E2 = force_reject ? 1e30f : pn_err_norm2(y, ynew, err, rtol, atol1, atS1, atS2);
 
         // ---------------- per-lane decision as straight-line selects ----------------
         // controller factor 0.9 (E^2)^{-1/10} on the FP32 special-function unit (R8)
@@ -206,15 +232,16 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         }
         if (accept) nland = 0;
         const real h_next = h * ratio;
-        // rare exits: finished, non-finite, landing failure, max_steps, step-size underflow
+        // rare exits: finished, non-finite, landing failure, max_steps, step-size underflow (t + h == t);
+        // priority by overwrite order, all selects, one branch
+        const real h_floor = pn_max(PnLimits<real>::tiny(), (real)(2.3e-16 * t));   // independent of the controller chain
         int code = 0;
-        if (active) {
-            if (!finite) code = PN_F_NONFINITE;
-            else if (landed) code = steps;
-            else if (nland > 50) code = PN_F_LANDING;
-            else if (steps >= p.max_steps) code = PN_F_MAXSTEPS;
-            else if (!(pn_abs(h_next) > PnLimits<real>::tiny()) || t + (double)h_next == t) code = PN_F_HUNDERFLOW;
-        }
+        code = !(pn_abs(h_next) > h_floor) ? PN_F_HUNDERFLOW : code;
+        code = (steps >= p.max_steps) ? PN_F_MAXSTEPS : code;
+        code = (nland > 50) ? PN_F_LANDING : code;
+        code = landed ? steps : code;
+        code = !finite ? PN_F_NONFINITE : code;
+        code = active ? code : 0;
         if (code != 0) {
             if (accept) pn_store_result(p, idx, ynew, code, t, nrej);
             else pn_store_result(p, idx, y, code, t, nrej);
