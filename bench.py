@@ -151,7 +151,8 @@ def run_ours(args, cfg):
     stream = torch.cuda.current_stream()
 
     def step():
-        pn.pn_integrate(d_y0, d_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, d_yf, d_steps)
+        pn.pn_integrate(d_y0, d_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, d_yf, d_steps,
+                        input_order=bool(args.input_order))
         pn.pn_histogram(d_yf, cfg.bins, d_counts)
         sharding.allreduce_counts(d_counts, dist if world > 1 else None)   # the one exchange step
 
@@ -189,7 +190,8 @@ def run_ours(args, cfg):
     e2e_steps = max(1, min(args.steps, 3))
 
     def e2e_step():
-        pn.pn_integrate(h_y0, h_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, h_yf, h_steps)
+        pn.pn_integrate(h_y0, h_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, h_yf, h_steps,
+                        input_order=bool(args.input_order))
         pn.pn_histogram(h_yf, cfg.bins, h_counts)
 
     e2e_step()
@@ -223,7 +225,7 @@ def run_ours(args, cfg):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if prec == pn.PN_FP32 else "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "n_inspirals_per_gpu": n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
-                   "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "parallelism": f"batch-sharded x{world}",
+                   "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "queue": "input order" if args.input_order else "longest-expected-first", "parallelism": f"batch-sharded x{world}",
                    "l2": "256 MiB memset between steps, inside the timed region (<0.1 % of a step)"},
         "rhs_evals_per_sec": world * (6 * float(np.mean(trial_steps)) + n) / (ms_step * 1e-3),
         "trial_steps_per_inspiral": float(np.mean(trial_steps)) / n,
@@ -261,6 +263,7 @@ def main():
     ap.add_argument("--n", type=int, default=0, help="override the batch size (not a bench line)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--input-order", type=int, default=0, help="1: issue the work queue in input order instead of longest-expected-first")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     cfg = W.CONFIGS[args.workload]

@@ -84,8 +84,9 @@ typedef struct pn_options {
                               init_states, masses and out_final (no staging pass) */
     int host_buffers;      /* != 0: every array argument is a HOST pointer (see Conventions) */
     int async;             /* != 0: enqueue only (device pointers only) */
-    int sort_by_cost;      /* != 0: systems are issued to the work queue longest-expected-first
-                              (cost model in DESIGN.md 7); results are unaffected */
+    int input_order;       /* 0 (default): systems are issued to the work queue longest-expected-first
+                              (cost model in DESIGN.md 7.5); != 0: in input order.  Results do not
+                              depend on the order */
     double* out_time;      /* [N] or NULL: time t_f at which omega_f was reached */
     int* out_rejected;     /* [N] or NULL: rejected trial steps */
     void* stream;          /* cudaStream_t, or NULL for the default stream */

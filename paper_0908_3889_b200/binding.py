@@ -26,7 +26,7 @@ EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex",
 class PnOptions(C.Structure):
     _fields_ = [("size", C.c_int), ("fixed_steps", C.c_int), ("h0", C.c_double), ("max_steps", C.c_int),
                 ("term_mask", C.c_uint), ("tau_land", C.c_double), ("layout", C.c_int), ("host_buffers", C.c_int),
-                ("async_", C.c_int), ("sort_by_cost", C.c_int), ("out_time", C.c_void_p), ("out_rejected", C.c_void_p),
+                ("async_", C.c_int), ("input_order", C.c_int), ("out_time", C.c_void_p), ("out_rejected", C.c_void_p),
                 ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int)]
 
 
@@ -90,12 +90,12 @@ def _is_host(a) -> bool:
 
 
 def make_options(*, fixed_steps=0, h0=0.0, max_steps=0, term_mask=0, tau_land=0.0, layout=0, host_buffers=False,
-                 async_=False, sort_by_cost=False, out_time=None, out_rejected=None, stream=None, block_threads=0,
+                 async_=False, input_order=False, out_time=None, out_rejected=None, stream=None, block_threads=0,
                  grid_blocks=0) -> PnOptions:
     o = PnOptions()
     o.size = C.sizeof(PnOptions)
     o.fixed_steps, o.h0, o.max_steps, o.term_mask, o.tau_land = int(fixed_steps), float(h0), int(max_steps), int(term_mask), float(tau_land)
-    o.layout, o.host_buffers, o.async_, o.sort_by_cost = int(layout), int(bool(host_buffers)), int(bool(async_)), int(bool(sort_by_cost))
+    o.layout, o.host_buffers, o.async_, o.input_order = int(layout), int(bool(host_buffers)), int(bool(async_)), int(bool(input_order))
     o.out_time, o.out_rejected = _ptr(out_time), _ptr(out_rejected)
     o.stream = None if stream is None else int(getattr(stream, "cuda_stream", stream))
     o.block_threads, o.grid_blocks = int(block_threads), int(grid_blocks)

@@ -39,7 +39,7 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
 static cudaEvent_t g_ev[5];
 static bool g_ev_ok = false;
 static float g_ms[4] = {0, 0, 0, 0};
@@ -130,8 +130,20 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     } else {
         p.y0 = d_init; p.masses = d_m; p.yf = d_final;
     }
+    p.order = nullptr;
+    if (!o.input_order && !fixed && n > 1024) {
+        // longest-expected-first queue order; part of the stage-in time
+        const size_t tb = pn_cost_order_temp_bytes(n);
+        if ((rc = g_sort_keys.ensure(sizeof(float) * 2 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_sort_idx.ensure(sizeof(int) * 2 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = g_sort_tmp.ensure(tb)) != PN_OK) return rc;
+        float* keys = (float*)g_sort_keys.p;
+        int* idx = (int*)g_sort_idx.p;
+        CK(pn_launch_cost_order(p.y0, p.masses, n, omegaf, keys, keys + n, idx, idx + n, g_sort_tmp.p, tb, s));
+        p.order = idx + n;
+    }
     CK(cudaEventRecord(g_ev[1], s));
-    p.steps = d_steps; p.time = d_time; p.rejected = d_rej; p.order = nullptr;
+    p.steps = d_steps; p.time = d_time; p.rejected = d_rej;
     p.n = n;
     p.omega0 = omega0; p.omegaf = omegaf; p.rtol = rtol; p.atol = atol; p.h0 = o.h0;
     p.tau = o.tau_land > 0.0 ? o.tau_land : (precision == PN_FP64 ? 1e-13 : 3e-7);
@@ -292,7 +304,7 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
     for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
     if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
     g_stream_status.clear();

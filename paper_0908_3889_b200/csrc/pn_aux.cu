@@ -1,5 +1,6 @@
 // pn_aux.cu -- staging (AoS <-> SoA), dot-product histogram and FMA-peak kernels of libpn_b200.
 #include <cstdint>
+#include <cub/device/device_radix_sort.cuh>
 #include "pn_internal.h"
 
 // ------------------------------------------------------------------------------------------------
@@ -150,6 +151,49 @@ cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long 
 #undef PN_HIST_LAUNCH
     ++g_pn_launches;
     return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Queue ordering by expected cost (default; pn_options.input_order turns it off).  The number of trial steps of
+// an inspiral follows the number of precession cycles of the faster-precessing body,
+//     key = (4 + 3 m_big/m_small)/eta * (1/(M omega_0) - 1/(M omega_f))        (Eq. (4) over Eq. (1), leading order)
+// (log-correlation 0.98 with the measured step counts on C3 and C5).  Issuing the queue longest-first
+// (LPT) shortens the drain tail of the persistent grid; results do not depend on the order.
+// ------------------------------------------------------------------------------------------------
+__global__ void pn_cost_key_kernel(const double* __restrict__ y0, const double* __restrict__ masses, int n,
+                                   double omegaf, float* __restrict__ keys, int* __restrict__ idx)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double m1 = masses[i], m2 = masses[(size_t)n + i], M = m1 + m2;
+    const double eta = m1 * m2 / (M * M);
+    const double big = fmax(m1, m2), small = fmin(m1, m2);
+    double key = (4.0 + 3.0 * big / small) / eta * (1.0 / (M * y0[i]) - 1.0 / (M * omegaf));
+    if (!(key > 0.0) || !isfinite(key)) key = 0.0;      // bad inputs go last; they are rejected at refill
+    keys[i] = (float)key;
+    idx[i] = i;
+}
+
+size_t pn_cost_order_temp_bytes(int n)
+{
+    size_t bytes = 0;
+    cub::DeviceRadixSort::SortPairsDescending(nullptr, bytes, (const float*)nullptr, (float*)nullptr,
+                                              (const int*)nullptr, (int*)nullptr, n);
+    return bytes;
+}
+
+cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys_in,
+                                 float* keys_out, int* idx_in, int* idx_out, void* temp, size_t temp_bytes,
+                                 cudaStream_t s)
+{
+    if (n <= 0) return cudaSuccess;
+    pn_cost_key_kernel<<<(n + 255) / 256, 256, 0, s>>>(y0_soa, m_soa, n, omegaf, keys_in, idx_in);
+    ++g_pn_launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    e = cub::DeviceRadixSort::SortPairsDescending(temp, temp_bytes, keys_in, keys_out, idx_in, idx_out, n, 0, 32, s);
+    g_pn_launches += 3;   // cub's histogram + onesweep passes (library kernels, counted approximately)
+    return e;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -35,6 +35,10 @@ cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int widt
 cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long n, int bins,
                                 unsigned long long* counts /*[3][bins]*/, unsigned long long* skipped /*[3]*/,
                                 cudaStream_t s);
+size_t pn_cost_order_temp_bytes(int n);
+cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys_in,
+                                 float* keys_out, int* idx_in, int* idx_out, void* temp, size_t temp_bytes,
+                                 cudaStream_t s);
 cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
                             double* cycles_per_warp_inst);
 

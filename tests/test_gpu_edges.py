@@ -99,6 +99,12 @@ def test_layouts_host_buffers_and_determinism(pn, oracle):
     h_yf = np.empty_like(y0); h_steps = np.empty(cfg.n, dtype=np.int32); h_t = np.empty(cfg.n)
     pn.pn_integrate(y0, m, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, h_yf, h_steps, out_time=h_t)
     assert np.array_equal(h_yf, a["final"]) and np.array_equal(h_steps, a["steps"]) and np.array_equal(h_t, a["time"])
+    # queue order does not change any result: input order vs the default longest-expected-first
+    d = gpu_integrate(pn, W.generate(W.with_size(cfg, 3000))[0], W.generate(W.with_size(cfg, 3000))[1], W.with_size(cfg, 3000))
+    e = gpu_integrate(pn, W.generate(W.with_size(cfg, 3000))[0], W.generate(W.with_size(cfg, 3000))[1], W.with_size(cfg, 3000), input_order=True)
+    assert np.array_equal(d["final"], e["final"]) and np.array_equal(d["steps"], e["steps"])
+    d = gpu_integrate(pn, y0, m, cfg, input_order=True)
+    assert np.array_equal(d["final"], a["final"]) and np.array_equal(d["steps"], a["steps"])
     # both block shapes agree bit for bit
     c = gpu_integrate(pn, y0, m, cfg, block_threads=256)
     assert np.array_equal(c["final"], a["final"])
