@@ -39,7 +39,7 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
 static cudaEvent_t g_ev[5];
 static bool g_ev_ok = false;
 static float g_ms[4] = {0, 0, 0, 0};
@@ -151,6 +151,10 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     p.fixed_steps = fixed ? o.fixed_steps : 0;
     p.mask = o.term_mask;
     if ((rc = g_redo.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+    if (!fixed) {
+        if ((rc = g_seed.ensure((precision == PN_FP64 ? sizeof(double) : sizeof(float)) * 40 * (size_t)n)) != PN_OK) return rc;
+        p.seed = g_seed.p;
+    }
     p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
     p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = (int*)g_redo.p;
     CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s));
@@ -304,7 +308,7 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
     for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
     if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
     g_stream_status.clear();

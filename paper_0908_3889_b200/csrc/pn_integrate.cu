@@ -24,6 +24,18 @@ template <typename real> struct PnLimits;
 template <> struct PnLimits<double> { static __device__ double tiny() { return 1e-300; } static __device__ double huge() { return DBL_MAX; } };
 template <> struct PnLimits<float> { static __device__ float tiny() { return 1e-30f; } static __device__ float huge() { return FLT_MAX; } };
 
+template <typename real> struct PnVec;
+template <> struct PnVec<double> {
+    typedef double2 type;
+    static __device__ __forceinline__ double2 make(const double* a) { return make_double2(a[0], a[1]); }
+    static __device__ __forceinline__ void unpack(double2 v, double* a) { a[0] = v.x; a[1] = v.y; }
+};
+template <> struct PnVec<float> {
+    typedef float4 type;
+    static __device__ __forceinline__ float4 make(const float* a) { return make_float4(a[0], a[1], a[2], a[3]); }
+    static __device__ __forceinline__ void unpack(float4 v, float* a) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
+};
+
 // 0.9 * E^{-1/5} (controller, DESIGN.md 3 R8).  Evaluated with the FP32 special-function unit in both
 // precisions: the factor only sets the next trial's step size, 1e-6 relative accuracy is ample and
 // it keeps ~100 instructions per trial step off the FP64 pipe.
@@ -90,6 +102,77 @@ __device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float 
     return sum * 0.1f;
 }
 
+// ---- per-system seed records (stage-in, row a1/a2 of the scope table) ------------------------------------
+// Everything a lane needs to start an inspiral is computed ONCE per system by a plain one-thread-per-system
+// kernel at full lane efficiency, instead of inside the divergent refill section of the persistent kernel
+// (where one lane works and 31 wait): the per-system constants (~10 FP64 divides), the base powers
+// (rcbrt + log), the scaled seed slope K1 = h0 f(y0) and the norm-scaled atol.  One contiguous record of
+// PN_REC reals per system (FP64 320 B, FP32 160 B), so a lane's refill is 20 (10) 16-byte loads.
+//   [0..9] y0   [10..19] K1 = h0 f(y0)   [20..34] PnConsts   [35..37] PnBase   [38] atol |S1|   [39] atol |S2|
+// A record with [38] < 0 marks a system the seed kernel has already failed (bad input).
+#define PN_REC 40
+template <typename real>
+__global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
+{
+    const int i = blockIdx.x * 128 + threadIdx.x;
+    if (i >= p.n) return;
+    double y0[10];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) y0[j] = p.y0[(size_t)j * p.n + i];
+    const double m1 = p.masses[i], m2 = p.masses[(size_t)p.n + i];
+    real* rec = (real*)p.seed + (size_t)i * PN_REC;
+    real y[10], k1[10];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
+    if (!(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
+        (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0))) {
+        pn_store_result(p, i, y, PN_F_BADINPUT, 0.0, 0);
+        atomicMax(p.status, PN_ST_EINVAL);
+        atomicAdd(p.counters + 3, 1ull);
+        rec[38] = (real)-1;
+        return;
+    }
+    PnConsts<real> c;
+    PnBase<real> base;
+    PnUni<real> u;
+    pn_make_uni<real>(p.mask, u);
+    pn_make_consts<real>(m1, m2, p.mask, c);
+    pn_base_init(c.M * y[0], base);
+    const real h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;      // first step (R13); same expression at refill
+    real r_tmp, l_tmp;
+    bool bad_tmp = false;
+    PnScaled<real> sc;
+    pn_make_scaled(c, h, sc);
+    pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad_tmp);      // K1 = h0 f(y0)
+    // atol scaled by the conserved spin norms (R7)
+    const double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
+    const double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
+    real out[PN_REC];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) { out[j] = y[j]; out[10 + j] = k1[j]; }
+    out[20] = c.M; out[21] = c.c2; out[22] = c.c4; out[23] = c.c5; out[24] = c.c6; out[25] = c.c7;
+    out[26] = c.p1; out[27] = c.p2; out[28] = c.q1; out[29] = c.q2; out[30] = c.K0; out[31] = c.A1;
+    out[32] = c.A2; out[33] = c.Bc; out[34] = c.G;
+    out[35] = base.r0; out[36] = base.r03; out[37] = base.l0;
+    out[38] = (real)(p.atol * (s1 > 0.0 ? s1 : 1.0));
+    out[39] = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
+    using vec = typename PnVec<real>::type;           // 16-byte stores
+    vec* dst = (vec*)rec;
+    constexpr int W = 16 / (int)sizeof(real);
+#pragma unroll
+    for (int j = 0; j < PN_REC / W; ++j) dst[j] = PnVec<real>::make(&out[j * W]);
+}
+
+template <typename real>
+__device__ __forceinline__ void pn_load_record(const void* seed, int i, real (&out)[PN_REC])
+{
+    using vec = typename PnVec<real>::type;
+    constexpr int W = 16 / (int)sizeof(real);
+    const vec* src = (const vec*)((const real*)seed + (size_t)i * PN_REC);
+#pragma unroll
+    for (int j = 0; j < PN_REC / W; ++j) PnVec<real>::unpack(__ldg(src + j), &out[j * W]);
+}
+
 // SMEM = true (FP64 only): k2..k5 and the error partial live in dynamic shared memory (pn_dp5_smem.cuh)
 // SLOW = true: the redo pass.  Systems whose step left the range of the cbrt/log series in the fast kernel
 // are re-integrated from their initial state with the wide-range evaluation (pn_rhs.cuh) in every stage.
@@ -143,36 +226,22 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                 const unsigned q = qbase + (unsigned)__popc(wm & ((1u << lane) - 1u));
                 if (q < n_queue) {
                     const int i = order ? order[q] : (int)q;
-                    double y0[10];
-#pragma unroll
-                    for (int j = 0; j < 10; ++j) y0[j] = __ldg(p.y0 + (size_t)j * p.n + i);
-                    const double m1 = __ldg(p.masses + i), m2 = __ldg(p.masses + (size_t)p.n + i);
-                    if (!(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
-                        (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0))) {
-                        real ybad[10];
-#pragma unroll
-                        for (int j = 0; j < 10; ++j) ybad[j] = (real)y0[j];
-                        pn_store_result(p, i, ybad, PN_F_BADINPUT, 0.0, 0);
-                        atomicMax(p.status, PN_ST_EINVAL);
-                        ++tot_fail;          // the lane stays frozen and asks again next iteration
+                    real rec[PN_REC];
+                    pn_load_record<real>(p.seed, i, rec);
+                    if (rec[38] < (real)0) {
+                        // bad input: already failed and stored by the seed kernel; the lane stays frozen and
+                        // asks again next iteration
                     } else {
 #pragma unroll
-                        for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
+                        for (int j = 0; j < 10; ++j) { y[j] = rec[j]; k1[j] = rec[10 + j]; }
+                        c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
+                        c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
+                        c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
+                        base.r0 = rec[35]; base.r03 = rec[36]; base.l0 = rec[37];
+                        atS1 = (float)rec[38]; atS2 = (float)rec[39];
                         t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
                         idx = i;
-                        pn_make_consts<real>(m1, m2, p.mask, c);
-                        pn_base_init(c.M * y[0], base);
-                        h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
-                        real r_tmp, l_tmp;
-                        bool bad_tmp = false;
-                        PnScaled<real> sc;
-                        pn_make_scaled(c, h, sc);
-                        pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad_tmp);      // K1 = h f(y0)
-                        // atol scaled by the conserved spin norms (R7)
-                        double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
-                        double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
-                        atS1 = (float)(p.atol * (s1 > 0.0 ? s1 : 1.0));
-                        atS2 = (float)(p.atol * (s2 > 0.0 ? s2 : 1.0));
+                        h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;
                     }
                 }
             }
@@ -374,6 +443,15 @@ cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int bloc
         }
         ++g_pn_launches;
         return cudaGetLastError();
+    }
+    {
+        // stage-in: per-system seed records (constants, base powers, K1 = h0 f(y0)); bad inputs fail here
+        const int grid = (p.n + 127) / 128;
+        if (precision == 0) pn_seed_kernel<double><<<grid, 128, 0, s>>>(p);
+        else pn_seed_kernel<float><<<grid, 128, 0, s>>>(p);
+        ++g_pn_launches;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
     }
     if (precision == 0) {
         cudaError_t e;

@@ -12,6 +12,7 @@ struct PnKernelParams {
     double* time;        // may be null
     int* rejected;       // may be null
     const int* order;    // may be null: queue position -> system index
+    void* seed;          // [n][40] reals of the launch precision: per-system seed records (pn_integrate.cu)
     int n;
     double omega0;       // > 0: every initial omega must match it to 1e-12 relative
     double omegaf, rtol, atol, h0, tau;
