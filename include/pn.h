@@ -115,6 +115,45 @@ int pn_histogram(const double* final_states, long long N, int bins,
 int pn_histogram_ex(const double* final_states, long long N, int bins,
                     unsigned long long* counts, unsigned long long* n_skipped, const pn_options* opt);
 
+/*
+ * pn_statistics -- one pass over the (initial, final) states of an integrated batch: the ensemble
+ * statistics of the paper's section V.  For each of the three unit dot
+ * products d = S1^.S2^, S1^.L^, S2^.L^ (A^.B^ = (A.B)/(|A||B|), norms from the state itself), with
+ * x = d(initial state) and y = d(final state) of every system of an ensemble:
+ *   - the Pearson product-moment coefficient r = 1/(n-1) sum ((x-xbar)/sigma_x)((y-ybar)/sigma_y)
+ *     (sigma = sample standard deviation, DESIGN.md 3 R18), NaN if n < 2 or a variance is 0;
+ *   - the moments n, xbar, ybar, M2x = sum (x-xbar)^2, M2y, Cxy = sum (x-xbar)(y-ybar);
+ *   - the histogram of y on bins1 equal bins of [-1,1] and the bivariate histogram of
+ *     (x, y) on bins2 x bins2 equal cells (row = bin of x, column = bin of y), its largest
+ *     count, and the histogram divided by that count ("normalized such that the maximum value is 1").
+ * Ensembles ("groups"): group g is the contiguous range [g*group_size, (g+1)*group_size) of systems, so a
+ * parameter sweep (Figs. 6-7) is one pn_integrate call and one pn_statistics call.
+ * group_size <= 0 means one group of N systems; otherwise N must be a multiple of group_size.  G = N/group_size.
+ * A system is left out of the statistics of a dot product (and counted in n_skipped) if either value is
+ * undefined (zero norm, non-finite), and out of all three if steps != NULL and steps[i] < 0.
+ *   init_states, final_states  [N][10] AoS doubles, 16-byte aligned (read with bulk copies).  Read only.
+ *                              init_states == NULL: only hist1 and n_skipped (of the final states) are computed.
+ *   steps                      [N] out_steps of pn_integrate, or NULL.
+ *   out                        any member may be NULL (not computed); bins1 / bins2 < 1 disable hist1 / hist2*.
+ * Bin rule on every axis: bin = clamp(floor((d+1) bins/2), 0, bins-1) (R14).
+ * Results are bit-identical from run to run (no floating-point atomics).
+ * opt: host_buffers, async and stream are honoured; layout must be 0.
+ */
+typedef struct pn_stats_out {
+    int size;                       /* = sizeof(pn_stats_out); checked */
+    double* pearson_r;              /* [G][3] */
+    double* moments;                /* [G][3][6]: n, xbar, ybar, M2x, M2y, Cxy */
+    unsigned long long* n_skipped;  /* [G][3] */
+    unsigned long long* hist1;      /* [G][3][bins1] */
+    unsigned long long* hist2;      /* [G][3][bins2][bins2] */
+    unsigned long long* hist2_max;  /* [G][3]; needs hist2 */
+    double* hist2_norm;             /* [G][3][bins2][bins2]; needs hist2 */
+} pn_stats_out;
+
+int pn_statistics(const double* init_states, const double* final_states, const int* steps, long long N,
+                  long long group_size, int bins1, int bins2, const pn_stats_out* out,
+                  const struct pn_options* opt);
+
 /* Worst pn_status of the async calls enqueued on `stream` since the last pn_stream_status; synchronises it. */
 int pn_stream_status(void* stream);
 
@@ -144,7 +183,7 @@ unsigned long long pn_last_redo_count(void);
 
 /* Duration in milliseconds of the kernels of the last synchronous pn_integrate* / pn_histogram* call,
  * measured with CUDA events on the call's stream: [0] stage-in, [1] integrator, [2] stage-out,
- * [3] histogram.  Entries a call did not run are left unchanged. */
+ * [3] histogram or statistics.  Entries a call did not run are left unchanged. */
 int pn_last_kernel_ms(float ms[4]);
 
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */

@@ -18,7 +18,7 @@ PN_FP64, PN_FP32 = 0, 1
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_stream_status",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -28,6 +28,11 @@ class PnOptions(C.Structure):
                 ("term_mask", C.c_uint), ("tau_land", C.c_double), ("layout", C.c_int), ("host_buffers", C.c_int),
                 ("async_", C.c_int), ("input_order", C.c_int), ("out_time", C.c_void_p), ("out_rejected", C.c_void_p),
                 ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int)]
+
+
+class PnStatsOut(C.Structure):
+    _fields_ = [("size", C.c_int), ("pearson_r", C.c_void_p), ("moments", C.c_void_p), ("n_skipped", C.c_void_p),
+                ("hist1", C.c_void_p), ("hist2", C.c_void_p), ("hist2_max", C.c_void_p), ("hist2_norm", C.c_void_p)]
 
 
 class PnError(RuntimeError):
@@ -52,6 +57,7 @@ def load():
         lib.pn_integrate_ex.argtypes = [vp, vp, ll, d, d, d, d, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_histogram.argtypes = [vp, ll, i, vp, vp]
         lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
+        lib.pn_statistics.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
         lib.pn_stream_status.argtypes = [vp]
         lib.pn_measure_fma_peak.argtypes = [i, d, C.POINTER(d), C.POINTER(d)]
         lib.pn_measure_fma_operands.argtypes = [i, i, C.POINTER(d)]
@@ -130,6 +136,23 @@ def pn_histogram(final_states, bins, counts, n_skipped=None, *, n=None, **opts):
         opts["host_buffers"] = True
     o = make_options(**opts)
     return _check(lib.pn_histogram_ex(_ptr(final_states), int(n), int(bins), _ptr(counts), _ptr(n_skipped), C.byref(o)))
+
+
+def pn_statistics(init_states, final_states, steps=None, *, group_size=0, bins1=0, bins2=0, pearson_r=None,
+                  moments=None, n_skipped=None, hist1=None, hist2=None, hist2_max=None, hist2_norm=None, **opts):
+    """pn_statistics of include/pn.h.  Output arrays are caller-allocated (torch CUDA tensors, or numpy when
+    the inputs are on the host); any of them may be None.  init_states may be None (final-only mode)."""
+    lib = load()
+    n = int(final_states.shape[0])
+    if _is_host(final_states):
+        opts["host_buffers"] = True
+    o = make_options(**opts)
+    out = PnStatsOut()
+    out.size = C.sizeof(PnStatsOut)
+    out.pearson_r, out.moments, out.n_skipped = _ptr(pearson_r), _ptr(moments), _ptr(n_skipped)
+    out.hist1, out.hist2, out.hist2_max, out.hist2_norm = _ptr(hist1), _ptr(hist2), _ptr(hist2_max), _ptr(hist2_norm)
+    return _check(lib.pn_statistics(_ptr(init_states), _ptr(final_states), _ptr(steps), n, int(group_size), int(bins1),
+                                    int(bins2), C.byref(out), C.byref(o)))
 
 
 def pn_stream_status(stream=None):

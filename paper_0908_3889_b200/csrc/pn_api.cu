@@ -1,5 +1,6 @@
 // pn_api.cu -- the C ABI of libpn_b200 (include/pn.h): argument checks, scratch management, staging,
 // launches, status collection.  Every CUDA call is checked.
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -39,7 +40,7 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts;
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts, g_st_scratch, g_st_in, g_st_out;
 static cudaEvent_t g_ev[5];
 static bool g_ev_ok = false;
 static float g_ms[4] = {0, 0, 0, 0};
@@ -238,6 +239,82 @@ extern "C" int pn_histogram(const double* final_states, long long N, int bins, u
     return pn_histogram_ex(final_states, N, bins, counts, n_skipped, nullptr);
 }
 
+extern "C" int pn_statistics(const double* init_states, const double* final_states, const int* steps, long long N,
+                             long long group_size, int bins1, int bins2, const pn_stats_out* out_in,
+                             const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (!out_in || out_in->size != (int)sizeof(pn_stats_out)) return PN_EINVAL;
+    pn_stats_out out = *out_in;
+    if (N < 0 || N > 0x7fffffffLL * 8 || o.layout != 0) return PN_EINVAL;
+    if (N > 0 && !final_states) return PN_EINVAL;
+    if (o.async && o.host_buffers) return PN_EINVAL;
+    if (bins1 > 8192 || bins2 > 4096) return PN_EINVAL;
+    if (bins1 < 1) { bins1 = 0; out.hist1 = nullptr; }
+    if (bins2 < 1 || !init_states) { bins2 = 0; out.hist2 = nullptr; }
+    if (!out.hist2) { if (out.hist2_max || out.hist2_norm) return PN_EINVAL; }
+    const long long gs = group_size > 0 ? group_size : N;
+    if (N > 0 && N % gs != 0) return PN_EINVAL;
+    const long long G = N > 0 ? N / gs : 0;
+    if (N == 0) return PN_OK;
+    if (!o.host_buffers && (((uintptr_t)final_states & 15u) || ((uintptr_t)init_states & 15u))) return PN_EINVAL;
+    cudaStream_t s = (cudaStream_t)o.stream;
+    int rc;
+    if ((rc = ensure_events()) != PN_OK) return rc;
+    if ((rc = g_st_scratch.ensure(pn_stats_scratch_bytes(N, group_size, nullptr))) != PN_OK) return rc;
+
+    const double* d_init = init_states;
+    const double* d_fin = final_states;
+    const int* d_steps = steps;
+    pn_stats_out d = out;
+    // host buffers: stage inputs and outputs through device scratch
+    const size_t row = sizeof(double) * 10 * (size_t)N;
+    const size_t b_r = sizeof(double) * 3 * (size_t)G, b_m = 6 * b_r, b_sk = sizeof(unsigned long long) * 3 * (size_t)G;
+    const size_t b_h1 = sizeof(unsigned long long) * 3 * (size_t)bins1 * G, b_h2 = sizeof(unsigned long long) * 3 * (size_t)bins2 * bins2 * G;
+    if (o.host_buffers) {
+        const size_t in_bytes = row * (init_states ? 2 : 1) + (steps ? sizeof(int) * (size_t)N : 0);
+        if ((rc = g_st_in.ensure(in_bytes)) != PN_OK) return rc;
+        char* q = (char*)g_st_in.p;
+        CK(cudaMemcpyAsync(q, final_states, row, cudaMemcpyHostToDevice, s));
+        d_fin = (const double*)q; q += row;
+        if (init_states) { CK(cudaMemcpyAsync(q, init_states, row, cudaMemcpyHostToDevice, s)); d_init = (const double*)q; q += row; }
+        if (steps) { CK(cudaMemcpyAsync(q, steps, sizeof(int) * (size_t)N, cudaMemcpyHostToDevice, s)); d_steps = (const int*)q; }
+        if ((rc = g_st_out.ensure(b_r + b_m + 2 * b_sk + b_h1 + 2 * b_h2 + 64)) != PN_OK) return rc;
+        char* w = (char*)g_st_out.p;
+        auto take = [&](size_t bytes) { char* r = w; w += (bytes + 15) & ~(size_t)15; return r; };
+        if (out.pearson_r) d.pearson_r = (double*)take(b_r);
+        if (out.moments) d.moments = (double*)take(b_m);
+        if (out.n_skipped) d.n_skipped = (unsigned long long*)take(b_sk);
+        if (out.hist1) d.hist1 = (unsigned long long*)take(b_h1);
+        if (out.hist2) d.hist2 = (unsigned long long*)take(b_h2);
+        if (out.hist2_max) d.hist2_max = (unsigned long long*)take(b_sk);
+        if (out.hist2_norm) d.hist2_norm = (double*)take(b_h2);
+    }
+    CK(cudaEventRecord(g_ev[3], s));
+    CK(pn_launch_stats(d_init, d_fin, d_steps, N, group_size, bins1, bins2, g_st_scratch.p, d.pearson_r, d.moments,
+                       d.n_skipped, d.hist1, d.hist2, d.hist2_max, d.hist2_norm, s));
+    CK(cudaEventRecord(g_ev[4], s));
+    if (o.async) return PN_OK;
+    if (o.host_buffers) {
+        if (out.pearson_r) CK(cudaMemcpyAsync(out.pearson_r, d.pearson_r, b_r, cudaMemcpyDeviceToHost, s));
+        if (out.moments) CK(cudaMemcpyAsync(out.moments, d.moments, b_m, cudaMemcpyDeviceToHost, s));
+        if (out.n_skipped) CK(cudaMemcpyAsync(out.n_skipped, d.n_skipped, b_sk, cudaMemcpyDeviceToHost, s));
+        if (out.hist1) CK(cudaMemcpyAsync(out.hist1, d.hist1, b_h1, cudaMemcpyDeviceToHost, s));
+        if (out.hist2) CK(cudaMemcpyAsync(out.hist2, d.hist2, b_h2, cudaMemcpyDeviceToHost, s));
+        if (out.hist2_max) CK(cudaMemcpyAsync(out.hist2_max, d.hist2_max, b_sk, cudaMemcpyDeviceToHost, s));
+        if (out.hist2_norm) CK(cudaMemcpyAsync(out.hist2_norm, d.hist2_norm, b_h2, cudaMemcpyDeviceToHost, s));
+    }
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    CK(cudaEventElapsedTime(&g_ms[3], g_ev[3], g_ev[4]));
+    return PN_OK;
+}
+
 extern "C" int pn_stream_status(void* stream)
 {
     cudaStream_t s = (cudaStream_t)stream;
@@ -308,7 +385,7 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts};
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts, &g_st_scratch, &g_st_in, &g_st_out};
     for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
     if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
     g_stream_status.clear();

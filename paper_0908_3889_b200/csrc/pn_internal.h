@@ -40,6 +40,12 @@ size_t pn_cost_order_temp_bytes(int n);
 cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys_in,
                                  float* keys_out, int* idx_in, int* idx_out, void* temp, size_t temp_bytes,
                                  cudaStream_t s);
+// ensemble statistics (pn_stats.cu)
+size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out);
+cudaError_t pn_launch_stats(const double* init, const double* fin, const int* steps, long long n, long long group_size,
+                            int bins1, int bins2, void* scratch, double* r_out, double* mom_out,
+                            unsigned long long* skipped_out, unsigned long long* hist1, unsigned long long* hist2,
+                            unsigned long long* hist2_max, double* hist2_norm, cudaStream_t s);
 cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
                             double* cycles_per_warp_inst);
 

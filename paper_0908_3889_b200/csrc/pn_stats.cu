@@ -1,0 +1,392 @@
+// pn_stats.cu -- one-pass ensemble statistics of (initial, final) states for sm_100a:
+// Pearson r of the initial vs final unit dot products, their bivariate histograms
+// and the 1-D histograms of the final ones, per ensemble ("group":
+// a contiguous range of group_size systems, so a parameter sweep -- Figs. 6, 7 -- is one launch).
+//
+// HBM-bound: 160 B per system (two AoS rows) + 4 B (steps).  One persistent block per SM streams tiles of
+// 256 systems (2 x 20 KB, contiguous in the AoS arrays) through a 3-stage shared-memory ring filled by
+// cp.async.bulk (TMA 1-D bulk copies, one elected thread, completion on an mbarrier), so ~80 KB per SM
+// are always in flight.  Per-thread shifted sums -> (n, mean, M2, C) -> Chan's pairwise merge over the
+// warp (xor butterfly), the block (shared memory) and the grid (one record per (block, group), merged in
+// block order by the finish kernel): no floating-point atomics, results are bit-identical run to run.
+// Histograms are privatised in shared memory (3 x bins1 + 3 x bins2^2 u32) and flushed with 64-bit global
+// atomics when the block leaves a group.
+// This file shares nothing with oracle/ (which evaluates the two-pass definitions in numpy).
+#include <cstdint>
+#include "pn_internal.h"
+
+#define ST_TILE 256
+#define ST_STAGES 3
+#define ST_ROW 10
+#define ST_TILE_BYTES (ST_TILE * ST_ROW * 8)
+
+// ---- mbarrier / bulk-copy PTX ---------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t st_smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void st_mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void st_mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void st_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void st_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok)
+                     : "r"(bar), "r"(parity)
+                     : "memory");
+    } while (!ok);
+}
+
+// ---- moments ----------------------------------------------------------------------------------------------
+struct StMom { double n, mx, my, m2x, m2y, cxy; };
+
+// Chan et al. pairwise update: merge b into a
+__device__ __forceinline__ void st_merge(StMom& a, const StMom& b)
+{
+    const double n = a.n + b.n;
+    if (n == 0.0) return;
+    const double dx = b.mx - a.mx, dy = b.my - a.my;
+    const double w = a.n * b.n / n, f = b.n / n;
+    a.m2x += b.m2x + dx * dx * w;
+    a.m2y += b.m2y + dy * dy * w;
+    a.cxy += b.cxy + dx * dy * w;
+    a.mx = (b.n == 0.0) ? a.mx : ((a.n == 0.0) ? b.mx : a.mx + dx * f);
+    a.my = (b.n == 0.0) ? a.my : ((a.n == 0.0) ? b.my : a.my + dy * f);
+    a.n = n;
+}
+__device__ __forceinline__ StMom st_shfl_xor(const StMom& a, int o)
+{
+    StMom r;
+    r.n = __shfl_xor_sync(0xffffffffu, a.n, o);
+    r.mx = __shfl_xor_sync(0xffffffffu, a.mx, o);
+    r.my = __shfl_xor_sync(0xffffffffu, a.my, o);
+    r.m2x = __shfl_xor_sync(0xffffffffu, a.m2x, o);
+    r.m2y = __shfl_xor_sync(0xffffffffu, a.m2y, o);
+    r.cxy = __shfl_xor_sync(0xffffffffu, a.cxy, o);
+    return r;
+}
+
+// per-thread running sums of (x - x0), (y - y0) about the thread's first sample of the group
+struct StAcc {
+    double n, x0, y0, sx, sy, sxx, syy, sxy;
+    __device__ __forceinline__ void reset() { n = x0 = y0 = sx = sy = sxx = syy = sxy = 0.0; }
+    __device__ __forceinline__ void add(double x, double y)
+    {
+        if (n == 0.0) { x0 = x; y0 = y; }
+        const double dx = x - x0, dy = y - y0;
+        n += 1.0;
+        sx += dx; sy += dy;
+        sxx = fma(dx, dx, sxx); syy = fma(dy, dy, syy); sxy = fma(dx, dy, sxy);
+    }
+    __device__ __forceinline__ StMom moments() const
+    {
+        StMom m;
+        m.n = n;
+        if (n == 0.0) { m.mx = m.my = m.m2x = m.m2y = m.cxy = 0.0; return m; }
+        const double inv = 1.0 / n;
+        m.mx = x0 + sx * inv; m.my = y0 + sy * inv;
+        m.m2x = fmax(sxx - sx * sx * inv, 0.0);
+        m.m2y = fmax(syy - sy * sy * inv, 0.0);
+        m.cxy = sxy - sx * sy * inv;
+        return m;
+    }
+};
+
+// unit dot products of one AoS row; ok[k] false where a norm is zero or the quotient is not finite (R14)
+__device__ __forceinline__ void st_unit_dots(const double* __restrict__ row, double (&d)[3], bool (&ok)[3])
+{
+    const double s1x = row[1], s1y = row[2], s1z = row[3], s2x = row[4], s2y = row[5], s2z = row[6];
+    const double lx = row[7], ly = row[8], lz = row[9];
+    const double a = fma(s1x, s1x, fma(s1y, s1y, s1z * s1z));
+    const double b = fma(s2x, s2x, fma(s2y, s2y, s2z * s2z));
+    const double c = fma(lx, lx, fma(ly, ly, lz * lz));
+    const double ra = rsqrt(a), rb = rsqrt(b), rc = rsqrt(c);
+    d[0] = fma(s1x, s2x, fma(s1y, s2y, s1z * s2z)) * ra * rb;
+    d[1] = fma(s1x, lx, fma(s1y, ly, s1z * lz)) * ra * rc;
+    d[2] = fma(s2x, lx, fma(s2y, ly, s2z * lz)) * rb * rc;
+    // a unit dot product cannot leave [-1, 1]; the three roundings above can overshoot by an ulp or two
+    ok[0] = a > 0.0 && b > 0.0 && isfinite(d[0]);
+    ok[1] = a > 0.0 && c > 0.0 && isfinite(d[1]);
+    ok[2] = b > 0.0 && c > 0.0 && isfinite(d[2]);
+}
+__device__ __forceinline__ int st_bin(double d, int bins)
+{
+    const int b = (int)floor((d + 1.0) * (double)bins * 0.5);
+    return max(0, min(bins - 1, b));
+}
+
+struct StParams {
+    const double* init;     // [N][10] or null (final-only mode: 1-D histograms and skipped counts only)
+    const double* fin;      // [N][10]
+    const int* steps;       // [N] or null
+    long long n, group_size;
+    int n_groups, tiles_per_group, items_per_block;
+    long long n_items;
+    int bins1, bins2, hist2_smem;
+    double* records;                 // [(blocks + groups)][3][6]
+    unsigned long long* rec_skipped; // [(blocks + groups)][3]
+    unsigned long long* hist1;       // [G][3][bins1] or null
+    unsigned long long* hist2;       // [G][3][bins2][bins2] or null
+};
+
+template <bool HAVE_INIT>
+__global__ void __launch_bounds__(ST_TILE, 1) pn_stats_kernel(const StParams p)
+{
+    extern __shared__ __align__(128) unsigned char st_smem[];
+    // layout: [stages][2 tiles] | mbarriers | warp scratch | hist1 | hist2
+    constexpr int NT = HAVE_INIT ? 2 : 1;
+    double* tiles = reinterpret_cast<double*>(st_smem);
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(st_smem + (size_t)ST_STAGES * NT * ST_TILE_BYTES);
+    double* wscr = reinterpret_cast<double*>(bars + 8);                        // [8 warps][3][6]
+    unsigned* skip_s = reinterpret_cast<unsigned*>(wscr + 8 * 18);             // [4]
+    unsigned* hist1 = skip_s + 4;
+    unsigned* hist2 = hist1 + 3 * p.bins1;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nh1 = 3 * p.bins1, nh2 = p.hist2_smem ? 3 * p.bins2 * p.bins2 : 0;
+
+    const long long w_begin = (long long)blockIdx.x * p.items_per_block;
+    const long long w_end = min(w_begin + (long long)p.items_per_block, p.n_items);
+    if (w_begin >= w_end) return;
+
+    for (int b = tid; b < nh1 + nh2; b += ST_TILE) hist1[b] = 0u;
+    if (tid < 4) skip_s[tid] = 0u;
+    if (tid == 0) {
+        for (int s = 0; s < ST_STAGES; ++s) st_mbar_init(st_smem_addr(&bars[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    auto item_range = [&](long long w, long long& start, int& cnt, int& g) {
+        g = (int)(w / p.tiles_per_group);
+        const long long t = w - (long long)g * p.tiles_per_group;
+        start = (long long)g * p.group_size + t * ST_TILE;
+        cnt = (int)min((long long)ST_TILE, p.group_size - t * ST_TILE);
+    };
+    auto issue = [&](long long w, int stage) {       // one elected thread
+        long long start; int cnt, g;
+        item_range(w, start, cnt, g);
+        const uint32_t bar = st_smem_addr(&bars[stage]);
+        const uint32_t bytes = (uint32_t)cnt * ST_ROW * 8u;
+        st_mbar_expect_tx(bar, bytes * NT);
+        double* dst = tiles + (size_t)stage * NT * ST_TILE * ST_ROW;
+        st_bulk_g2s(st_smem_addr(dst), p.fin + start * ST_ROW, bytes, bar);
+        if (HAVE_INIT) st_bulk_g2s(st_smem_addr(dst + ST_TILE * ST_ROW), p.init + start * ST_ROW, bytes, bar);
+    };
+    if (tid == 0)
+        for (int s = 0; s < ST_STAGES && w_begin + s < w_end; ++s) issue(w_begin + s, s);
+
+    StAcc acc[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) acc[k].reset();
+    unsigned skip[3] = {0u, 0u, 0u};
+
+    int stage = 0;
+    uint32_t parity = 0;
+    for (long long w = w_begin; w < w_end; ++w) {
+        long long start; int cnt, g;
+        item_range(w, start, cnt, g);
+        st_mbar_wait(st_smem_addr(&bars[stage]), parity);
+        double rf[ST_ROW], ri[ST_ROW];
+        const bool have = tid < cnt;
+        if (have) {
+            const double* src = tiles + (size_t)stage * NT * ST_TILE * ST_ROW + tid * ST_ROW;
+#pragma unroll
+            for (int c = 0; c < ST_ROW; ++c) rf[c] = src[c];
+            if (HAVE_INIT)
+#pragma unroll
+                for (int c = 0; c < ST_ROW; ++c) ri[c] = src[ST_TILE * ST_ROW + c];
+        }
+        const bool failed = have && p.steps && (p.steps[start + tid] < 0);
+        __syncthreads();                                   // every thread has read this stage
+        if (tid == 0 && w + ST_STAGES < w_end) issue(w + ST_STAGES, stage);
+        if (++stage == ST_STAGES) { stage = 0; parity ^= 1u; }
+
+        if (have) {
+            double df[3], di[3];
+            bool okf[3], oki[3] = {true, true, true};
+            st_unit_dots(rf, df, okf);
+            if (HAVE_INIT) st_unit_dots(ri, di, oki);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const bool ok = okf[k] && oki[k] && !failed;
+                if (!ok) { ++skip[k]; continue; }
+                if (HAVE_INIT) acc[k].add(di[k], df[k]);
+                if (p.bins1) atomicAdd(&hist1[k * p.bins1 + st_bin(df[k], p.bins1)], 1u);
+                if (HAVE_INIT && p.bins2) {
+                    const size_t cell = ((size_t)k * p.bins2 + st_bin(di[k], p.bins2)) * p.bins2 + st_bin(df[k], p.bins2);
+                    if (p.hist2_smem) atomicAdd(&hist2[cell], 1u);
+                    else atomicAdd(&p.hist2[(size_t)g * 3 * p.bins2 * p.bins2 + cell], 1ull);
+                }
+            }
+        }
+
+        // ---- leaving group g (or the block's range): merge and flush ----
+        const bool last_of_group = (w + 1 == w_end) || ((int)((w + 1) / p.tiles_per_group) != g);
+        if (last_of_group) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                StMom m = acc[k].moments();
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { StMom other = st_shfl_xor(m, o); st_merge(m, other); }
+                // the butterfly leaves every lane with a (not bitwise identical) total; lane 0's is the result
+                if (lane == 0) {
+                    double* q = wscr + (warp * 3 + k) * 6;
+                    q[0] = m.n; q[1] = m.mx; q[2] = m.my; q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
+                }
+                unsigned sk = skip[k];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sk += __shfl_xor_sync(0xffffffffu, sk, o);
+                if (lane == 0 && sk) atomicAdd(&skip_s[k], sk);
+                acc[k].reset();
+                skip[k] = 0u;
+            }
+            __syncthreads();
+            const size_t slot = (size_t)blockIdx.x + (size_t)g;        // unique per (block, group): both only grow
+            if (tid < 3) {
+                StMom m = {0, 0, 0, 0, 0, 0};
+                for (int ww = 0; ww < ST_TILE / 32; ++ww) {
+                    const double* q = wscr + (ww * 3 + tid) * 6;
+                    StMom o = {q[0], q[1], q[2], q[3], q[4], q[5]};
+                    st_merge(m, o);
+                }
+                double* r = p.records + (slot * 3 + tid) * 6;
+                r[0] = m.n; r[1] = m.mx; r[2] = m.my; r[3] = m.m2x; r[4] = m.m2y; r[5] = m.cxy;
+                p.rec_skipped[slot * 3 + tid] = skip_s[tid];
+            }
+            if (p.hist1)
+                for (int b = tid; b < nh1; b += ST_TILE)
+                    if (hist1[b]) { atomicAdd(&p.hist1[(size_t)g * nh1 + b], (unsigned long long)hist1[b]); hist1[b] = 0u; }
+            if (nh2)
+                for (int b = tid; b < nh2; b += ST_TILE)
+                    if (hist2[b]) { atomicAdd(&p.hist2[(size_t)g * nh2 + b], (unsigned long long)hist2[b]); hist2[b] = 0u; }
+            __syncthreads();
+            if (tid < 4) skip_s[tid] = 0u;
+            __syncthreads();
+        }
+    }
+}
+
+// One thread per (group, dot product): merge the per-block records of that group in block order.
+__global__ void pn_stats_finish_kernel(const StParams p, int n_blocks, double* __restrict__ r_out,
+                                       double* __restrict__ mom_out, unsigned long long* __restrict__ skipped_out)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= p.n_groups * 3) return;
+    const int g = j / 3, k = j % 3;
+    const long long w_lo = (long long)g * p.tiles_per_group, w_hi = w_lo + p.tiles_per_group - 1;
+    const int b_lo = (int)(w_lo / p.items_per_block), b_hi = min((int)(w_hi / p.items_per_block), n_blocks - 1);
+    StMom m = {0, 0, 0, 0, 0, 0};
+    unsigned long long sk = 0;
+    for (int b = b_lo; b <= b_hi; ++b) {
+        const size_t slot = (size_t)b + (size_t)g;
+        const double* q = p.records + (slot * 3 + k) * 6;
+        StMom o = {q[0], q[1], q[2], q[3], q[4], q[5]};
+        st_merge(m, o);
+        sk += p.rec_skipped[slot * 3 + k];
+    }
+    if (mom_out) {
+        double* q = mom_out + (size_t)j * 6;
+        q[0] = m.n; q[1] = m.n > 0 ? m.mx : nan(""); q[2] = m.n > 0 ? m.my : nan(""); q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
+    }
+    // PAPER.md:138 with sample standard deviations (R18): r = Cxy / sqrt(M2x M2y); undefined for n < 2 or zero variance
+    if (r_out) r_out[j] = (m.n >= 2.0 && m.m2x > 0.0 && m.m2y > 0.0) ? m.cxy / sqrt(m.m2x * m.m2y) : nan("");
+    if (skipped_out) skipped_out[j] = sk;
+}
+
+// One block per (group, dot product): maximum count of the bivariate histogram and counts / max.
+__global__ void __launch_bounds__(256) pn_stats_norm_kernel(const unsigned long long* __restrict__ hist2, int cells,
+                                                            unsigned long long* __restrict__ max_out, double* __restrict__ norm_out)
+{
+    __shared__ unsigned long long red[256];
+    const unsigned long long* h = hist2 + (size_t)blockIdx.x * cells;
+    unsigned long long mx = 0;
+    for (int c = threadIdx.x; c < cells; c += 256) mx = max(mx, h[c]);
+    red[threadIdx.x] = mx;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) red[threadIdx.x] = max(red[threadIdx.x], red[threadIdx.x + o]);
+        __syncthreads();
+    }
+    mx = red[0];
+    if (threadIdx.x == 0 && max_out) max_out[blockIdx.x] = mx;
+    if (norm_out) {
+        for (int c = threadIdx.x; c < cells; c += 256)
+            norm_out[(size_t)blockIdx.x * cells + c] = mx ? (double)h[c] / (double)mx : 0.0;    // correctly rounded quotient
+    }
+}
+
+size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out)
+{
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long gs = group_size > 0 ? group_size : n;
+    const long long G = gs > 0 ? n / gs : 0;
+    const long long tpg = (gs + ST_TILE - 1) / ST_TILE;
+    const long long items = G * tpg;
+    const long long blocks = items < sms ? items : sms;
+    if (n_blocks_out) *n_blocks_out = (int)blocks;
+    return (size_t)(blocks + G + 1) * 3 * (6 * sizeof(double) + sizeof(unsigned long long));
+}
+
+cudaError_t pn_launch_stats(const double* init, const double* fin, const int* steps, long long n, long long group_size,
+                            int bins1, int bins2, void* scratch, double* r_out, double* mom_out,
+                            unsigned long long* skipped_out, unsigned long long* hist1, unsigned long long* hist2,
+                            unsigned long long* hist2_max, double* hist2_norm, cudaStream_t s)
+{
+    const long long gs = group_size > 0 ? group_size : n;
+    const long long G = gs > 0 ? n / gs : 0;
+    cudaError_t e;
+    if (hist1 && (e = cudaMemsetAsync(hist1, 0, sizeof(unsigned long long) * 3 * (size_t)bins1 * G, s)) != cudaSuccess) return e;
+    if (hist2 && (e = cudaMemsetAsync(hist2, 0, sizeof(unsigned long long) * 3 * (size_t)bins2 * bins2 * G, s)) != cudaSuccess) return e;
+    if (n <= 0 || G <= 0) return cudaSuccess;
+    int n_blocks = 0;
+    const size_t scr = pn_stats_scratch_bytes(n, group_size, &n_blocks);
+    if ((e = cudaMemsetAsync(scratch, 0, scr, s)) != cudaSuccess) return e;
+    StParams p;
+    p.init = init; p.fin = fin; p.steps = steps; p.n = n; p.group_size = gs; p.n_groups = (int)G;
+    p.tiles_per_group = (int)((gs + ST_TILE - 1) / ST_TILE);
+    p.n_items = G * p.tiles_per_group;
+    p.items_per_block = (int)((p.n_items + n_blocks - 1) / n_blocks);
+    n_blocks = (int)((p.n_items + p.items_per_block - 1) / p.items_per_block);
+    p.bins1 = hist1 ? bins1 : 0;
+    p.bins2 = (hist2 && init) ? bins2 : 0;
+    p.records = (double*)scratch;
+    p.rec_skipped = (unsigned long long*)((char*)scratch + (size_t)(n_blocks + G + 1) * 3 * 6 * sizeof(double));
+    p.hist1 = hist1; p.hist2 = hist2;
+    const int nt = init ? 2 : 1;
+    const size_t fixed = (size_t)ST_STAGES * nt * ST_TILE_BYTES + 64 + 8 * 18 * sizeof(double) + 16 + 3 * (size_t)p.bins1 * 4;
+    const size_t h2 = 3 * (size_t)p.bins2 * p.bins2 * 4;
+    const size_t cap = 220 * 1024;
+    if (fixed > cap) return cudaErrorInvalidValue;
+    p.hist2_smem = (p.bins2 > 0 && fixed + h2 <= cap) ? 1 : 0;
+    const size_t shm = fixed + (p.hist2_smem ? h2 : 0);
+    if (init) {
+        if ((e = cudaFuncSetAttribute(pn_stats_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm)) != cudaSuccess) return e;
+        pn_stats_kernel<true><<<n_blocks, ST_TILE, shm, s>>>(p);
+    } else {
+        if ((e = cudaFuncSetAttribute(pn_stats_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm)) != cudaSuccess) return e;
+        pn_stats_kernel<false><<<n_blocks, ST_TILE, shm, s>>>(p);
+    }
+    ++g_pn_launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    pn_stats_finish_kernel<<<(int)((G * 3 + 127) / 128), 128, 0, s>>>(p, n_blocks, r_out, mom_out, skipped_out);
+    ++g_pn_launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (p.bins2 && (hist2_max || hist2_norm)) {
+        pn_stats_norm_kernel<<<(int)(G * 3), 256, 0, s>>>(hist2, bins2 * bins2, hist2_max, hist2_norm);
+        ++g_pn_launches;
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
