@@ -95,6 +95,19 @@ def generate(cfg: Config):
     return np.ascontiguousarray(y0), np.ascontiguousarray(masses)
 
 
+def philox_key(seed: int):
+    """The Philox4x64 key numpy derives from an integer seed (SeedSequence): with it and counter 0 the raw
+    stream of `np.random.Philox(seed)` is reproducible by any Philox4x64-10 implementation."""
+    k = np.random.Philox(seed).state["state"]["key"]
+    return int(k[0]), int(k[1])
+
+
+def generator_spec(cfg: Config) -> dict:
+    """The parameters of `generate(cfg)` in the form the on-device generator (pn_generate) and its oracle take."""
+    return dict(key=philox_key(cfg.seed), omega0=cfg.omega0, q=cfg.q, chi1=cfg.chi1, chi2=cfg.chi2,
+                m1_fixed=cfg.m1_fixed, s1_tilt_deg=cfg.s1_fixed_tilt_deg)
+
+
 def sample_indices(n: int, k: int, seed: int = 12345) -> np.ndarray:
     """k distinct system indices of a batch of n (sorted), for sampled oracle comparisons."""
     rng = np.random.Generator(np.random.Philox(seed))
