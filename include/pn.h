@@ -154,6 +154,37 @@ int pn_statistics(const double* init_states, const double* final_states, const i
                   long long group_size, int bins1, int bins2, const pn_stats_out* out,
                   const struct pn_options* opt);
 
+/*
+ * pn_generate -- random initial data on the device ("generated on the GPU"; recipe of
+ * PAPER.md:68, 102-104 as fixed in DESIGN.md 5 and 12): for every system seven uniform variates
+ * (q, chi1, chi2, z1, phi1, z2, phi2) from ONE counter-based Philox4x64-10 stream per ensemble, laid out
+ * like numpy.random.Philox: variate (k, i) = U(word (e mod 4) of Philox(counter = e/4 + 1, key)),
+ * e = k*n_total + i, U(x) = (x >> 11) 2^-53.  q = m2/m1 uniform in [q_lo, q_hi] (q_lo if q_hi <= q_lo),
+ * m1 = 1/(1+q), m2 = q/(1+q), or (m1_fixed, 1 - m1_fixed) if m1_fixed > 0; chi_i uniform in
+ * [chi_i_lo, chi_i_hi]; unit spins (sqrt(1-z^2) cos phi, sqrt(1-z^2) sin phi, z), z = 2u - 1,
+ * phi = 2 pi u' (uniform on the sphere), or S^_1 = (sin t, 0, cos t) if s1_tilt_deg = t >= 0;
+ * S_i = chi_i m_i^2 S^_i; L^ = (0,0,1); omega = omega0.
+ *   ens           HOST array of n_ensembles descriptions (a parameter sweep is several ensembles).
+ *   n_total       systems per ensemble: fixes the layout of the variate stream.
+ *   first, count  the chunk [first, first+count) of every ensemble to generate (first+count <= n_total);
+ *                 chunks of one ensemble generated by separate calls (or GPUs) are identical to one big call.
+ *   init_states   [n_ensembles*count][10], masses [n_ensembles*count][2], AoS, 16-byte aligned; ensemble e
+ *                 occupies rows [e*count, (e+1)*count).  Device pointers (host with opt->host_buffers).
+ * A system's state is a pure function of (key, n_total, index): results are bit-identical from run to run.
+ */
+typedef struct pn_ensemble {
+    int size;                          /* = sizeof(pn_ensemble); checked */
+    unsigned long long key[2];         /* Philox4x64 key */
+    double omega0;
+    double q_lo, q_hi;
+    double m1_fixed;                   /* > 0: fixed masses (m1_fixed, 1 - m1_fixed); q_* then only consume their variate */
+    double chi1_lo, chi1_hi, chi2_lo, chi2_hi;
+    double s1_tilt_deg;                /* >= 0: S^_1 fixed in the x-z plane, tilted from L^ by this angle; < 0: isotropic */
+} pn_ensemble;
+
+int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,
+                double* init_states, double* masses, const struct pn_options* opt);
+
 /* Worst pn_status of the async calls enqueued on `stream` since the last pn_stream_status; synchronises it. */
 int pn_stream_status(void* stream);
 

@@ -18,7 +18,7 @@ PN_FP64, PN_FP32 = 0, 1
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_generate", "pn_stream_status",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -33,6 +33,23 @@ class PnOptions(C.Structure):
 class PnStatsOut(C.Structure):
     _fields_ = [("size", C.c_int), ("pearson_r", C.c_void_p), ("moments", C.c_void_p), ("n_skipped", C.c_void_p),
                 ("hist1", C.c_void_p), ("hist2", C.c_void_p), ("hist2_max", C.c_void_p), ("hist2_norm", C.c_void_p)]
+
+
+class PnEnsemble(C.Structure):
+    _fields_ = [("size", C.c_int), ("key", C.c_ulonglong * 2), ("omega0", C.c_double), ("q_lo", C.c_double),
+                ("q_hi", C.c_double), ("m1_fixed", C.c_double), ("chi1_lo", C.c_double), ("chi1_hi", C.c_double),
+                ("chi2_lo", C.c_double), ("chi2_hi", C.c_double), ("s1_tilt_deg", C.c_double)]
+
+
+def make_ensemble(key, omega0, q=(1.0, 1.0), chi1=(1.0, 1.0), chi2=(1.0, 1.0), m1_fixed=None, s1_tilt_deg=None) -> PnEnsemble:
+    e = PnEnsemble()
+    e.size = C.sizeof(PnEnsemble)
+    e.key[0], e.key[1] = int(key[0]), int(key[1])
+    e.omega0, e.q_lo, e.q_hi = float(omega0), float(q[0]), float(q[1])
+    e.m1_fixed = float(m1_fixed) if m1_fixed is not None else 0.0
+    e.chi1_lo, e.chi1_hi, e.chi2_lo, e.chi2_hi = float(chi1[0]), float(chi1[1]), float(chi2[0]), float(chi2[1])
+    e.s1_tilt_deg = float(s1_tilt_deg) if s1_tilt_deg is not None else -1.0
+    return e
 
 
 class PnError(RuntimeError):
@@ -58,6 +75,7 @@ def load():
         lib.pn_histogram.argtypes = [vp, ll, i, vp, vp]
         lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_statistics.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
+        lib.pn_generate.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, vp, vp, C.POINTER(PnOptions)]
         lib.pn_stream_status.argtypes = [vp]
         lib.pn_measure_fma_peak.argtypes = [i, d, C.POINTER(d), C.POINTER(d)]
         lib.pn_measure_fma_operands.argtypes = [i, i, C.POINTER(d)]
@@ -153,6 +171,19 @@ def pn_statistics(init_states, final_states, steps=None, *, group_size=0, bins1=
     out.hist1, out.hist2, out.hist2_max, out.hist2_norm = _ptr(hist1), _ptr(hist2), _ptr(hist2_max), _ptr(hist2_norm)
     return _check(lib.pn_statistics(_ptr(init_states), _ptr(final_states), _ptr(steps), n, int(group_size), int(bins1),
                                     int(bins2), C.byref(out), C.byref(o)))
+
+
+def pn_generate(ensembles, n_total, init_states, masses, *, first=0, count=None, **opts):
+    """pn_generate of include/pn.h.  `ensembles`: one PnEnsemble (make_ensemble) or a list of them; output arrays
+    [len(ensembles)*count, 10] and [.., 2] float64 (torch CUDA tensors, or numpy for host buffers)."""
+    lib = load()
+    ens = ensembles if isinstance(ensembles, (list, tuple)) else [ensembles]
+    arr = (PnEnsemble * len(ens))(*ens)
+    count = int(n_total) - int(first) if count is None else int(count)
+    if _is_host(init_states):
+        opts["host_buffers"] = True
+    o = make_options(**opts)
+    return _check(lib.pn_generate(arr, len(ens), int(n_total), int(first), count, _ptr(init_states), _ptr(masses), C.byref(o)))
 
 
 def pn_stream_status(stream=None):

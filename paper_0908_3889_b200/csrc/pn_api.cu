@@ -5,6 +5,7 @@
 #include <cstring>
 #include <map>
 #include <string>
+#include <vector>
 #include "../../include/pn.h"
 #include "pn_internal.h"
 
@@ -40,7 +41,7 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts, g_st_scratch, g_st_in, g_st_out;
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts, g_st_scratch, g_st_in, g_st_out, g_gen_specs, g_gen_y, g_gen_m;
 static cudaEvent_t g_ev[5];
 static bool g_ev_ok = false;
 static float g_ms[4] = {0, 0, 0, 0};
@@ -315,6 +316,61 @@ extern "C" int pn_statistics(const double* init_states, const double* final_stat
     return PN_OK;
 }
 
+extern "C" int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,
+                           double* init_states, double* masses, const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (!ens || n_ensembles < 1 || n_ensembles > 65536 || n_total < 0 || first < 0 || count < 0 || first + count > n_total ||
+        o.layout != 0 || (o.async && o.host_buffers))
+        return PN_EINVAL;
+    if (n_total > (1LL << 59)) return PN_EINVAL;                       // 7 n_total variates must fit the 2^64 word stream
+    if (count == 0) return PN_OK;
+    if (!init_states || !masses) return PN_EINVAL;
+    if (!o.host_buffers && ((((uintptr_t)init_states) | ((uintptr_t)masses)) & 15u)) return PN_EINVAL;
+    struct Spec { unsigned long long k0, k1; double v[9]; };
+    std::vector<Spec> h(n_ensembles);
+    for (int e = 0; e < n_ensembles; ++e) {
+        const pn_ensemble& x = ens[e];
+        if (x.size != (int)sizeof(pn_ensemble) || !(x.omega0 > 0.0) || !(x.q_lo > 0.0) || !(x.chi1_lo >= 0.0) || !(x.chi2_lo >= 0.0) ||
+            !(x.m1_fixed < 1.0))
+            return PN_EINVAL;
+        h[e].k0 = x.key[0]; h[e].k1 = x.key[1];
+        const double v[9] = {x.omega0, x.q_lo, x.q_hi, x.m1_fixed, x.chi1_lo, x.chi1_hi, x.chi2_lo, x.chi2_hi, x.s1_tilt_deg};
+        memcpy(h[e].v, v, sizeof v);
+    }
+    cudaStream_t s = (cudaStream_t)o.stream;
+    int rc;
+    if ((rc = ensure_events()) != PN_OK) return rc;
+    if ((rc = g_gen_specs.ensure(sizeof(Spec) * (size_t)n_ensembles)) != PN_OK) return rc;
+    CK(cudaMemcpyAsync(g_gen_specs.p, h.data(), sizeof(Spec) * (size_t)n_ensembles, cudaMemcpyHostToDevice, s));
+    CK(cudaStreamSynchronize(s));      // h is a local: the copy must have left it before we return
+    const size_t rows = (size_t)n_ensembles * (size_t)count;
+    double* d_y = init_states;
+    double* d_m = masses;
+    if (o.host_buffers) {
+        if ((rc = g_gen_y.ensure(sizeof(double) * 10 * rows)) != PN_OK) return rc;
+        if ((rc = g_gen_m.ensure(sizeof(double) * 2 * rows)) != PN_OK) return rc;
+        d_y = (double*)g_gen_y.p; d_m = (double*)g_gen_m.p;
+    }
+    CK(cudaEventRecord(g_ev[0], s));
+    CK(pn_launch_generate(g_gen_specs.p, n_ensembles, n_total, first, count, d_y, d_m, s));
+    CK(cudaEventRecord(g_ev[1], s));
+    if (o.async) return PN_OK;
+    if (o.host_buffers) {
+        CK(cudaMemcpyAsync(init_states, d_y, sizeof(double) * 10 * rows, cudaMemcpyDeviceToHost, s));
+        CK(cudaMemcpyAsync(masses, d_m, sizeof(double) * 2 * rows, cudaMemcpyDeviceToHost, s));
+    }
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    CK(cudaEventElapsedTime(&g_ms[0], g_ev[0], g_ev[1]));
+    return PN_OK;
+}
+
 extern "C" int pn_stream_status(void* stream)
 {
     cudaStream_t s = (cudaStream_t)stream;
@@ -385,7 +441,7 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts, &g_st_scratch, &g_st_in, &g_st_out};
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts, &g_st_scratch, &g_st_in, &g_st_out, &g_gen_specs, &g_gen_y, &g_gen_m};
     for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
     if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
     g_stream_status.clear();

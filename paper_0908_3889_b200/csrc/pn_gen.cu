@@ -1,0 +1,129 @@
+// pn_gen.cu -- on-device initial data for sm_100a: random spin orientations uniform on the sphere, random
+// mass ratios and spin magnitudes, L^ = (0,0,1), M = 1.
+//
+// Counter-based, so a system's initial state is a pure function of (key, ensemble size, system index):
+// seven uniform variates per system, variate column k = the k-th length-n_total block of ONE Philox4x64-10
+// stream laid out like numpy.random.Philox (counter incremented before every block of four 64-bit words,
+// double = (word >> 11) * 2^-53), so that pn_generate reproduces paper_0908_3889_b200/workloads.generate
+// to the last bits that do not depend on sin/cos.  Any chunk [first, first+count) of an ensemble can be
+// generated on its own (chunked 10^8-system runs, multi-GPU shards).
+//
+// HBM-bound: 96 B written per system, nothing read.  One thread per system writes its AoS row into a
+// shared-memory tile; the tile leaves with one TMA bulk store (cp.async.bulk.global.shared::cta) per
+// array, so global writes are full 16-byte-aligned bursts.
+// This file shares nothing with oracle/.
+#include <cstdint>
+#include "pn_internal.h"
+
+#define GEN_TILE 256
+
+#define PHILOX_M0 0xD2E7470EE14C6C93ULL
+#define PHILOX_M1 0xCA5A826395121157ULL
+#define PHILOX_W0 0x9E3779B97F4A7C15ULL
+#define PHILOX_W1 0xBB67AE8584CAA73BULL
+
+// word (e & 3) of Philox4x64-10(counter = (e >> 2) + 1, key)
+__device__ __forceinline__ unsigned long long gen_raw(unsigned long long k0, unsigned long long k1, unsigned long long e)
+{
+    unsigned long long c0 = (e >> 2) + 1ull, c1 = 0ull, c2 = 0ull, c3 = 0ull;
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) { k0 += PHILOX_W0; k1 += PHILOX_W1; }
+        const unsigned long long hi0 = __umul64hi(PHILOX_M0, c0), lo0 = PHILOX_M0 * c0;
+        const unsigned long long hi1 = __umul64hi(PHILOX_M1, c2), lo1 = PHILOX_M1 * c2;
+        const unsigned long long n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    const unsigned w = (unsigned)(e & 3ull);
+    return w == 0 ? c0 : (w == 1 ? c1 : (w == 2 ? c2 : c3));
+}
+__device__ __forceinline__ double gen_uniform(unsigned long long k0, unsigned long long k1, unsigned long long e)
+{
+    return (double)(gen_raw(k0, k1, e) >> 11) * (1.0 / 9007199254740992.0);
+}
+// lo + (hi - lo) u without contraction (the reference recipe rounds the product, then the sum)
+__device__ __forceinline__ double gen_lerp(double lo, double hi, double u)
+{
+    return hi > lo ? __dadd_rn(lo, __dmul_rn(__dsub_rn(hi, lo), u)) : lo;
+}
+__device__ __forceinline__ void gen_unit(double uz, double uphi, double (&v)[3])
+{
+    const double z = __dsub_rn(__dmul_rn(2.0, uz), 1.0);
+    const double phi = __dmul_rn(2.0 * 3.14159265358979323846, uphi);
+    const double r = sqrt(fmax(0.0, __dsub_rn(1.0, __dmul_rn(z, z))));
+    double s, c;
+    sincos(phi, &s, &c);
+    v[0] = __dmul_rn(r, c); v[1] = __dmul_rn(r, s); v[2] = z;
+}
+
+struct GenSpec {           // device copy of pn_ensemble
+    unsigned long long key0, key1;
+    double omega0, q_lo, q_hi, m1_fixed, chi1_lo, chi1_hi, chi2_lo, chi2_hi, s1_tilt_deg;
+};
+
+__global__ void __launch_bounds__(GEN_TILE) pn_generate_kernel(const GenSpec* __restrict__ specs, long long n_total,
+                                                               long long first, long long count, int tiles_per_ens,
+                                                               double* __restrict__ init_states, double* __restrict__ masses)
+{
+    __shared__ __align__(128) double tile_y[GEN_TILE * 10];
+    __shared__ __align__(128) double tile_m[GEN_TILE * 2];
+    const int ens = blockIdx.x / tiles_per_ens;
+    const long long j0 = (long long)(blockIdx.x - ens * tiles_per_ens) * GEN_TILE;      // first row of this tile within the chunk
+    const int cnt = (int)min((long long)GEN_TILE, count - j0);
+    const GenSpec sp = specs[ens];
+    const int t = threadIdx.x;
+    if (t < cnt) {
+        const unsigned long long i = (unsigned long long)(first + j0 + t), N = (unsigned long long)n_total;
+        double u[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) u[k] = gen_uniform(sp.key0, sp.key1, (unsigned long long)k * N + i);
+        const double q = gen_lerp(sp.q_lo, sp.q_hi, u[0]);
+        const double chi1 = gen_lerp(sp.chi1_lo, sp.chi1_hi, u[1]);
+        const double chi2 = gen_lerp(sp.chi2_lo, sp.chi2_hi, u[2]);
+        double s1[3], s2[3];
+        gen_unit(u[3], u[4], s1);
+        gen_unit(u[5], u[6], s2);
+        double m1, m2;
+        if (sp.m1_fixed > 0.0) { m1 = sp.m1_fixed; m2 = __dsub_rn(1.0, m1); }
+        else { const double d = __dadd_rn(1.0, q); m1 = __ddiv_rn(1.0, d); m2 = __ddiv_rn(q, d); }
+        if (sp.s1_tilt_deg >= 0.0) {
+            const double th = __dmul_rn(sp.s1_tilt_deg, 3.14159265358979323846 / 180.0);
+            sincos(th, &s1[0], &s1[2]);
+            s1[1] = 0.0;
+        }
+        const double a1 = __dmul_rn(__dmul_rn(chi1, m1), m1), a2 = __dmul_rn(__dmul_rn(chi2, m2), m2);
+        double* y = tile_y + t * 10;
+        y[0] = sp.omega0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { y[1 + c] = __dmul_rn(a1, s1[c]); y[4 + c] = __dmul_rn(a2, s2[c]); }
+        y[7] = 0.0; y[8] = 0.0; y[9] = 1.0;
+        tile_m[2 * t] = m1; tile_m[2 * t + 1] = m2;
+    }
+    // generic-proxy writes -> visible to the async proxy, then one bulk store per array by one thread
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (t == 0) {
+        const long long row = (long long)ens * count + j0;
+        const uint32_t sy = (uint32_t)__cvta_generic_to_shared(tile_y), sm = (uint32_t)__cvta_generic_to_shared(tile_m);
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(init_states + row * 10), "r"(sy),
+                     "r"((uint32_t)cnt * 80u)
+                     : "memory");
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(masses + row * 2), "r"(sm),
+                     "r"((uint32_t)cnt * 16u)
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");     // the block may exit only after the stores have left smem
+    }
+}
+
+cudaError_t pn_launch_generate(const void* specs_dev, int n_ens, long long n_total, long long first, long long count,
+                               double* init_states, double* masses, cudaStream_t s)
+{
+    if (count <= 0 || n_ens <= 0) return cudaSuccess;
+    const long long tiles = (count + GEN_TILE - 1) / GEN_TILE;
+    if (tiles * n_ens > 0x7fffffffLL) return cudaErrorInvalidValue;
+    pn_generate_kernel<<<(unsigned)(tiles * n_ens), GEN_TILE, 0, s>>>((const GenSpec*)specs_dev, n_total, first, count,
+                                                                      (int)tiles, init_states, masses);
+    ++g_pn_launches;
+    return cudaGetLastError();
+}

@@ -46,6 +46,10 @@ cudaError_t pn_launch_stats(const double* init, const double* fin, const int* st
                             int bins1, int bins2, void* scratch, double* r_out, double* mom_out,
                             unsigned long long* skipped_out, unsigned long long* hist1, unsigned long long* hist2,
                             unsigned long long* hist2_max, double* hist2_norm, cudaStream_t s);
+// on-device initial data (pn_gen.cu); specs_dev: n_ens packed {u64 key0, key1; double omega0, q_lo, q_hi, m1_fixed,
+// chi1_lo, chi1_hi, chi2_lo, chi2_hi, s1_tilt_deg}
+cudaError_t pn_launch_generate(const void* specs_dev, int n_ens, long long n_total, long long first, long long count,
+                               double* init_states, double* masses, cudaStream_t s);
 cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
                             double* cycles_per_warp_inst);
 
