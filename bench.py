@@ -204,6 +204,39 @@ def run_ours(args, cfg):
     h2d = (10 + 2) * 8 * n + 10 * 8 * n          # states + masses for pn_integrate, final states for pn_histogram
     d2h = 10 * 8 * n + 4 * n + 3 * cfg.bins * 8
 
+    # rows beyond the hot path, timed outside the step: on-device statistics of
+    # (initial, final) states and on-device generation of the same batch; both HBM-bound
+    widened = None
+    if world == 1:
+        hbm = None
+        pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(pk):
+            hbm = json.load(open(pk)).get("hbm_gbs")
+        hbm_src = "MEASURED_PEAKS.json hbm_gbs" if hbm else "fallback 6500 GB/s (B200_PROFILING.md)"
+        hbm = float(hbm or 6500.0)
+        out = dict(pearson_r=torch.zeros(1, 3, dtype=torch.float64, device=dev),
+                   moments=torch.zeros(1, 3, 6, dtype=torch.float64, device=dev),
+                   hist1=torch.zeros(1, 3, cfg.bins, dtype=torch.int64, device=dev),
+                   hist2=torch.zeros(1, 3, 79, 79, dtype=torch.int64, device=dev),
+                   hist2_max=torch.zeros(1, 3, dtype=torch.int64, device=dev))
+        st_ms, gen_ms = [], []
+        g_y0, g_m = torch.empty_like(d_y0), torch.empty_like(d_m)
+        ens = pn.make_ensemble(**W.generator_spec(cfg))
+        for i in range(4):
+            flush.zero_()
+            pn.pn_statistics(d_y0, d_yf, d_steps, bins1=cfg.bins, bins2=79, **out)
+            st_ms.append(pn.pn_last_kernel_ms()["histogram"])
+            flush.zero_()
+            pn.pn_generate(ens, n, g_y0, g_m)
+            gen_ms.append(pn.pn_last_kernel_ms()["stage_in"])
+        st, ge = float(np.median(st_ms[1:])), float(np.median(gen_ms[1:]))
+        widened = {"statistics": {"ms": st, "bytes_per_system": 164, "achieved_gbs": 164 * n / st / 1e6,
+                                  "frac_of_hbm": 164 * n / st / 1e6 / hbm, "pearson_r": out["pearson_r"].cpu().numpy()[0].tolist(),
+                                  "bins2": 79},
+                   "generate": {"ms": ge, "bytes_per_system": 96, "achieved_gbs": 96 * n / ge / 1e6,
+                                "frac_of_hbm": 96 * n / ge / 1e6 / hbm,
+                                "max_abs_diff_vs_host_recipe": float((g_y0 - d_y0).abs().max().item())},
+                   "hbm_peak_gbs": hbm, "hbm_peak_source": hbm_src}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -244,6 +277,8 @@ def run_ours(args, cfg):
                 "d2h_bytes_per_step": d2h, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,
     }
+    if widened:
+        line["widened"] = widened
     if world == 1 and not args.no_cpu_baseline:
         cb = oracle_throughput(cfg, target_seconds=args.cpu_seconds)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}

@@ -3,10 +3,11 @@
 // and the 1-D histograms of the final ones, per ensemble ("group":
 // a contiguous range of group_size systems, so a parameter sweep -- Figs. 6, 7 -- is one launch).
 //
-// HBM-bound: 160 B per system (two AoS rows) + 4 B (steps).  One persistent block per SM streams tiles of
-// 256 systems (2 x 20 KB, contiguous in the AoS arrays) through a 3-stage shared-memory ring filled by
-// cp.async.bulk (TMA 1-D bulk copies, one elected thread, completion on an mbarrier), so ~80 KB per SM
-// are always in flight.  Per-thread shifted sums -> (n, mean, M2, C) -> Chan's pairwise merge over the
+// HBM-bound: 160 B per system (two AoS rows) + 4 B (steps).  One persistent block (two consumer groups of 256
+// threads) per SM streams tiles of
+// 256 systems (2 x 20 KB, contiguous in the AoS arrays) through one shared-memory slot per group, filled by
+// cp.async.bulk (TMA 1-D bulk copies, one elected thread, completion on an mbarrier), so up to 80 KB per SM
+// are in flight.  Per-thread shifted sums -> (n, mean, M2, C) -> Chan's pairwise merge over the
 // warp (xor butterfly), the block (shared memory) and the grid (one record per (block, group), merged in
 // block order by the finish kernel): no floating-point atomics, results are bit-identical run to run.
 // Histograms are privatised in shared memory (3 x bins1 + 3 x bins2^2 u32) and flushed with 64-bit global
@@ -16,7 +17,7 @@
 #include "pn_internal.h"
 
 #define ST_TILE 256
-#define ST_STAGES 3
+#define ST_STAGES 2      /* one ring slot per consumer group (see pn_stats_kernel) */
 #define ST_ROW 10
 #define ST_TILE_BYTES (ST_TILE * ST_ROW * 8)
 
@@ -78,22 +79,23 @@ __device__ __forceinline__ StMom st_shfl_xor(const StMom& a, int o)
 
 // per-thread running sums of (x - x0), (y - y0) about the thread's first sample of the group
 struct StAcc {
-    double n, x0, y0, sx, sy, sxx, syy, sxy;
-    __device__ __forceinline__ void reset() { n = x0 = y0 = sx = sy = sxx = syy = sxy = 0.0; }
+    int n;
+    double x0, y0, sx, sy, sxx, syy, sxy;
+    __device__ __forceinline__ void reset() { n = 0; x0 = y0 = sx = sy = sxx = syy = sxy = 0.0; }
     __device__ __forceinline__ void add(double x, double y)
     {
-        if (n == 0.0) { x0 = x; y0 = y; }
+        if (n == 0) { x0 = x; y0 = y; }
         const double dx = x - x0, dy = y - y0;
-        n += 1.0;
+        ++n;
         sx += dx; sy += dy;
         sxx = fma(dx, dx, sxx); syy = fma(dy, dy, syy); sxy = fma(dx, dy, sxy);
     }
     __device__ __forceinline__ StMom moments() const
     {
         StMom m;
-        m.n = n;
-        if (n == 0.0) { m.mx = m.my = m.m2x = m.m2y = m.cxy = 0.0; return m; }
-        const double inv = 1.0 / n;
+        m.n = (double)n;
+        if (n == 0) { m.mx = m.my = m.m2x = m.m2y = m.cxy = 0.0; return m; }
+        const double inv = 1.0 / m.n;
         m.mx = x0 + sx * inv; m.my = y0 + sy * inv;
         m.m2x = fmax(sxx - sx * sx * inv, 0.0);
         m.m2y = fmax(syy - sy * sy * inv, 0.0);
@@ -139,26 +141,38 @@ struct StParams {
     unsigned long long* hist2;       // [G][3][bins2][bins2] or null
 };
 
+// ST_GROUPS consumer groups of ST_TILE threads, each with its own shared-memory slot and mbarrier: item k of the
+// block (k = 0, 1, ...) is consumed by group k % ST_GROUPS.  A group copies its rows to registers, syncs on its own
+// named barrier and its first thread immediately re-arms the slot for the group's next item, so each group's next
+// tile (40 KB) is in flight while it does its FP64 work, and the groups run out of phase with one another
+// (16 warps per SM hide the rsqrt / atomic latencies that 8 lock-stepped warps could not).  A slot is never
+// shared between groups: a consumer that ran ahead of the re-arming group would see the PREVIOUS phase of the
+// mbarrier as complete and read a stale tile.
+#define ST_GROUPS 2
+#define ST_THREADS (ST_GROUPS * ST_TILE)
 template <bool HAVE_INIT>
-__global__ void __launch_bounds__(ST_TILE, 1) pn_stats_kernel(const StParams p)
+__global__ void __launch_bounds__(ST_THREADS, 1) pn_stats_kernel(const StParams p)
 {
     extern __shared__ __align__(128) unsigned char st_smem[];
     // layout: [stages][2 tiles] | mbarriers | warp scratch | hist1 | hist2
     constexpr int NT = HAVE_INIT ? 2 : 1;
+    constexpr int NW = ST_THREADS / 32;
     double* tiles = reinterpret_cast<double*>(st_smem);
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(st_smem + (size_t)ST_STAGES * NT * ST_TILE_BYTES);
-    double* wscr = reinterpret_cast<double*>(bars + 8);                        // [8 warps][3][6]
-    unsigned* skip_s = reinterpret_cast<unsigned*>(wscr + 8 * 18);             // [4]
+    double* wscr = reinterpret_cast<double*>(bars + 8);                        // [NW warps][3][6]
+    unsigned* skip_s = reinterpret_cast<unsigned*>(wscr + NW * 18);            // [4]
     unsigned* hist1 = skip_s + 4;
     unsigned* hist2 = hist1 + 3 * p.bins1;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int grp = tid / ST_TILE, row = tid - grp * ST_TILE;
     const int nh1 = 3 * p.bins1, nh2 = p.hist2_smem ? 3 * p.bins2 * p.bins2 : 0;
 
-    const long long w_begin = (long long)blockIdx.x * p.items_per_block;
-    const long long w_end = min(w_begin + (long long)p.items_per_block, p.n_items);
+    // item indices fit an int: n_items = N/256 < 2^31 for any N the ABI accepts
+    const int w_begin = blockIdx.x * p.items_per_block;
+    const int w_end = (int)min((long long)w_begin + p.items_per_block, p.n_items);
     if (w_begin >= w_end) return;
 
-    for (int b = tid; b < nh1 + nh2; b += ST_TILE) hist1[b] = 0u;
+    for (int b = tid; b < nh1 + nh2; b += ST_THREADS) hist1[b] = 0u;
     if (tid < 4) skip_s[tid] = 0u;
     if (tid == 0) {
         for (int s = 0; s < ST_STAGES; ++s) st_mbar_init(st_smem_addr(&bars[s]), 1);
@@ -166,15 +180,15 @@ __global__ void __launch_bounds__(ST_TILE, 1) pn_stats_kernel(const StParams p)
     }
     __syncthreads();
 
-    auto item_range = [&](long long w, long long& start, int& cnt, int& g) {
-        g = (int)(w / p.tiles_per_group);
-        const long long t = w - (long long)g * p.tiles_per_group;
+    auto item_range = [&](int w, long long& start, int& cnt) {
+        const int g = w / p.tiles_per_group;
+        const long long t = w - g * p.tiles_per_group;
         start = (long long)g * p.group_size + t * ST_TILE;
         cnt = (int)min((long long)ST_TILE, p.group_size - t * ST_TILE);
     };
-    auto issue = [&](long long w, int stage) {       // one elected thread
-        long long start; int cnt, g;
-        item_range(w, start, cnt, g);
+    auto issue = [&](int w, int stage) {       // one elected thread
+        long long start; int cnt;
+        item_range(w, start, cnt);
         const uint32_t bar = st_smem_addr(&bars[stage]);
         const uint32_t bytes = (uint32_t)cnt * ST_ROW * 8u;
         st_mbar_expect_tx(bar, bytes * NT);
@@ -188,112 +202,118 @@ __global__ void __launch_bounds__(ST_TILE, 1) pn_stats_kernel(const StParams p)
     StAcc acc[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) acc[k].reset();
-    unsigned skip[3] = {0u, 0u, 0u};
 
-    int stage = 0;
-    uint32_t parity = 0;
-    for (long long w = w_begin; w < w_end; ++w) {
-        long long start; int cnt, g;
-        item_range(w, start, cnt, g);
-        st_mbar_wait(st_smem_addr(&bars[stage]), parity);
-        double rf[ST_ROW], ri[ST_ROW];
-        const bool have = tid < cnt;
-        if (have) {
-            const double* src = tiles + (size_t)stage * NT * ST_TILE * ST_ROW + tid * ST_ROW;
+    int w = w_begin + grp;                    // this consumer group's next item
+    const int g_first = w_begin / p.tiles_per_group, g_last = (w_end - 1) / p.tiles_per_group;
+    for (int g = g_first; g <= g_last; ++g) {
+        const int w_g_end = (int)min((long long)w_end, (long long)(g + 1) * p.tiles_per_group);
+        for (; w < w_g_end; w += ST_GROUPS) {
+            const int stage = grp;                                            // each group owns one slot
+            const uint32_t parity = (uint32_t)(((w - w_begin) / ST_GROUPS) & 1);
+            long long start; int cnt;
+            item_range(w, start, cnt);
+            st_mbar_wait(st_smem_addr(&bars[stage]), parity);
+            // final-state rows first: their dot products are formed before the initial-state rows are read, so the
+            // two 10-double rows are never live together (the kernel must fit 128 registers at 512 threads)
+            double ri[ST_ROW], df[3], di[3];
+            bool okf[3] = {false, false, false}, oki[3] = {true, true, true};
+            const bool have = row < cnt;
+            if (have) {
+                // 16-byte shared loads: rows are 80 B apart, so a quarter-warp covers 8 distinct 16-byte bank groups
+                const double2* src = reinterpret_cast<const double2*>(tiles + (size_t)stage * NT * ST_TILE * ST_ROW + row * ST_ROW);
+                double rf[ST_ROW];
 #pragma unroll
-            for (int c = 0; c < ST_ROW; ++c) rf[c] = src[c];
-            if (HAVE_INIT)
+                for (int c = 0; c < ST_ROW / 2; ++c) { const double2 v = src[c]; rf[2 * c] = v.x; rf[2 * c + 1] = v.y; }
+                st_unit_dots(rf, df, okf);
+                if (HAVE_INIT)
 #pragma unroll
-                for (int c = 0; c < ST_ROW; ++c) ri[c] = src[ST_TILE * ST_ROW + c];
-        }
-        const bool failed = have && p.steps && (p.steps[start + tid] < 0);
-        __syncthreads();                                   // every thread has read this stage
-        if (tid == 0 && w + ST_STAGES < w_end) issue(w + ST_STAGES, stage);
-        if (++stage == ST_STAGES) { stage = 0; parity ^= 1u; }
+                    for (int c = 0; c < ST_ROW / 2; ++c) { const double2 v = src[ST_TILE * ST_ROW / 2 + c]; ri[2 * c] = v.x; ri[2 * c + 1] = v.y; }
+            }
+            const bool failed = have && p.steps && (p.steps[start + row] < 0);
+            asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(ST_TILE) : "memory");     // this group has read the stage
+            if (row == 0 && w + ST_STAGES < w_end) issue(w + ST_STAGES, stage);
 
-        if (have) {
-            double df[3], di[3];
-            bool okf[3], oki[3] = {true, true, true};
-            st_unit_dots(rf, df, okf);
-            if (HAVE_INIT) st_unit_dots(ri, di, oki);
+            if (have) {
+                if (HAVE_INIT) st_unit_dots(ri, di, oki);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const bool ok = okf[k] && oki[k] && !failed;
-                if (!ok) { ++skip[k]; continue; }
-                if (HAVE_INIT) acc[k].add(di[k], df[k]);
-                if (p.bins1) atomicAdd(&hist1[k * p.bins1 + st_bin(df[k], p.bins1)], 1u);
-                if (HAVE_INIT && p.bins2) {
-                    const size_t cell = ((size_t)k * p.bins2 + st_bin(di[k], p.bins2)) * p.bins2 + st_bin(df[k], p.bins2);
-                    if (p.hist2_smem) atomicAdd(&hist2[cell], 1u);
-                    else atomicAdd(&p.hist2[(size_t)g * 3 * p.bins2 * p.bins2 + cell], 1ull);
+                for (int kk = 0; kk < 3; ++kk) {
+                    const bool ok = okf[kk] && oki[kk] && !failed;
+                    if (!ok) { atomicAdd(&skip_s[kk], 1u); continue; }      // rare: straight to the block counter
+                    if (HAVE_INIT) acc[kk].add(di[kk], df[kk]);
+                    if (p.bins1) atomicAdd(&hist1[kk * p.bins1 + st_bin(df[kk], p.bins1)], 1u);
+                    if (HAVE_INIT && p.bins2) {
+                        const size_t cell = ((size_t)kk * p.bins2 + st_bin(di[kk], p.bins2)) * p.bins2 + st_bin(df[kk], p.bins2);
+                        if (p.hist2_smem) atomicAdd(&hist2[cell], 1u);
+                        else atomicAdd(&p.hist2[(size_t)g * 3 * p.bins2 * p.bins2 + cell], 1ull);
+                    }
                 }
             }
         }
 
-        // ---- leaving group g (or the block's range): merge and flush ----
-        const bool last_of_group = (w + 1 == w_end) || ((int)((w + 1) / p.tiles_per_group) != g);
-        if (last_of_group) {
+        // ---- the block leaves ensemble g: merge (warp butterfly, then warps in order) and flush ----
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                StMom m = acc[k].moments();
+        for (int k = 0; k < 3; ++k) {
+            StMom m = acc[k].moments();
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) { StMom other = st_shfl_xor(m, o); st_merge(m, other); }
-                // the butterfly leaves every lane with a (not bitwise identical) total; lane 0's is the result
-                if (lane == 0) {
-                    double* q = wscr + (warp * 3 + k) * 6;
-                    q[0] = m.n; q[1] = m.mx; q[2] = m.my; q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
-                }
-                unsigned sk = skip[k];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) sk += __shfl_xor_sync(0xffffffffu, sk, o);
-                if (lane == 0 && sk) atomicAdd(&skip_s[k], sk);
-                acc[k].reset();
-                skip[k] = 0u;
+            for (int o = 1; o < 32; o <<= 1) { StMom other = st_shfl_xor(m, o); st_merge(m, other); }
+            // the butterfly leaves every lane with a (not bitwise identical) total; lane 0's is the result
+            if (lane == 0) {
+                double* q = wscr + (warp * 3 + k) * 6;
+                q[0] = m.n; q[1] = m.mx; q[2] = m.my; q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
             }
-            __syncthreads();
-            const size_t slot = (size_t)blockIdx.x + (size_t)g;        // unique per (block, group): both only grow
-            if (tid < 3) {
-                StMom m = {0, 0, 0, 0, 0, 0};
-                for (int ww = 0; ww < ST_TILE / 32; ++ww) {
-                    const double* q = wscr + (ww * 3 + tid) * 6;
-                    StMom o = {q[0], q[1], q[2], q[3], q[4], q[5]};
-                    st_merge(m, o);
-                }
-                double* r = p.records + (slot * 3 + tid) * 6;
-                r[0] = m.n; r[1] = m.mx; r[2] = m.my; r[3] = m.m2x; r[4] = m.m2y; r[5] = m.cxy;
-                p.rec_skipped[slot * 3 + tid] = skip_s[tid];
-            }
-            if (p.hist1)
-                for (int b = tid; b < nh1; b += ST_TILE)
-                    if (hist1[b]) { atomicAdd(&p.hist1[(size_t)g * nh1 + b], (unsigned long long)hist1[b]); hist1[b] = 0u; }
-            if (nh2)
-                for (int b = tid; b < nh2; b += ST_TILE)
-                    if (hist2[b]) { atomicAdd(&p.hist2[(size_t)g * nh2 + b], (unsigned long long)hist2[b]); hist2[b] = 0u; }
-            __syncthreads();
-            if (tid < 4) skip_s[tid] = 0u;
-            __syncthreads();
+            acc[k].reset();
         }
+        __syncthreads();
+        const size_t slot = (size_t)blockIdx.x + (size_t)g;        // unique per (block, ensemble): both only grow
+        if (tid < 3) {
+            StMom m = {0, 0, 0, 0, 0, 0};
+            for (int ww = 0; ww < NW; ++ww) {
+                const double* q = wscr + (ww * 3 + tid) * 6;
+                StMom o = {q[0], q[1], q[2], q[3], q[4], q[5]};
+                st_merge(m, o);
+            }
+            double* r = p.records + (slot * 3 + tid) * 6;
+            r[0] = m.n; r[1] = m.mx; r[2] = m.my; r[3] = m.m2x; r[4] = m.m2y; r[5] = m.cxy;
+            p.rec_skipped[slot * 3 + tid] = skip_s[tid];
+        }
+        if (p.hist1)
+            for (int b = tid; b < nh1; b += ST_THREADS)
+                if (hist1[b]) { atomicAdd(&p.hist1[(size_t)g * nh1 + b], (unsigned long long)hist1[b]); hist1[b] = 0u; }
+        if (nh2)
+            for (int b = tid; b < nh2; b += ST_THREADS)
+                if (hist2[b]) { atomicAdd(&p.hist2[(size_t)g * nh2 + b], (unsigned long long)hist2[b]); hist2[b] = 0u; }
+        __syncthreads();
+        if (tid < 4) skip_s[tid] = 0u;
+        __syncthreads();
     }
 }
 
-// One thread per (group, dot product): merge the per-block records of that group in block order.
-__global__ void pn_stats_finish_kernel(const StParams p, int n_blocks, double* __restrict__ r_out,
-                                       double* __restrict__ mom_out, unsigned long long* __restrict__ skipped_out)
+// One warp per (ensemble, dot product): the per-block records of that ensemble are merged lane-strided in block
+// order, then over the lanes with the same xor butterfly as in the main kernel (fixed order: deterministic).
+__global__ void __launch_bounds__(128) pn_stats_finish_kernel(const StParams p, int n_blocks, double* __restrict__ r_out,
+                                                              double* __restrict__ mom_out, unsigned long long* __restrict__ skipped_out)
 {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (j >= p.n_groups * 3) return;
     const int g = j / 3, k = j % 3;
     const long long w_lo = (long long)g * p.tiles_per_group, w_hi = w_lo + p.tiles_per_group - 1;
     const int b_lo = (int)(w_lo / p.items_per_block), b_hi = min((int)(w_hi / p.items_per_block), n_blocks - 1);
     StMom m = {0, 0, 0, 0, 0, 0};
     unsigned long long sk = 0;
-    for (int b = b_lo; b <= b_hi; ++b) {
+    for (int b = b_lo + lane; b <= b_hi; b += 32) {
         const size_t slot = (size_t)b + (size_t)g;
         const double* q = p.records + (slot * 3 + k) * 6;
         StMom o = {q[0], q[1], q[2], q[3], q[4], q[5]};
         st_merge(m, o);
         sk += p.rec_skipped[slot * 3 + k];
     }
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        StMom other = st_shfl_xor(m, o);
+        st_merge(m, other);
+        sk += __shfl_xor_sync(0xffffffffu, sk, o);
+    }
+    if (lane != 0) return;
     if (mom_out) {
         double* q = mom_out + (size_t)j * 6;
         q[0] = m.n; q[1] = m.n > 0 ? m.mx : nan(""); q[2] = m.n > 0 ? m.my : nan(""); q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
@@ -357,6 +377,7 @@ cudaError_t pn_launch_stats(const double* init, const double* fin, const int* st
     p.init = init; p.fin = fin; p.steps = steps; p.n = n; p.group_size = gs; p.n_groups = (int)G;
     p.tiles_per_group = (int)((gs + ST_TILE - 1) / ST_TILE);
     p.n_items = G * p.tiles_per_group;
+    if (p.n_items > 0x7fffffffLL) return cudaErrorInvalidValue;
     p.items_per_block = (int)((p.n_items + n_blocks - 1) / n_blocks);
     n_blocks = (int)((p.n_items + p.items_per_block - 1) / p.items_per_block);
     p.bins1 = hist1 ? bins1 : 0;
@@ -365,22 +386,24 @@ cudaError_t pn_launch_stats(const double* init, const double* fin, const int* st
     p.rec_skipped = (unsigned long long*)((char*)scratch + (size_t)(n_blocks + G + 1) * 3 * 6 * sizeof(double));
     p.hist1 = hist1; p.hist2 = hist2;
     const int nt = init ? 2 : 1;
-    const size_t fixed = (size_t)ST_STAGES * nt * ST_TILE_BYTES + 64 + 8 * 18 * sizeof(double) + 16 + 3 * (size_t)p.bins1 * 4;
+    const size_t fixed = (size_t)ST_STAGES * nt * ST_TILE_BYTES + 64 + (ST_THREADS / 32) * 18 * sizeof(double) + 16 + 3 * (size_t)p.bins1 * 4;
     const size_t h2 = 3 * (size_t)p.bins2 * p.bins2 * 4;
     const size_t cap = 220 * 1024;
     if (fixed > cap) return cudaErrorInvalidValue;
     p.hist2_smem = (p.bins2 > 0 && fixed + h2 <= cap) ? 1 : 0;
     const size_t shm = fixed + (p.hist2_smem ? h2 : 0);
-    if (init) {
-        if ((e = cudaFuncSetAttribute(pn_stats_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm)) != cudaSuccess) return e;
-        pn_stats_kernel<true><<<n_blocks, ST_TILE, shm, s>>>(p);
-    } else {
-        if ((e = cudaFuncSetAttribute(pn_stats_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm)) != cudaSuccess) return e;
-        pn_stats_kernel<false><<<n_blocks, ST_TILE, shm, s>>>(p);
+    // opt in to large dynamic shared memory once per process (a host-side call per launch leaves the GPU idle)
+    static bool attr_done = false;
+    if (!attr_done) {
+        if ((e = cudaFuncSetAttribute(pn_stats_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cap)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(pn_stats_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cap)) != cudaSuccess) return e;
+        attr_done = true;
     }
+    if (init) pn_stats_kernel<true><<<n_blocks, ST_THREADS, shm, s>>>(p);
+    else pn_stats_kernel<false><<<n_blocks, ST_THREADS, shm, s>>>(p);
     ++g_pn_launches;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    pn_stats_finish_kernel<<<(int)((G * 3 + 127) / 128), 128, 0, s>>>(p, n_blocks, r_out, mom_out, skipped_out);
+    pn_stats_finish_kernel<<<(int)((G * 3 + 3) / 4), 128, 0, s>>>(p, n_blocks, r_out, mom_out, skipped_out);
     ++g_pn_launches;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     if (p.bins2 && (hist2_max || hist2_norm)) {
