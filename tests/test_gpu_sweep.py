@@ -1,0 +1,63 @@
+"""NEXT-3: parameter sweeps as one launch (Figs. 6-7).  G ensembles laid end to end:
+one pn_generate, one pn_integrate, one pn_statistics(group_size).  Checked against the oracle chain
+(generator oracle -> integrator oracle -> statistics oracle) per ensemble, and against what the paper says
+about the curves (soft pins: two printed digits / qualitative statements)."""
+import numpy as np
+import pytest
+
+from oracle import pn_gen_oracle as G
+from oracle import pn_stats_oracle as S
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+N_E = 20000
+OMEGA0, OMEGAF, TOL = 0.00395, 0.05, 5e-7
+
+
+def specs():
+    out = []
+    for e, m1 in enumerate((0.5, 0.45, 0.4, 0.3)):                     # Fig. 6: chi = 1, m1 varied
+        q = (1 - m1) / m1
+        out.append(dict(key=(2024, e), omega0=OMEGA0, q=(q, q), chi1=(1.0, 1.0), chi2=(1.0, 1.0)))
+    for e, chi in enumerate((0.3, 0.5, 0.7)):                          # Fig. 7: m1 = m2, chi varied
+        out.append(dict(key=(2025, e), omega0=OMEGA0, q=(1.0, 1.0), chi1=(chi, chi), chi2=(chi, chi)))
+    return out
+
+
+def test_sweep_one_launch_against_oracle_chain(oracle):
+    import paper_0908_3889_b200 as pn
+
+    sp = specs()
+    n = N_E * len(sp)
+    d_y0 = torch.empty(n, 10, dtype=torch.float64, device="cuda")
+    d_m = torch.empty(n, 2, dtype=torch.float64, device="cuda")
+    pn.pn_generate([pn.make_ensemble(**s) for s in sp], N_E, d_y0, d_m)
+    d_yf = torch.empty_like(d_y0)
+    d_steps = torch.empty(n, dtype=torch.int32, device="cuda")
+    pn.pn_integrate(d_y0, d_m, OMEGA0, OMEGAF, TOL, TOL, pn.PN_FP64, d_yf, d_steps)
+    r = torch.zeros(len(sp), 3, dtype=torch.float64, device="cuda")
+    mom = torch.zeros(len(sp), 3, 6, dtype=torch.float64, device="cuda")
+    h2 = torch.zeros(len(sp), 3, 79, 79, dtype=torch.int64, device="cuda")
+    pn.pn_statistics(d_y0, d_yf, d_steps, group_size=N_E, bins2=79, pearson_r=r, moments=mom, hist2=h2)
+    r, mom, h2 = r.cpu().numpy(), mom.cpu().numpy(), h2.cpu().numpy()
+    assert np.all(mom[..., 0] == N_E) and np.all(h2.sum(axis=(2, 3)) == N_E)
+
+    # oracle chain per ensemble (different step sequences at tol 5e-7: final dots differ by ~1e-5, r by less)
+    r_ref = np.zeros_like(r)
+    for e, s in enumerate(sp):
+        y0, m = G.generate(G.make_spec(**s), N_E)
+        assert np.abs(y0 - d_y0[e * N_E:(e + 1) * N_E].cpu().numpy()).max() <= 4e-16
+        o = oracle.integrate(y0, m, OMEGAF, TOL, TOL)
+        r_ref[e] = S.statistics(y0, o["final"], o["steps"])["r"][0]
+    assert np.abs(r - r_ref).max() < 2e-4, np.abs(r - r_ref).max()
+
+    # equal mass, maximal spin: 0.99 and 0.65
+    assert 0.98 <= r[0, 0] <= 0.995 and 0.62 <= r[0, 1] <= 0.68 and 0.62 <= r[0, 2] <= 0.68
+    # PAPER.md:148-150, Fig. 6: "the correlation drops quickly as the masses become uneven"
+    assert r[0, 0] > r[1, 0] > r[2, 0] > r[3, 0] and r[3, 0] < 0.5 * r[0, 0]
+    # PAPER.md:156, Fig. 7: r(S1^.S2^) > 0.98 for every chi at equal masses, while r(S_j^.L^) varies and is the
+    # same for j = 1, 2 ("both BHs enter symmetrically")
+    assert np.all(r[4:, 0] > 0.98)
+    assert np.abs(r[4:, 1] - r[4:, 2]).max() < 0.03
+    assert np.ptp(np.concatenate([r[4:, 1], r[:1, 1]])) > 0.05
