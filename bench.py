@@ -136,7 +136,7 @@ def run_ours(args, cfg):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    prec = pn.PN_FP32 if cfg.precision == "fp32" else pn.PN_FP64
+    prec = {"fp32": pn.PN_FP32, "mixed": pn.PN_MIXED}.get(cfg.precision, pn.PN_FP64)
 
     # every rank integrates its own seeded batch of the full workload size (weak scaling)
     from paper_0908_3889_b200 import sharding
@@ -242,12 +242,13 @@ def run_ours(args, cfg):
             dist.destroy_process_group()
         return
     # roofline of the dominant kernel (the integrator): algorithmic flops / CUDA-event duration
-    lanes = FP32_LANES_PER_SM if prec == pn.PN_FP32 else FP64_LANES_PER_SM
+    lanes = FP64_LANES_PER_SM if prec == pn.PN_FP64 else FP32_LANES_PER_SM
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
     sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
     peak_nominal = sms * lanes * 2 * sm_max * 1e6 / 1e12
-    peak_meas, peak_mhz = pn.pn_measure_fma_peak(prec, 0.5)
+    peak_prec = pn.PN_FP64 if prec == pn.PN_FP64 else pn.PN_FP32       # the pipe the slopes are computed on
+    peak_meas, peak_mhz = pn.pn_measure_fma_peak(peak_prec, 0.5)
     flops_launch = float(np.mean(trial_steps)) * F_STEP + n * F_RHS
     k_ms = float(np.mean(kern_ms))
     achieved = flops_launch / (k_ms * 1e-3) / 1e12
@@ -256,7 +257,7 @@ def run_ours(args, cfg):
         "metric": "inspirals_per_sec", "value": total_inspirals / (ms_step * 1e-3), "unit": "inspirals/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if prec == pn.PN_FP32 else "f64", "data": "synthetic",
+        "dtype": {pn.PN_FP32: "f32", pn.PN_MIXED: "f32 slopes + f64 state"}.get(prec, "f64"), "data": "synthetic",
         "config": {"workload": cfg.name, "n_inspirals_per_gpu": n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
                    "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "queue": "input order" if args.input_order else "longest-expected-first", "parallelism": f"batch-sharded x{world}",
                    "l2": "256 MiB memset between steps, inside the timed region (<0.1 % of a step)"},
@@ -275,7 +276,7 @@ def run_ours(args, cfg):
                      "flops_per_trial_step": F_STEP, "flops_per_rhs": F_RHS,
                      "frac_with_oracle_as_printed_count": (float(np.mean(trial_steps)) * F_STEP_ORACLE + n * F_RHS_ORACLE)
                      / (k_ms * 1e-3) / 1e12 / peak_nominal,
-                     "fma_issue_cycles_by_register_sources": {str(k): pn.pn_measure_fma_operands(prec, k) for k in (1, 2, 3)}},
+                     "fma_issue_cycles_by_register_sources": {str(k): pn.pn_measure_fma_operands(peak_prec, k) for k in (1, 2, 3)}},
         "e2e": {"value": total_inspirals / e2e_s, "unit": "inspirals/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,

@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-typedef enum { PN_FP64 = 0, PN_FP32 = 1 } pn_precision;
+typedef enum { PN_FP64 = 0, PN_FP32 = 1, PN_MIXED = 2 } pn_precision;
 
 typedef enum {
     PN_OK = 0,
@@ -62,6 +62,9 @@ typedef enum {
  *               omega and L^, |S_i(0)| for the components of S_i (R6-R7).
  *   precision   PN_FP64: all arithmetic in double.  PN_FP32: state, slopes, RHS and error norm in
  *               float; time accumulation, step counters and all arrays of this interface in double.
+ *               PN_MIXED: as PN_FP32, but the state is carried in double: an accepted step adds the float
+ *               increment sum_s b_s K_s to it, and omega is compared with omega_f in double ("only a few
+ *               critical computations in double").  Usable down to rtol ~ 1e-8.
  *   out_final   [N][10] final states (the omega slot holds the landed omega, within tau of omega_f).
  *   out_steps   [N] trial steps taken (accepted + rejected + discarded landing trials), or a
  *               negative PN_FAIL_* code.  RHS evaluations of a system = 6*steps + 1.
@@ -79,7 +82,7 @@ typedef struct pn_options {
     int max_steps;         /* per system; <= 0: 10,000,000 */
     unsigned term_mask;    /* tests only.  bit k (0..7) keeps the (M omega)^{k/3} term of the brace of
                               Eq. (1); bit 16 keeps the spin terms of Eq. (1).  0: everything */
-    double tau_land;       /* landing tolerance |omega - omega_f| <= tau*omega_f; <= 0: 1e-13 (FP64), 3e-7 (FP32) */
+    double tau_land;       /* landing tolerance |omega - omega_f| <= tau*omega_f; <= 0: 1e-13 (FP64), 3e-7 (FP32), 1e-8 (MIXED) */
     int layout;            /* 0: AoS [N][10] / [N][2] as above.  1: SoA [10][N] / [2][N] for
                               init_states, masses and out_final (no staging pass) */
     int host_buffers;      /* != 0: every array argument is a HOST pointer (see Conventions) */

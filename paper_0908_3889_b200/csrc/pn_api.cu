@@ -80,7 +80,7 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     if (N < 0 || N > 0x7fffffffLL / 16) return PN_EINVAL;
     if (N == 0) return PN_OK;
     if (!init_states || !masses || !out_final || !out_steps) return PN_EINVAL;
-    if (precision != PN_FP64 && precision != PN_FP32) return PN_EINVAL;
+    if (precision != PN_FP64 && precision != PN_FP32 && precision != PN_MIXED) return PN_EINVAL;
     const bool fixed = o.fixed_steps > 0;
     if (!fixed) {
         if (!(rtol > 0.0) || !(atol >= 0.0) || !(omegaf > 0.0)) return PN_EINVAL;
@@ -148,7 +148,7 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     p.steps = d_steps; p.time = d_time; p.rejected = d_rej;
     p.n = n;
     p.omega0 = omega0; p.omegaf = omegaf; p.rtol = rtol; p.atol = atol; p.h0 = o.h0;
-    p.tau = o.tau_land > 0.0 ? o.tau_land : (precision == PN_FP64 ? 1e-13 : 3e-7);
+    p.tau = o.tau_land > 0.0 ? o.tau_land : (precision == PN_FP64 ? 1e-13 : (precision == PN_MIXED ? 1e-8 : 3e-7));
     p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
     p.fixed_steps = fixed ? o.fixed_steps : 0;
     p.mask = o.term_mask;

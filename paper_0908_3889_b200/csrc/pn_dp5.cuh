@@ -40,10 +40,13 @@
 // Trial step from (y, K1 = h f(y)) with step h.  All slopes are "scaled" (K_s = h k_s, see pn_rhs.cuh), so
 // every coefficient below is a compile-time constant.  Outputs y_new (5th order), K7 = h f(y_new) and the
 // error estimate err = sum_s e_s K_s.  6 RHS evaluations, 200 + 60 FMAs.
-template <bool SLOW, typename real>
+// WANT_DY (mixed precision): the increment dy = sum_s b_s K_s is formed on its own and
+// y_new = y + dy, so that the caller can add dy to a higher-precision copy of the state.
+template <bool SLOW, typename real, bool WANT_DY = false>
 __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K1)[10], real h,
                                              const PnConsts<real>& c, const PnUni<real>& u, const PnBase<real>& base,
-                                             real (&ynew)[10], real (&K7)[10], real (&err)[10], PnBase<real>& base_new, bool& bad)
+                                             real (&ynew)[10], real (&K7)[10], real (&err)[10], PnBase<real>& base_new, bool& bad,
+                                             real* dy = nullptr)
 {
     real K2[10], K3[10], K4[10], K5[10], K6[10], ys[10];
     real r_tmp, l_tmp;
@@ -72,9 +75,16 @@ __device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K
     pn_rhs<SLOW>(ys, c, u, sc, base, K6, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
-        ynew[i] = pn_fma((real)DP_B6, K6[i],
-                         pn_fma((real)DP_B5, K5[i],
-                                pn_fma((real)DP_B4, K4[i], pn_fma((real)DP_B3, K3[i], pn_fma((real)DP_B1, K1[i], y[i])))));
+        if (WANT_DY) {
+            dy[i] = pn_fma((real)DP_B6, K6[i],
+                           pn_fma((real)DP_B5, K5[i],
+                                  pn_fma((real)DP_B4, K4[i], pn_fma((real)DP_B3, K3[i], (real)DP_B1 * K1[i]))));
+            ynew[i] = y[i] + dy[i];
+        } else {
+            ynew[i] = pn_fma((real)DP_B6, K6[i],
+                             pn_fma((real)DP_B5, K5[i],
+                                    pn_fma((real)DP_B4, K4[i], pn_fma((real)DP_B3, K3[i], pn_fma((real)DP_B1, K1[i], y[i])))));
+        }
         err[i] = pn_fma((real)DP_E6, K6[i],
                         pn_fma((real)DP_E5, K5[i],
                                pn_fma((real)DP_E4, K4[i], pn_fma((real)DP_E3, K3[i], (real)DP_E1 * K1[i]))));

@@ -176,7 +176,11 @@ __device__ __forceinline__ void pn_load_record(const void* seed, int i, real (&o
 // SMEM = true (FP64 only): k2..k5 and the error partial live in dynamic shared memory (pn_dp5_smem.cuh)
 // SLOW = true: the redo pass.  Systems whose step left the range of the cbrt/log series in the fast kernel
 // are re-integrated from their initial state with the wide-range evaluation (pn_rhs.cuh) in every stage.
-template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW>
+// MIXED = true (real = float only; PN_MIXED): slopes, RHS, stage sums and error norm in float, but the
+// state itself is carried in double: an accepted step adds the float increment dy = sum b_s K_s to the double copy,
+// so the per-step rounding error is eps32 |dy| instead of eps32 |y| ("only a few critical computations in
+// double"); omega is compared with omega_f in double.
+template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
 {
     const unsigned n_queue = SLOW ? *p.redo_count : (unsigned)p.n;     // length of the work queue
@@ -191,14 +195,15 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     // lane state.  k1 holds the SCALED slope h*f(y).  Idle lanes are frozen (h = 0, k1 = 0) on a benign
     // dummy state, so the lock-step arithmetic stays finite and never leaves the series' range.
     real y[10], k1[10];
+    double yd[10];                   // MIXED only: the state in double (y is its rounded copy)
     PnConsts<real> c;
     PnBase<real> base;
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
     pn_make_consts<real>(0.5, 0.5, 0u, c);
 #pragma unroll
-    for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; }
-    y[0] = (real)0.01; y[9] = (real)1;
+    for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; yd[i] = 0.0; }
+    y[0] = (real)0.01; y[9] = (real)1; yd[0] = 0.01; yd[9] = 1.0;
     pn_base_init(c.M * y[0], base);
     real h = (real)0;
     float atS1 = (float)p.atol, atS2 = (float)p.atol;
@@ -234,6 +239,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                     } else {
 #pragma unroll
                         for (int j = 0; j < 10; ++j) { y[j] = rec[j]; k1[j] = rec[10 + j]; }
+                        if constexpr (MIXED)
+#pragma unroll
+                            for (int j = 0; j < 10; ++j) yd[j] = __ldg(p.y0 + (size_t)j * p.n + i);
                         c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
                         c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
                         c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
@@ -252,10 +260,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         }
 
         // ---------------- one DP5(4) trial step, all lanes, one basic block ----------------
-        real ynew[10], k7[10], err[10];
+        real ynew[10], k7[10], err[10], dy[10];
         PnBase<real> base_new;
         bool bad = false;
         if constexpr (SMEM) pn_dp5_trial_smem<SLOW, BLOCK>(y, k1, h, c, u, base, sm, ynew, k7, err, base_new, bad);
+        else if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad, dy);
         else pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
         // fast kernel: a lane whose step left the series' range (|1 - x/x0| > 0.03, only at very loose
         // tolerances) hands its system to the redo pass and frees itself; redo kernel: `bad` means omega more
@@ -280,9 +289,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         const bool finite = E2 <= FLT_MAX;                 // false for NaN and inf
         const bool ok = E2 <= 1.0f;
         const real om_new = ynew[0];
-        const bool over = active && ok && (om_new > om_hi);            // passes error control, overshoots omega_f
+        // omega_new - omega_f; MIXED forms it in double from the double state (float could not resolve tau = 1e-8)
+        real om_ex = om_new - omegaf;
+        if constexpr (MIXED) om_ex = (real)((yd[0] + (double)dy[0]) - p.omegaf);
+        const bool over = active && ok && (MIXED ? (om_ex > om_tol) : (om_new > om_hi));   // passes error control, overshoots omega_f
         const bool accept = active && ok && !over;
-        const bool landed = accept && (pn_abs(om_new - omegaf) <= om_tol);
+        const bool landed = accept && (pn_abs(om_ex) <= om_tol);
         const bool reject = active && finite && !ok;
         real ratio = (real)fminf(fmaxf(fac, 0.2f), (after_reject || reject) ? 1.0f : 5.0f);   // h_next / h
         if (!active) ratio = (real)0;                      // idle (or just handed to the redo pass): frozen
@@ -295,7 +307,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         if (over || (accept && landing)) {
             // landing on omega_f (R12): Newton on h with d(omega_new)/dh ~ k7[0]/h.
             // over: discard the step and retry from the same state; accepted-short: first guess from the new state
-            const real d = (over ? (om_new - omegaf) : (omegaf - om_new)) / k7[0];
+            const real d = (over ? om_ex : -om_ex) / k7[0];
             ratio = over ? pn_max((real)1 - d, (real)0.1) : pn_min((real)1, d);
             if (over) { ++tot_land; ++nland; landing = true; }
         }
@@ -312,8 +324,15 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         code = !finite ? PN_F_NONFINITE : code;
         code = active ? code : 0;
         if (code != 0) {
-            if (accept) pn_store_result(p, idx, ynew, code, t, nrej);
-            else pn_store_result(p, idx, y, code, t, nrej);
+            if constexpr (MIXED) {
+                double yo[10];
+#pragma unroll
+                for (int i = 0; i < 10; ++i) yo[i] = accept ? yd[i] + (double)dy[i] : yd[i];
+                pn_store_result(p, idx, yo, code, t, nrej);
+            } else {
+                if (accept) pn_store_result(p, idx, ynew, code, t, nrej);
+                else pn_store_result(p, idx, y, code, t, nrej);
+            }
             if (code < 0) {
                 atomicMax(p.status, code == PN_F_NONFINITE ? PN_ST_ENONFINITE : PN_ST_ENOTCONVERGED);
                 ++tot_fail;
@@ -325,7 +344,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
 #pragma unroll
         for (int i = 0; i < 10; ++i) {
             k1[i] = ratio * (accept ? k7[i] : k1[i]);
-            y[i] = accept ? ynew[i] : y[i];
+            if constexpr (MIXED) {
+                yd[i] = accept ? yd[i] + (double)dy[i] : yd[i];      // the one double-precision operation per component
+                y[i] = (real)yd[i];
+            } else {
+                y[i] = accept ? ynew[i] : y[i];
+            }
         }
         base.r0 = accept ? base_new.r0 : base.r0;
         base.r03 = accept ? base_new.r03 : base.r03;
@@ -402,10 +426,10 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
 
 unsigned long long g_pn_launches = 0;
 
-template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW>
+template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false>
 static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
-    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM, SLOW>;
+    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM, SLOW, MIXED>;
     const int shm = SMEM ? PN_SM_SLOTS * BLOCK * (int)sizeof(double) : 0;
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t e;
@@ -463,6 +487,7 @@ cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int bloc
         // redo pass for systems that left the series' range; its queue length is read on the device
         return launch_adaptive<double, 128, 2, false, true>(p, grid_blocks, s);
     }
+    if (precision == 2) return launch_adaptive<float, 128, 3, false, false, true>(p, grid_blocks, s);   // PN_MIXED
     if (block_threads == 128) return launch_adaptive<float, 128, 4, false, false>(p, grid_blocks, s);
     return launch_adaptive<float, 256, 2, false, false>(p, grid_blocks, s);
 }

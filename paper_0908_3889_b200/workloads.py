@@ -46,6 +46,9 @@ CONFIGS = {
     "C4f": Config("C4f", 1 << 22, 3, 0.01, 0.05, (0.4 / 0.6, 0.4 / 0.6), (0.9, 0.9), (1.0, 1.0),
                   s1_fixed_tilt_deg=60.0, m1_fixed=0.6, precision="fp32", rtol=1e-5, atol=1e-7),
     "C5": Config("C5", 1 << 18, 4, 0.001, 0.05, (0.25, 1.0), (0.0, 1.0), (0.0, 1.0)),
+    # not a BASELINE.json config: C4 in mixed precision (float slopes, double state)
+    "C4m": Config("C4m", 1 << 22, 3, 0.01, 0.05, (0.4 / 0.6, 0.4 / 0.6), (0.9, 0.9), (1.0, 1.0),
+                  s1_fixed_tilt_deg=60.0, m1_fixed=0.6, precision="mixed", rtol=1e-7, atol=1e-9),
 }
 
 
