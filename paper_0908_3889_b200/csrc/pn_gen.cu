@@ -17,30 +17,8 @@
 
 #define GEN_TILE 256
 
-#define PHILOX_M0 0xD2E7470EE14C6C93ULL
-#define PHILOX_M1 0xCA5A826395121157ULL
-#define PHILOX_W0 0x9E3779B97F4A7C15ULL
-#define PHILOX_W1 0xBB67AE8584CAA73BULL
+#include "pn_philox.cuh"
 
-// word (e & 3) of Philox4x64-10(counter = (e >> 2) + 1, key)
-__device__ __forceinline__ unsigned long long gen_raw(unsigned long long k0, unsigned long long k1, unsigned long long e)
-{
-    unsigned long long c0 = (e >> 2) + 1ull, c1 = 0ull, c2 = 0ull, c3 = 0ull;
-#pragma unroll
-    for (int round = 0; round < 10; ++round) {
-        if (round > 0) { k0 += PHILOX_W0; k1 += PHILOX_W1; }
-        const unsigned long long hi0 = __umul64hi(PHILOX_M0, c0), lo0 = PHILOX_M0 * c0;
-        const unsigned long long hi1 = __umul64hi(PHILOX_M1, c2), lo1 = PHILOX_M1 * c2;
-        const unsigned long long n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-    }
-    const unsigned w = (unsigned)(e & 3ull);
-    return w == 0 ? c0 : (w == 1 ? c1 : (w == 2 ? c2 : c3));
-}
-__device__ __forceinline__ double gen_uniform(unsigned long long k0, unsigned long long k1, unsigned long long e)
-{
-    return (double)(gen_raw(k0, k1, e) >> 11) * (1.0 / 9007199254740992.0);
-}
 // lo + (hi - lo) u without contraction (the reference recipe rounds the product, then the sum)
 __device__ __forceinline__ double gen_lerp(double lo, double hi, double u)
 {
