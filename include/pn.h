@@ -188,6 +188,36 @@ typedef struct pn_ensemble {
 int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,
                 double* init_states, double* masses, const struct pn_options* opt);
 
+/*
+ * pn_selfcheck -- the paper's cross-check ("a random ~1 % subset" evolved in double precision next to
+ * the single-precision GPU run and compared afterwards), on the device.
+ *   selection   system i is checked iff u_i < fraction, u_i = element i of the uniform stream of `key`
+ *               (Philox4x64-10 in numpy.random.Philox's layout, as in pn_generate); expected subset size fraction*N.
+ *   reference   the selected systems are re-integrated from init_states by pn_integrate in PN_FP64 at
+ *               (rtol_ref, atol_ref) (<= 0: 1e-10, 1e-12) to omegaf.
+ *   comparison  per unit dot product (S1^.S2^, S1^.L^, S2^.L^; norms from the states) the largest
+ *               |d(final_states[i]) - d(reference)| over the subset and the lowest index where it occurs; the largest
+ *               |times[i]/t_ref - 1| if times != NULL.  Systems whose reference failed are counted and left out.
+ *   init_states, masses, final_states [N][10] / [N][2] / [N][10] AoS, times [N] or NULL: DEVICE pointers
+ *               (host with opt->host_buffers).  out: HOST struct.  checked_indices: DEVICE (host with host_buffers)
+ *               array of capacity >= max_indices receiving the sorted subset, or NULL.
+ * Synchronous (opt->async is rejected).  Deterministic.  Returns the status of the reference integration.
+ */
+typedef struct pn_check_out {
+    int size;                     /* = sizeof(pn_check_out); checked */
+    long long n_checked;          /* size of the subset */
+    long long n_failed_ref;       /* subset systems whose FP64 reference integration failed */
+    double max_dot_dev[3];        /* worst absolute deviation per dot product (0 if nothing comparable) */
+    long long worst_index[3];     /* system index of that deviation, -1 if none */
+    double max_time_rel_dev;      /* worst relative deviation of the final time (0 without times) */
+    float ms_reference;           /* duration of the reference integrator kernels, CUDA events */
+} pn_check_out;
+
+int pn_selfcheck(const double* init_states, const double* masses, const double* final_states, const double* times,
+                 long long N, double omegaf, double fraction, const unsigned long long key[2], double rtol_ref,
+                 double atol_ref, pn_check_out* out, long long* checked_indices, long long max_indices,
+                 const struct pn_options* opt);
+
 /* Worst pn_status of the async calls enqueued on `stream` since the last pn_stream_status; synchronises it. */
 int pn_stream_status(void* stream);
 

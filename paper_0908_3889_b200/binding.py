@@ -18,7 +18,7 @@ PN_FP64, PN_FP32, PN_MIXED = 0, 1, 2
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_generate", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_generate", "pn_selfcheck", "pn_stream_status",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -52,6 +52,11 @@ def make_ensemble(key, omega0, q=(1.0, 1.0), chi1=(1.0, 1.0), chi2=(1.0, 1.0), m
     return e
 
 
+class PnCheckOut(C.Structure):
+    _fields_ = [("size", C.c_int), ("n_checked", C.c_longlong), ("n_failed_ref", C.c_longlong), ("max_dot_dev", C.c_double * 3),
+                ("worst_index", C.c_longlong * 3), ("max_time_rel_dev", C.c_double), ("ms_reference", C.c_float)]
+
+
 class PnError(RuntimeError):
     def __init__(self, status, msg):
         super().__init__(msg)
@@ -76,6 +81,8 @@ def load():
         lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_statistics.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
         lib.pn_generate.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, vp, vp, C.POINTER(PnOptions)]
+        lib.pn_selfcheck.argtypes = [vp, vp, vp, vp, ll, d, d, C.POINTER(C.c_ulonglong), d, d, C.POINTER(PnCheckOut), vp, ll,
+                                     C.POINTER(PnOptions)]
         lib.pn_stream_status.argtypes = [vp]
         lib.pn_measure_fma_peak.argtypes = [i, d, C.POINTER(d), C.POINTER(d)]
         lib.pn_measure_fma_operands.argtypes = [i, i, C.POINTER(d)]
@@ -184,6 +191,25 @@ def pn_generate(ensembles, n_total, init_states, masses, *, first=0, count=None,
         opts["host_buffers"] = True
     o = make_options(**opts)
     return _check(lib.pn_generate(arr, len(ens), int(n_total), int(first), count, _ptr(init_states), _ptr(masses), C.byref(o)))
+
+
+def pn_selfcheck(init_states, masses, final_states, omegaf, *, fraction=0.01, key=(0, 0), times=None, rtol_ref=0.0,
+                 atol_ref=0.0, checked_indices=None, allow_failures=False, **opts):
+    """pn_selfcheck of include/pn.h (the paper's 1 % double-precision cross-check).  Returns a dict."""
+    lib = load()
+    n = int(final_states.shape[0])
+    if _is_host(final_states):
+        opts["host_buffers"] = True
+    o = make_options(**opts)
+    out = PnCheckOut()
+    out.size = C.sizeof(PnCheckOut)
+    k = (C.c_ulonglong * 2)(int(key[0]), int(key[1]))
+    cap = 0 if checked_indices is None else int(checked_indices.shape[0])
+    st = lib.pn_selfcheck(_ptr(init_states), _ptr(masses), _ptr(final_states), _ptr(times), n, float(omegaf), float(fraction), k,
+                          float(rtol_ref), float(atol_ref), C.byref(out), _ptr(checked_indices), cap, C.byref(o))
+    _check(st, allow=(PN_ENOTCONVERGED, PN_ENONFINITE, PN_EINVAL) if allow_failures else ())
+    return dict(status=st, n_checked=int(out.n_checked), n_failed_ref=int(out.n_failed_ref), max_dot_dev=list(out.max_dot_dev),
+                worst_index=list(out.worst_index), max_time_rel_dev=float(out.max_time_rel_dev), ms_reference=float(out.ms_reference))
 
 
 def pn_stream_status(stream=None):

@@ -41,7 +41,7 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts, g_st_scratch, g_st_in, g_st_out, g_gen_specs, g_gen_y, g_gen_m;
+static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts, g_st_scratch, g_st_in, g_st_out, g_gen_specs, g_gen_y, g_gen_m, g_ck_idx, g_ck_tmp, g_ck_sub, g_ck_out, g_ck_in;
 static cudaEvent_t g_ev[5];
 static bool g_ev_ok = false;
 static float g_ms[4] = {0, 0, 0, 0};
@@ -381,6 +381,86 @@ extern "C" int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_
     return PN_OK;
 }
 
+extern "C" int pn_selfcheck(const double* init_states, const double* masses, const double* final_states, const double* times,
+                            long long N, double omegaf, double fraction, const unsigned long long key[2], double rtol_ref,
+                            double atol_ref, pn_check_out* out, long long* checked_indices, long long max_indices,
+                            const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (!out || out->size != (int)sizeof(pn_check_out) || !key || N < 0 || N > 0x7fffffffLL / 16 || o.async || o.layout != 0 ||
+        !(fraction >= 0.0) || !(fraction <= 1.0) || !(omegaf > 0.0))
+        return PN_EINVAL;
+    if (N > 0 && (!init_states || !masses || !final_states)) return PN_EINVAL;
+    if (!(rtol_ref > 0.0)) rtol_ref = 1e-10;
+    if (!(atol_ref > 0.0)) atol_ref = 1e-12;
+    out->n_checked = out->n_failed_ref = 0;
+    out->max_time_rel_dev = 0.0; out->ms_reference = 0.0f;
+    for (int k = 0; k < 3; ++k) { out->max_dot_dev[k] = 0.0; out->worst_index[k] = -1; }
+    if (N == 0) return PN_OK;
+    cudaStream_t s = (cudaStream_t)o.stream;
+    int rc;
+    const double* d_init = init_states; const double* d_m = masses; const double* d_fin = final_states; const double* d_t = times;
+    if (o.host_buffers) {
+        const size_t rows = sizeof(double) * (size_t)N;
+        if ((rc = g_ck_in.ensure(rows * 23)) != PN_OK) return rc;
+        double* q = (double*)g_ck_in.p;
+        CK(cudaMemcpyAsync(q, init_states, rows * 10, cudaMemcpyHostToDevice, s)); d_init = q; q += 10 * N;
+        CK(cudaMemcpyAsync(q, final_states, rows * 10, cudaMemcpyHostToDevice, s)); d_fin = q; q += 10 * N;
+        CK(cudaMemcpyAsync(q, masses, rows * 2, cudaMemcpyHostToDevice, s)); d_m = q; q += 2 * N;
+        if (times) { CK(cudaMemcpyAsync(q, times, rows, cudaMemcpyHostToDevice, s)); d_t = q; }
+    }
+    // 1. selection (sorted index list + count)
+    const size_t tb = pn_check_select_temp_bytes(N);
+    if ((rc = g_ck_idx.ensure(sizeof(long long) * ((size_t)N + 1))) != PN_OK) return rc;
+    if ((rc = g_ck_tmp.ensure(tb)) != PN_OK) return rc;
+    long long* d_idx = (long long*)g_ck_idx.p;
+    long long* d_cnt = d_idx + N;
+    CK(pn_launch_check_select(N, fraction, key[0], key[1], d_idx, d_cnt, g_ck_tmp.p, tb, s));
+    long long m = 0;
+    CK(cudaMemcpyAsync(&m, d_cnt, sizeof m, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    out->n_checked = m;
+    if (checked_indices && m > 0) {
+        if (m > max_indices) return PN_EINVAL;
+        CK(cudaMemcpyAsync(checked_indices, d_idx, sizeof(long long) * (size_t)m,
+                           o.host_buffers ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, s));
+    }
+    if (m == 0) { CK(cudaStreamSynchronize(s)); return PN_OK; }
+    // 2. gather + FP64 reference integration of the subset (the library's own integrator)
+    if ((rc = g_ck_sub.ensure(sizeof(double) * 23 * (size_t)m + sizeof(int) * (size_t)m)) != PN_OK) return rc;
+    double* sub_init = (double*)g_ck_sub.p;
+    double* sub_fin = sub_init + 10 * m;
+    double* sub_m = sub_fin + 10 * m;
+    double* sub_t = sub_m + 2 * m;
+    int* sub_steps = (int*)(sub_t + m);
+    CK(pn_launch_check_gather(d_idx, m, d_init, d_m, sub_init, sub_m, s));
+    pn_options ro;
+    default_options(&ro);
+    ro.stream = o.stream;
+    ro.out_time = sub_t;
+    const int st = pn_integrate_ex(sub_init, sub_m, m, 0.0, omegaf, rtol_ref, atol_ref, PN_FP64, sub_fin, sub_steps, &ro);
+    if (st == PN_ECUDA) return st;
+    out->ms_reference = g_ms[1];
+    // 3. comparison
+    if ((rc = g_ck_out.ensure(64)) != PN_OK) return rc;
+    CK(pn_launch_check_compare(d_idx, m, d_fin, d_t, sub_fin, sub_t, sub_steps, (double*)g_ck_out.p, s));
+    double h[8];
+    CK(cudaMemcpyAsync(h, g_ck_out.p, sizeof h, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    long long hi[8];
+    memcpy(hi, h, sizeof hi);
+    for (int k = 0; k < 3; ++k) { out->max_dot_dev[k] = h[k]; out->worst_index[k] = hi[4 + k]; }
+    out->max_time_rel_dev = h[3];
+    out->n_failed_ref = hi[7];
+    return st;
+}
+
 extern "C" int pn_stream_status(void* stream)
 {
     cudaStream_t s = (cudaStream_t)stream;
@@ -451,7 +531,7 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts, &g_st_scratch, &g_st_in, &g_st_out, &g_gen_specs, &g_gen_y, &g_gen_m};
+    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts, &g_st_scratch, &g_st_in, &g_st_out, &g_gen_specs, &g_gen_y, &g_gen_m, &g_ck_idx, &g_ck_tmp, &g_ck_sub, &g_ck_out, &g_ck_in};
     for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
     if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
     g_stream_status.clear();

@@ -50,6 +50,15 @@ cudaError_t pn_launch_stats(const double* init, const double* fin, const int* st
 // chi1_lo, chi1_hi, chi2_lo, chi2_hi, s1_tilt_deg}
 cudaError_t pn_launch_generate(const void* specs_dev, int n_ens, long long n_total, long long first, long long count,
                                double* init_states, double* masses, cudaStream_t s);
+// cross-check (pn_check.cu)
+size_t pn_check_select_temp_bytes(long long n);
+cudaError_t pn_launch_check_select(long long n, double fraction, unsigned long long k0, unsigned long long k1,
+                                   long long* indices, long long* n_selected, void* temp, size_t temp_bytes, cudaStream_t s);
+cudaError_t pn_launch_check_gather(const long long* indices, long long m, const double* init, const double* masses,
+                                   double* sub_init, double* sub_masses, cudaStream_t s);
+cudaError_t pn_launch_check_compare(const long long* indices, long long m, const double* fin, const double* times,
+                                    const double* ref_fin, const double* ref_times, const int* ref_steps, double* out,
+                                    cudaStream_t s);
 cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
                             double* cycles_per_warp_inst);
 
