@@ -39,6 +39,7 @@ struct GenSpec {           // device copy of pn_ensemble
     double omega0, q_lo, q_hi, m1_fixed, chi1_lo, chi1_hi, chi2_lo, chi2_hi, s1_tilt_deg;
 };
 
+template <bool SHARE>
 __global__ void __launch_bounds__(GEN_TILE) pn_generate_kernel(const GenSpec* __restrict__ specs, long long n_total,
                                                                long long first, long long count, int tiles_per_ens,
                                                                double* __restrict__ init_states, double* __restrict__ masses)
@@ -50,11 +51,34 @@ __global__ void __launch_bounds__(GEN_TILE) pn_generate_kernel(const GenSpec* __
     const int cnt = (int)min((long long)GEN_TILE, count - j0);
     const GenSpec sp = specs[ens];
     const int t = threadIdx.x;
+    // SHARE (n_total and first multiples of 4): the four systems 4q .. 4q+3 read the four words of the SAME Philox
+    // block in every variate column, so thread r of a quad evaluates only the blocks of columns r and r + 4 and the
+    // quad exchanges words through shared memory: 7 blocks per quad instead of 28.
+    __shared__ unsigned long long words[SHARE ? GEN_TILE / 4 * 7 * 4 : 1];
+    if (SHARE) {
+        const unsigned long long N = (unsigned long long)n_total;
+        const unsigned long long blk0 = (unsigned long long)(first + j0 + t) >> 2;     // block of this quad in column 0
+        const int q = t >> 2, r = t & 3;
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk) {
+            const int k = r + 4 * kk;
+            if (k < 7) {
+                unsigned long long w[4];
+                gen_block(sp.key0, sp.key1, (unsigned long long)k * (N >> 2) + blk0, w);
+#pragma unroll
+                for (int x = 0; x < 4; ++x) words[(q * 7 + k) * 4 + x] = w[x];
+            }
+        }
+        __syncthreads();
+    }
     if (t < cnt) {
         const unsigned long long i = (unsigned long long)(first + j0 + t), N = (unsigned long long)n_total;
         double u[7];
 #pragma unroll
-        for (int k = 0; k < 7; ++k) u[k] = gen_uniform(sp.key0, sp.key1, (unsigned long long)k * N + i);
+        for (int k = 0; k < 7; ++k) {
+            if (SHARE) u[k] = (double)(words[((t >> 2) * 7 + k) * 4 + (t & 3)] >> 11) * (1.0 / 9007199254740992.0);
+            else u[k] = gen_uniform(sp.key0, sp.key1, (unsigned long long)k * N + i);
+        }
         const double q = gen_lerp(sp.q_lo, sp.q_hi, u[0]);
         const double chi1 = gen_lerp(sp.chi1_lo, sp.chi1_hi, u[1]);
         const double chi2 = gen_lerp(sp.chi2_lo, sp.chi2_hi, u[2]);
@@ -100,8 +124,12 @@ cudaError_t pn_launch_generate(const void* specs_dev, int n_ens, long long n_tot
     if (count <= 0 || n_ens <= 0) return cudaSuccess;
     const long long tiles = (count + GEN_TILE - 1) / GEN_TILE;
     if (tiles * n_ens > 0x7fffffffLL) return cudaErrorInvalidValue;
-    pn_generate_kernel<<<(unsigned)(tiles * n_ens), GEN_TILE, 0, s>>>((const GenSpec*)specs_dev, n_total, first, count,
-                                                                      (int)tiles, init_states, masses);
+    if ((n_total & 3) == 0 && (first & 3) == 0)
+        pn_generate_kernel<true><<<(unsigned)(tiles * n_ens), GEN_TILE, 0, s>>>((const GenSpec*)specs_dev, n_total, first, count,
+                                                                                (int)tiles, init_states, masses);
+    else
+        pn_generate_kernel<false><<<(unsigned)(tiles * n_ens), GEN_TILE, 0, s>>>((const GenSpec*)specs_dev, n_total, first, count,
+                                                                                 (int)tiles, init_states, masses);
     ++g_pn_launches;
     return cudaGetLastError();
 }

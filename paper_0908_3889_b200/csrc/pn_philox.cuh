@@ -10,6 +10,22 @@
 #define PHILOX_W0 0x9E3779B97F4A7C15ULL
 #define PHILOX_W1 0xBB67AE8584CAA73BULL
 
+// all four words of Philox4x64-10(counter = blk + 1, key): raw words 4 blk ... 4 blk + 3 of the stream
+__device__ __forceinline__ void gen_block(unsigned long long k0, unsigned long long k1, unsigned long long blk,
+                                          unsigned long long (&w)[4])
+{
+    unsigned long long c0 = blk + 1ull, c1 = 0ull, c2 = 0ull, c3 = 0ull;
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) { k0 += PHILOX_W0; k1 += PHILOX_W1; }
+        const unsigned long long hi0 = __umul64hi(PHILOX_M0, c0), lo0 = PHILOX_M0 * c0;
+        const unsigned long long hi1 = __umul64hi(PHILOX_M1, c2), lo1 = PHILOX_M1 * c2;
+        const unsigned long long n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    w[0] = c0; w[1] = c1; w[2] = c2; w[3] = c3;
+}
+
 // word (e & 3) of Philox4x64-10(counter = (e >> 2) + 1, key)
 __device__ __forceinline__ unsigned long long gen_raw(unsigned long long k0, unsigned long long k1, unsigned long long e)
 {
