@@ -215,26 +215,28 @@ __global__ void __launch_bounds__(ST_THREADS, 1) pn_stats_kernel(const StParams 
             st_mbar_wait(st_smem_addr(&bars[stage]), parity);
             // final-state rows first: their dot products are formed before the initial-state rows are read, so the
             // two 10-double rows are never live together (the kernel must fit 128 registers at 512 threads)
-            double ri[ST_ROW], df[3], di[3];
+            double df[3], di[3];
             bool okf[3] = {false, false, false}, oki[3] = {true, true, true};
             const bool have = row < cnt;
             if (have) {
                 // 16-byte shared loads: rows are 80 B apart, so a quarter-warp covers 8 distinct 16-byte bank groups
                 const double2* src = reinterpret_cast<const double2*>(tiles + (size_t)stage * NT * ST_TILE * ST_ROW + row * ST_ROW);
-                double rf[ST_ROW];
+                double rw[ST_ROW];
 #pragma unroll
-                for (int c = 0; c < ST_ROW / 2; ++c) { const double2 v = src[c]; rf[2 * c] = v.x; rf[2 * c + 1] = v.y; }
-                st_unit_dots(rf, df, okf);
-                if (HAVE_INIT)
+                for (int c = 0; c < ST_ROW / 2; ++c) { const double2 v = src[c]; rw[2 * c] = v.x; rw[2 * c + 1] = v.y; }
+                st_unit_dots(rw, df, okf);
+                if (HAVE_INIT) {
 #pragma unroll
-                    for (int c = 0; c < ST_ROW / 2; ++c) { const double2 v = src[ST_TILE * ST_ROW / 2 + c]; ri[2 * c] = v.x; ri[2 * c + 1] = v.y; }
+                    for (int c = 0; c < ST_ROW / 2; ++c) { const double2 v = src[ST_TILE * ST_ROW / 2 + c]; rw[2 * c] = v.x; rw[2 * c + 1] = v.y; }
+                    st_unit_dots(rw, di, oki);
+                }
             }
             const bool failed = have && p.steps && (p.steps[start + row] < 0);
-            asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(ST_TILE) : "memory");     // this group has read the stage
+            // only six doubles per thread are live across the barrier (the kernel must fit 128 registers at 512 threads)
+            asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(ST_TILE) : "memory");     // this group has read the slot
             if (row == 0 && w + ST_STAGES < w_end) issue(w + ST_STAGES, stage);
 
             if (have) {
-                if (HAVE_INIT) st_unit_dots(ri, di, oki);
 #pragma unroll
                 for (int kk = 0; kk < 3; ++kk) {
                     const bool ok = okf[kk] && oki[kk] && !failed;
