@@ -55,6 +55,20 @@ def test_options_struct_matches_header(tmp_path):
                    PnOptions.stream.offset, PnOptions.grid_blocks.offset]
 
 
+def test_new_structs_match_header(tmp_path):
+    from paper_0908_3889_b200.binding import PnCheckOut, PnEnsemble, PnStatsOut
+
+    src = tmp_path / "sz2.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "pn.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu",'
+                   "sizeof(pn_stats_out), offsetof(pn_stats_out,hist2_norm), sizeof(pn_ensemble), offsetof(pn_ensemble,s1_tilt_deg),"
+                   "sizeof(pn_check_out), offsetof(pn_check_out,worst_index), offsetof(pn_check_out,ms_reference));return 0;}\n")
+    exe = tmp_path / "sz2"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    got = [int(t) for t in subprocess.check_output([str(exe)]).split()]
+    assert got == [C.sizeof(PnStatsOut), PnStatsOut.hist2_norm.offset, C.sizeof(PnEnsemble), PnEnsemble.s1_tilt_deg.offset,
+                   C.sizeof(PnCheckOut), PnCheckOut.worst_index.offset, PnCheckOut.ms_reference.offset]
+
+
 def test_product_does_not_import_oracle():
     for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_0908_3889_b200")):
         for f in files:
