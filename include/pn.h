@@ -158,6 +158,16 @@ int pn_statistics(const double* init_states, const double* final_states, const i
                   const struct pn_options* opt);
 
 /*
+ * pn_merge_statistics -- the exchange step of pn_statistics over several GPUs: `parts` holds the
+ * `moments` outputs of n_parts pn_statistics calls over disjoint parts of the SAME G ensembles, [n_parts][G][3][6]
+ * (e.g. gathered from all ranks with one all-gather); they are merged in part order with the pairwise update used
+ * inside a launch.  moments_out [G][3][6] and pearson_r_out [G][3] (either may be NULL).  Histogram counters need no
+ * such call: they are summed by an integer all-reduce.  DEVICE pointers; opt: stream and async only.
+ */
+int pn_merge_statistics(const double* parts, int n_parts, int n_groups, double* moments_out, double* pearson_r_out,
+                        const struct pn_options* opt);
+
+/*
  * pn_generate -- random initial data on the device ("generated on the GPU"; recipe of
  * PAPER.md:68, 102-104 as fixed in DESIGN.md 5 and 12): for every system seven uniform variates
  * (q, chi1, chi2, z1, phi1, z2, phi2) from ONE counter-based Philox4x64-10 stream per ensemble, laid out

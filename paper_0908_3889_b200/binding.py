@@ -18,7 +18,7 @@ PN_FP64, PN_FP32, PN_MIXED = 0, 1, 2
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_generate", "pn_selfcheck", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_merge_statistics", "pn_generate", "pn_selfcheck", "pn_stream_status",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -80,6 +80,7 @@ def load():
         lib.pn_histogram.argtypes = [vp, ll, i, vp, vp]
         lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_statistics.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
+        lib.pn_merge_statistics.argtypes = [vp, i, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_generate.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, vp, vp, C.POINTER(PnOptions)]
         lib.pn_selfcheck.argtypes = [vp, vp, vp, vp, ll, d, d, C.POINTER(C.c_ulonglong), d, d, C.POINTER(PnCheckOut), vp, ll,
                                      C.POINTER(PnOptions)]
@@ -178,6 +179,14 @@ def pn_statistics(init_states, final_states, steps=None, *, group_size=0, bins1=
     out.hist1, out.hist2, out.hist2_max, out.hist2_norm = _ptr(hist1), _ptr(hist2), _ptr(hist2_max), _ptr(hist2_norm)
     return _check(lib.pn_statistics(_ptr(init_states), _ptr(final_states), _ptr(steps), n, int(group_size), int(bins1),
                                     int(bins2), C.byref(out), C.byref(o)))
+
+
+def pn_merge_statistics(parts, moments=None, pearson_r=None, **opts):
+    """pn_merge_statistics of include/pn.h: parts [R, G, 3, 6] (torch CUDA float64) -> moments [G, 3, 6], pearson_r [G, 3]."""
+    lib = load()
+    o = make_options(**opts)
+    return _check(lib.pn_merge_statistics(_ptr(parts), int(parts.shape[0]), int(parts.shape[1]), _ptr(moments), _ptr(pearson_r),
+                                          C.byref(o)))
 
 
 def pn_generate(ensembles, n_total, init_states, masses, *, first=0, count=None, **opts):

@@ -326,6 +326,24 @@ extern "C" int pn_statistics(const double* init_states, const double* final_stat
     return PN_OK;
 }
 
+extern "C" int pn_merge_statistics(const double* parts, int n_parts, int n_groups, double* moments_out, double* pearson_r_out,
+                                   const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (n_parts < 1 || n_groups < 0 || o.host_buffers || (n_groups > 0 && !parts)) return PN_EINVAL;
+    cudaStream_t s = (cudaStream_t)o.stream;
+    CK(pn_launch_stats_merge(parts, n_parts, n_groups, moments_out, pearson_r_out, s));
+    if (o.async) return PN_OK;
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    return PN_OK;
+}
+
 extern "C" int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,
                            double* init_states, double* masses, const pn_options* opt_in)
 {

@@ -42,6 +42,7 @@ cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int 
                                  cudaStream_t s);
 // ensemble statistics (pn_stats.cu)
 size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out);
+cudaError_t pn_launch_stats_merge(const double* parts, int n_parts, int n_groups, double* mom_out, double* r_out, cudaStream_t s);
 cudaError_t pn_launch_stats(const double* init, const double* fin, const int* steps, long long n, long long group_size,
                             int bins1, int bins2, void* scratch, double* r_out, double* mom_out,
                             unsigned long long* skipped_out, unsigned long long* hist1, unsigned long long* hist2,

@@ -347,6 +347,35 @@ __global__ void __launch_bounds__(256) pn_stats_norm_kernel(const unsigned long 
     }
 }
 
+// Multi-GPU exchange step of the statistics: the moment records of R parts of the same ensembles
+// (one part per rank, gathered with one all-gather of R x G x 3 x 6 doubles) are merged in part order with the same
+// pairwise update as inside a launch.  One thread per (group, dot product).
+__global__ void pn_stats_merge_kernel(const double* __restrict__ parts, int n_parts, int n_groups,
+                                      double* __restrict__ mom_out, double* __restrict__ r_out)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_groups * 3) return;
+    StMom m = {0, 0, 0, 0, 0, 0};
+    for (int part = 0; part < n_parts; ++part) {
+        const double* q = parts + ((size_t)part * n_groups * 3 + j) * 6;
+        StMom o = {q[0], q[0] > 0 ? q[1] : 0.0, q[0] > 0 ? q[2] : 0.0, q[3], q[4], q[5]};      // empty parts carry NaN means
+        st_merge(m, o);
+    }
+    if (mom_out) {
+        double* q = mom_out + (size_t)j * 6;
+        q[0] = m.n; q[1] = m.n > 0 ? m.mx : nan(""); q[2] = m.n > 0 ? m.my : nan(""); q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
+    }
+    if (r_out) r_out[j] = (m.n >= 2.0 && m.m2x > 0.0 && m.m2y > 0.0) ? m.cxy / sqrt(m.m2x * m.m2y) : nan("");
+}
+
+cudaError_t pn_launch_stats_merge(const double* parts, int n_parts, int n_groups, double* mom_out, double* r_out, cudaStream_t s)
+{
+    if (n_groups <= 0) return cudaSuccess;
+    pn_stats_merge_kernel<<<(n_groups * 3 + 127) / 128, 128, 0, s>>>(parts, n_parts, n_groups, mom_out, r_out);
+    ++g_pn_launches;
+    return cudaGetLastError();
+}
+
 size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out)
 {
     int dev = 0, sms = 148;

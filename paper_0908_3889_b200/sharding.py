@@ -33,3 +33,15 @@ def max_over_ranks(value: float, device, dist=None) -> float:
     if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def allgather_moments(moments, dist=None):
+    """Statistics over a sharded ensemble: gathers every rank's `moments` output of pn_statistics ([G, 3, 6]) into
+    [world, G, 3, 6] in rank order, the input of pn_merge_statistics (which does the arithmetic on the device)."""
+    import torch
+
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return moments.unsqueeze(0).contiguous()
+    parts = [torch.empty_like(moments) for _ in range(dist.get_world_size())]
+    dist.all_gather(parts, moments.contiguous())
+    return torch.stack(parts).contiguous()

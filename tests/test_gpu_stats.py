@@ -174,3 +174,38 @@ def test_statistics_C2_full_size_through_the_integrator(pn, oracle):
     r_o = S.statistics(y0[idx], o["final"])["r"]
     r_g = S.statistics(y0[idx], yf[idx])["r"]
     assert np.abs(r_o - r_g).max() < 1e-7
+
+
+def test_merge_statistics_of_sharded_ensembles(pn):
+    """The multi-GPU exchange step on one GPU: three ranks' shares (sharding.shard_range) of the same two ensembles,
+    statistics per share, moments merged by pn_merge_statistics == statistics of the whole (oracle, 1e-12)."""
+    from paper_0908_3889_b200 import sharding
+
+    G, gs, world = 2, 3001, 3
+    cfg = W.with_size(W.CONFIGS["C3"], G * gs)
+    y0, _ = W.generate(cfg)
+    yf = fake_final(y0, 77)
+    ref = S.statistics(y0, yf, None, gs, 0, 0)
+    parts = torch.zeros(world, G, 3, 6, dtype=torch.float64, device="cuda")
+    counts = np.zeros((G, 3, 20), dtype=np.int64)
+    for rank in range(world):
+        lo, hi = sharding.shard_range(gs, rank, world)
+        rows = np.concatenate([np.arange(g * gs + lo, g * gs + hi) for g in range(G)])      # this rank's slice of every ensemble
+        got = gpu_stats(pn, y0[rows], yf[rows], None, hi - lo, 20, 0)
+        parts[rank] = torch.from_numpy(got["moments"]).cuda()
+        counts += got["hist1"]
+    mom = torch.zeros(G, 3, 6, dtype=torch.float64, device="cuda")
+    r = torch.zeros(G, 3, dtype=torch.float64, device="cuda")
+    pn.pn_merge_statistics(parts, moments=mom, pearson_r=r)
+    mom, r = mom.cpu().numpy(), r.cpu().numpy()
+    assert np.array_equal(mom[..., 0], ref["moments"][..., 0])
+    assert np.abs(mom[..., 1:3] - ref["moments"][..., 1:3]).max() <= 1e-14
+    assert (np.abs(mom[..., 3:] - ref["moments"][..., 3:]) / gs).max() <= 1e-11
+    assert np.abs(r - ref["r"]).max() <= 1e-12
+    assert np.abs(counts - S.statistics(y0, yf, None, gs, 20, 0)["hist1"].astype(np.int64)).sum() <= 2 * near_edge_count(S.unit_dots(yf), 20)
+    # an empty part (a rank with no systems) is neutral
+    parts2 = torch.cat([parts, torch.zeros(1, G, 3, 6, dtype=torch.float64, device="cuda")])
+    parts2[-1, :, :, 1:3] = float("nan")
+    r2 = torch.zeros(G, 3, dtype=torch.float64, device="cuda")
+    pn.pn_merge_statistics(parts2, pearson_r=r2)
+    assert np.array_equal(r2.cpu().numpy(), r)

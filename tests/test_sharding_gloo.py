@@ -33,7 +33,9 @@ def _worker(rank, world, port, out):
         sharding.allreduce_counts(counts, dist)
         tmax = sharding.max_over_ranks(10.0 + rank, torch.device("cpu"), dist)
         lo, hi = sharding.shard_range(1001, rank, world)
-        out.put((rank, local, counts.numpy(), tmax, lo, hi, float(y0[:, 1].sum())))
+        mom = torch.full((2, 3, 6), float(rank + 1), dtype=torch.float64)
+        parts = sharding.allgather_moments(mom, dist)
+        out.put((rank, local, counts.numpy(), tmax, lo, hi, float(y0[:, 1].sum()), parts.numpy()))
     finally:
         dist.destroy_process_group()
 
@@ -50,7 +52,8 @@ def test_two_rank_sharding_and_count_allreduce():
         p.join(timeout=60)
         assert p.exitcode == 0
     total = res[0][1] + res[1][1]
-    for rank, local, reduced, tmax, lo, hi, chk in res:
+    for rank, local, reduced, tmax, lo, hi, chk, parts in res:
+        assert parts.shape == (2, 2, 3, 6) and np.all(parts[0] == 1.0) and np.all(parts[1] == 2.0)   # rank order
         assert np.array_equal(reduced, total)           # every rank holds the global histogram
         assert reduced.sum() == 3 * 2000 * world
         assert tmax == 11.0                             # max over ranks
@@ -72,3 +75,4 @@ def test_single_process_is_a_noop():
     c = torch.ones(3, 5, dtype=torch.int64)
     assert sharding.allreduce_counts(c, dist).sum().item() == 15
     assert sharding.max_over_ranks(3.5, torch.device("cpu"), dist) == 3.5
+    assert sharding.allgather_moments(torch.ones(4, 3, 6, dtype=torch.float64), dist).shape == (1, 4, 3, 6)
