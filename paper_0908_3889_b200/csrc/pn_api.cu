@@ -50,7 +50,7 @@ static unsigned g_redo_count = 0;   // systems that went through the redo pass i
 static std::map<void*, int> g_stream_status;
 
 // layout of g_small: [0..3] counters (u64), then queue (u32), status (i32)
-struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned int queue2; unsigned int redo_count; unsigned long long skipped[3]; };
+struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned int queue2; unsigned int redo_count; unsigned long long skipped[3]; int nonuniform; int pad; };
 
 static int ensure_events()
 {
@@ -159,7 +159,8 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     }
     p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
     p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = (int*)g_redo.p;
-    CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s));
+    p.nonuniform = &small->nonuniform;
+    CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s, !o.async));
     CK(cudaEventRecord(g_ev[2], s));
     if (o.layout == 0) CK(pn_launch_soa_to_aos((const double*)g_soa_out.p, d_final, n, 10, s));
     CK(cudaEventRecord(g_ev[3], s));

@@ -132,6 +132,7 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
         rec[38] = (real)-1;
         return;
     }
+    if (m1 != p.masses[0] || m2 != p.masses[p.n]) *p.nonuniform = 1;      // benign race: every writer stores 1
     PnConsts<real> c;
     PnBase<real> base;
     PnUni<real> u;
@@ -180,7 +181,9 @@ __device__ __forceinline__ void pn_load_record(const void* seed, int i, real (&o
 // state itself is carried in double: an accepted step adds the float increment dy = sum b_s K_s to the double copy,
 // so the per-step rounding error is eps32 |dy| instead of eps32 |y| ("only a few critical computations in
 // double"); omega is compared with omega_f in double.
-template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false>
+// UNI = true (FP64): every system of the batch has the masses of system 0 (checked by the seed kernel), so the 15
+// mass-dependent constants are kernel parameters: constant-bank operands instead of per-lane registers.
+template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false, bool UNI = false>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
 {
     const unsigned n_queue = SLOW ? *p.redo_count : (unsigned)p.n;     // length of the work queue
@@ -201,6 +204,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
     pn_make_consts<real>(0.5, 0.5, 0u, c);
+    if constexpr (UNI) {
+        c.M = (real)p.uc[0]; c.c2 = (real)p.uc[1]; c.c4 = (real)p.uc[2]; c.c5 = (real)p.uc[3]; c.c6 = (real)p.uc[4]; c.c7 = (real)p.uc[5];
+        c.p1 = (real)p.uc[6]; c.p2 = (real)p.uc[7]; c.q1 = (real)p.uc[8]; c.q2 = (real)p.uc[9]; c.K0 = (real)p.uc[10];
+        c.A1 = (real)p.uc[11]; c.A2 = (real)p.uc[12]; c.Bc = (real)p.uc[13]; c.G = (real)p.uc[14];
+    }
 #pragma unroll
     for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; yd[i] = 0.0; }
     y[0] = (real)0.01; y[9] = (real)1; yd[0] = 0.01; yd[9] = 1.0;
@@ -242,9 +250,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                         if constexpr (MIXED)
 #pragma unroll
                             for (int j = 0; j < 10; ++j) yd[j] = __ldg(p.y0 + (size_t)j * p.n + i);
-                        c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
-                        c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
-                        c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
+                        if constexpr (!UNI) {
+                            c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
+                            c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
+                            c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
+                        }
                         base.r0 = rec[35]; base.r03 = rec[36]; base.l0 = rec[37];
                         atS1 = (float)rec[38]; atS2 = (float)rec[39];
                         t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
@@ -426,10 +436,10 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
 
 unsigned long long g_pn_launches = 0;
 
-template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false>
+template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false, bool UNI = false>
 static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
-    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM, SLOW, MIXED>;
+    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM, SLOW, MIXED, UNI>;
     const int shm = SMEM ? PN_SM_SLOTS * BLOCK * (int)sizeof(double) : 0;
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t e;
@@ -451,8 +461,8 @@ static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cud
     return cudaGetLastError();
 }
 
-cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int block_threads, int grid_blocks,
-                                cudaStream_t s)
+cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
+                                cudaStream_t s, bool may_sync)
 {
     if (p.n <= 0) return cudaSuccess;
     if (p.fixed_steps > 0) {
@@ -482,7 +492,23 @@ cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int bloc
         const char* v = getenv("PN_DEV_VARIANT");   // development switch, not part of the ABI
         if (block_threads == 256) e = launch_adaptive<double, 256, 1, false, false>(p, grid_blocks, s);
         else if (v && v[0] == 's') e = launch_adaptive<double, 128, 3, true, false>(p, grid_blocks, s);
-        else e = launch_adaptive<double, 128, 2, false, false>(p, grid_blocks, s);
+        else {
+            // uniform-mass fast path: needs the seed kernel's verdict on the host (one small copy + sync, ~10 us)
+            bool uni = false;
+            if (may_sync && !getenv("PN_NO_UNIFORM")) {
+                int flag = 1;
+                double rec0[PN_REC];          // the constants come from system 0's seed record: bitwise what the generic path uses
+                if ((e = cudaMemcpyAsync(&flag, p.nonuniform, sizeof flag, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return e;
+                if ((e = cudaMemcpyAsync(rec0, p.seed, sizeof rec0, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return e;
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return e;
+                if (flag == 0 && rec0[38] >= 0.0) {
+                    for (int k = 0; k < 15; ++k) p.uc[k] = rec0[20 + k];
+                    uni = true;
+                }
+            }
+            if (uni) e = launch_adaptive<double, 128, 2, false, false, false, true>(p, grid_blocks, s);
+            else e = launch_adaptive<double, 128, 2, false, false>(p, grid_blocks, s);
+        }
         if (e != cudaSuccess) return e;
         // redo pass for systems that left the series' range; its queue length is read on the device
         return launch_adaptive<double, 128, 2, false, true>(p, grid_blocks, s);

@@ -25,11 +25,13 @@ struct PnKernelParams {
     unsigned int* redo_count;
     unsigned long long* counters;   // [0] trial steps [1] rejected [2] landing trials [3] failed systems
     int* status;                    // worst pn_status seen on the device (atomicMax)
+    int* nonuniform;                // set by the seed kernel if some system's masses differ from system 0's
+    double uc[15];                  // FP64 uniform-mass path: the PnConsts of (masses[0]) as kernel parameters (constant bank)
 };
 
 // launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults
-cudaError_t pn_launch_integrate(const PnKernelParams& p, int precision, int block_threads, int grid_blocks,
-                                cudaStream_t s);
+cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
+                                cudaStream_t s, bool may_sync);
 // staging + histogram + peak (pn_aux.cu)
 cudaError_t pn_launch_aos_to_soa(const double* aos, double* soa, int n, int width, cudaStream_t s);
 cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int width, cudaStream_t s);

@@ -174,3 +174,28 @@ def test_loose_tolerance_uses_the_redo_pass(pn, oracle):
     assert pn.pn_last_counters()["redo"] > 0
     from test_gpu_parity import comp_scale
     assert (np.abs(g["final"] - r["final"]) / comp_scale(y0[:64])).max() <= 1e-11
+
+
+def test_uniform_mass_fast_path_is_bit_identical(pn):
+    """FP64 batches whose systems all have the masses of system 0 run a kernel that takes the 15 mass-dependent
+    constants as kernel parameters.  Same constants, same arithmetic: the results are bit-identical to
+    the generic kernel's; one deviating system anywhere in the batch switches the whole launch to the generic kernel."""
+    import os
+
+    cfg = W.with_size(W.CONFIGS["C4"], 3000 + 17)
+    y0, m = W.generate(cfg)
+    a = gpu_integrate(pn, y0, m, cfg)
+    os.environ["PN_NO_UNIFORM"] = "1"
+    try:
+        b = gpu_integrate(pn, y0, m, cfg)
+    finally:
+        del os.environ["PN_NO_UNIFORM"]
+    for k in ("final", "steps", "time", "rejected"):
+        assert np.array_equal(a[k], b[k]), k
+    # a batch that is uniform except for its last system, and one whose system 0 is invalid
+    m2 = m.copy(); m2[-1] = [0.5, 0.5]
+    c = gpu_integrate(pn, y0, m2, cfg)
+    assert np.array_equal(c["final"][:-1], a["final"][:-1]) and not np.array_equal(c["final"][-1], a["final"][-1])
+    m3 = m.copy(); m3[0, 0] = -1.0
+    d = gpu_integrate(pn, y0, m3, cfg, allow_failures=True)
+    assert d["steps"][0] == -5 and np.array_equal(d["final"][1:], a["final"][1:])
