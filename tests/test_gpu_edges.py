@@ -199,3 +199,39 @@ def test_uniform_mass_fast_path_is_bit_identical(pn):
     m3 = m.copy(); m3[0, 0] = -1.0
     d = gpu_integrate(pn, y0, m3, cfg, allow_failures=True)
     assert d["steps"][0] == -5 and np.array_equal(d["final"][1:], a["final"][1:])
+
+
+def test_large_batch_2_26_systems(pn):
+    """Maximum sizes: 2^26 + 3 systems (67 M; ~36 GB of device memory with the library's scratch) generated on the
+    device, integrated in FP32 over a short frequency range, reduced on the device.  Checked by properties that hold at
+    any size and by re-integrating sampled rows in small batches (results do not depend on the batch they are in)."""
+    n = (1 << 26) + 3
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~40 GB of free device memory")
+    ens = pn.make_ensemble((26, 3), 0.04, q=(0.5, 1.0), chi1=(0.2, 1.0), chi2=(0.2, 1.0))
+    y0 = torch.empty(n, 10, dtype=torch.float64, device="cuda")
+    m = torch.empty(n, 2, dtype=torch.float64, device="cuda")
+    pn.pn_generate(ens, n, y0, m)
+    yf = torch.empty_like(y0)
+    st = torch.empty(n, dtype=torch.int32, device="cuda")
+    assert pn.pn_integrate(y0, m, 0.04, 0.05, 1e-5, 1e-7, pn.PN_FP32, yf, st) == 0
+    assert int(st.min().item()) > 0 and pn.pn_last_counters()["failed"] == 0
+    mom = torch.zeros(1, 3, 6, dtype=torch.float64, device="cuda")
+    h1 = torch.zeros(1, 3, 50, dtype=torch.int64, device="cuda")
+    sk = torch.zeros(1, 3, dtype=torch.int64, device="cuda")
+    pn.pn_statistics(y0, yf, st, bins1=50, moments=mom, hist1=h1, n_skipped=sk)
+    mom, h1 = mom.cpu().numpy()[0], h1.cpu().numpy()[0]
+    assert np.all(mom[:, 0] == n) and np.all(h1.sum(axis=1) == n) and int(sk.sum().item()) == 0
+    # isotropic initial spins: <x> = 0, M2x / n = 1/3 (PAPER.md:104), to 5 sigma of 6.7e7 samples
+    assert np.abs(mom[:, 1]).max() < 5 * np.sqrt(1 / 3 / n) and np.abs(mom[:, 3] / n - 1 / 3).max() < 5 * np.sqrt(4 / 45 / n)
+    assert abs(float(yf[:, 0].max().item()) / 0.05 - 1) < 4e-7 and abs(float(yf[:, 0].min().item()) / 0.05 - 1) < 4e-7
+    # the first, the last and a middle slice re-integrated alone give the same bits
+    for lo in (0, n // 2 + 12345, n - 1000):
+        a = torch.empty(1000, 10, dtype=torch.float64, device="cuda")
+        s2 = torch.empty(1000, dtype=torch.int32, device="cuda")
+        pn.pn_integrate(y0[lo:lo + 1000].contiguous(), m[lo:lo + 1000].contiguous(), 0.04, 0.05, 1e-5, 1e-7, pn.PN_FP32, a, s2)
+        assert torch.equal(a, yf[lo:lo + 1000]) and torch.equal(s2, st[lo:lo + 1000])
+    del y0, m, yf, st
+    pn.pn_shutdown()                      # give the scratch back for the tests that follow
+    torch.cuda.empty_cache()
