@@ -176,8 +176,16 @@ __device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, dou
 template <bool SLOW>
 __device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float& v, float& lnx, float& r, bool&)
 {
-    v = cbrtf(x);
-    lnx = __logf(x);
+    // x > 0 always (omega > 0, M > 0): one lg2 serves both functions, no special-case code (cbrtf carries branches
+    // for 0, inf and denormals).  ln x = lg2(x) ln 2; x^{-1/3} = ex2(-lg2(x)/3) polished by one Newton step
+    // r <- r + r (1 - x r^3)/3 (seed error ~2e-7 -> ~1e-13, below float rounding); v = x r^2.
+    float l2, r0;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(x));
+    lnx = l2 * 0.693147180559945f;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(l2 * (-1.0f / 3.0f)));
+    const float e = fmaf(-x * r0, r0 * r0, 1.0f);
+    r0 = fmaf(r0 * e, 1.0f / 3.0f, r0);
+    v = x * (r0 * r0);
     r = 0.0f;
 }
 
