@@ -95,7 +95,7 @@ __device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float 
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         const float at = (i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1);
-        const float scl = fmaxf(fmaf(rtol, fmaxf(fabsf(y[i]), fabsf(ynew[i])), at), 1e-30f);
+        const float scl = fmaf(rtol, fmaxf(fabsf(y[i]), fabsf(ynew[i])), at);      // at >= 1e-30 (clamped at refill): never 0
         const float q = err[i] * pn_rcp_f(scl);
         sum = fmaf(q, q, sum);
     }
@@ -214,7 +214,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     y[0] = (real)0.01; y[9] = (real)1; yd[0] = 0.01; yd[9] = 1.0;
     pn_base_init(c.M * y[0], base);
     real h = (real)0;
-    float atS1 = (float)p.atol, atS2 = (float)p.atol;
+    float atS1 = fmaxf((float)p.atol, 1e-30f), atS2 = atS1;
     double t = 0.0;
     int idx = -1, steps = 0, nrej = 0, nland = 0;
     bool after_reject = false, landing = false;
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     const real omegaf = (real)p.omegaf;
     const real om_hi = (real)(p.omegaf * (1.0 + p.tau));
     const real om_tol = (real)(p.tau * p.omegaf);
-    const float rtol = (float)p.rtol, atol1 = (float)p.atol;
+    const float rtol = (float)p.rtol, atol1 = fmaxf((float)p.atol, 1e-30f);
 
     for (;;) {
         // ---------------- refill: lanes without a system pull the next queue entries ----------------
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                             c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
                         }
                         base.r0 = rec[35]; base.r03 = rec[36]; base.l0 = rec[37];
-                        atS1 = (float)rec[38]; atS2 = (float)rec[39];
+                        atS1 = fmaxf((float)rec[38], 1e-30f); atS2 = fmaxf((float)rec[39], 1e-30f);   // keeps every scale > 0 (atol = 0 is allowed)
                         t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
                         idx = i;
                         h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;

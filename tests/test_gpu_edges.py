@@ -235,3 +235,17 @@ def test_large_batch_2_26_systems(pn):
     del y0, m, yf, st
     pn.pn_shutdown()                      # give the scratch back for the tests that follow
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("prec", [0, 1, 2])
+def test_atol_zero_is_allowed(pn, oracle, prec):
+    """atol = 0 with components that start at exactly 0 (L^_x = L^_y = 0): the error scale of such a component must not
+    become 0 (0/0 in the norm); the run completes and agrees with the oracle at the same pure-relative tolerance."""
+    cfg = W.with_size(W.CONFIGS["C1"], 257)
+    y0, m = W.generate(cfg)
+    rtol = [1e-9, 1e-5, 1e-7][prec]
+    g = gpu_integrate(pn, y0, m, cfg, rtol=rtol, atol=0.0, precision=prec)
+    assert g["status"] == 0 and np.all(g["steps"] > 0)
+    r = oracle.integrate(y0, m, cfg.omegaf, 1e-10, 1e-12)
+    dg, dr = dots_of(oracle, g["final"]), dots_of(oracle, r["final"])
+    assert np.abs(dg - dr).max() <= [1e-6, 2e-3, 2e-4][prec]
