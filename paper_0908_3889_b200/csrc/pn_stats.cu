@@ -424,7 +424,10 @@ cudaError_t pn_launch_stats(const double* init, const double* fin, const int* st
     p.hist2_smem = (p.bins2 > 0 && fixed + h2 <= cap) ? 1 : 0;
     const size_t shm = fixed + (p.hist2_smem ? h2 : 0);
     // opt in to large dynamic shared memory once per process (a host-side call per launch leaves the GPU idle)
-    static bool attr_done = false;
+    static bool attr_done_dev[64] = {false};          // the attribute is per device
+    int dev_id = 0;
+    if ((e = cudaGetDevice(&dev_id)) != cudaSuccess) return e;
+    bool& attr_done = attr_done_dev[dev_id & 63];
     if (!attr_done) {
         if ((e = cudaFuncSetAttribute(pn_stats_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cap)) != cudaSuccess) return e;
         if ((e = cudaFuncSetAttribute(pn_stats_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cap)) != cudaSuccess) return e;
