@@ -1,6 +1,7 @@
 // pn_api.cu -- the C ABI of libpn_b200 (include/pn.h): argument checks, scratch management, staging,
 // launches, status collection.  Every CUDA call is checked.
 #include <cstdint>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -149,6 +150,12 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     p.n = n;
     p.omega0 = omega0; p.omegaf = omegaf; p.rtol = rtol; p.atol = atol; p.h0 = o.h0;
     p.tau = o.tau_land > 0.0 ? o.tau_land : (precision == PN_FP64 ? 1e-13 : (precision == PN_MIXED ? 1e-8 : 3e-7));
+    // range of the series for (M omega)^{1/3} and ln(M omega) in the FP64 fast kernel (pn_rhs.cuh): |1 - x/x0| <= emax.
+    // 0.03 up to rtol 1e-10 and in fixed-step mode (truncation s10 emax^9 = 6e-17 relative); at looser tolerances the
+    // largest range whose truncation stays below 1e-3 rtol, at most 0.2: a run at rtol 1e-7 need not evaluate f to 1e-16.
+    // A system with an ACCEPTED step beyond the range goes to the wide-range redo pass.
+    p.emax = 0.03;
+    if (!fixed && rtol > 1e-10) { p.emax = pow(1e-3 * rtol / 0.0852, 1.0 / 9.0); if (p.emax > 0.2) p.emax = 0.2; }
     p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
     p.fixed_steps = fixed ? o.fixed_steps : 0;
     p.mask = o.term_mask;

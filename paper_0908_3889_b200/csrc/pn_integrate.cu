@@ -137,6 +137,7 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     PnBase<real> base;
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
+    u.emax = (real)p.emax;
     pn_make_consts<real>(m1, m2, p.mask, c);
     pn_base_init(c.M * y[0], base);
     const real h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;      // first step (R13); same expression at refill
@@ -203,6 +204,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     PnBase<real> base;
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
+    u.emax = (real)p.emax;
     pn_make_consts<real>(0.5, 0.5, 0u, c);
     if constexpr (UNI) {
         c.M = (real)p.uc[0]; c.c2 = (real)p.uc[1]; c.c4 = (real)p.uc[2]; c.c5 = (real)p.uc[3]; c.c6 = (real)p.uc[4]; c.c7 = (real)p.uc[5];
@@ -276,21 +278,27 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         if constexpr (SMEM) pn_dp5_trial_smem<SLOW, BLOCK>(y, k1, h, c, u, base, sm, ynew, k7, err, base_new, bad);
         else if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad, dy);
         else pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
-        // fast kernel: a lane whose step left the series' range (|1 - x/x0| > 0.03, only at very loose
-        // tolerances) hands its system to the redo pass and frees itself; redo kernel: `bad` means omega more
-        // than doubled inside one step, which is treated as a rejected step.
-        const bool force_reject = SLOW && bad;
-        if (!SLOW && idx >= 0 && bad) {
-            p.redo_list[atomicAdd(p.redo_count, 1u)] = idx;
-            idx = -1;
-        }
-
         // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|), E^2 = mean (err_j/sc_j)^2.
         // It only decides accept/reject and the next step size, so ~1e-6 relative accuracy is ample:
         // FP64: the larger magnitude is picked by comparing the high words (integer pipe), 1/sc_j is the raw
         // MUFU seed (rcp.approx.ftz.f64, ~2^-23, no Newton step): 3 FP64 instructions per component and no
         // F64<->F32 conversions (which issue at 1/8 rate and put a long serial tail at the end of the step).
-        const float E2 = force_reject ? 1e30f : pn_err_norm2(y, ynew, err, rtol, atol1, atS1, atS2);
+        float E2 = pn_err_norm2(y, ynew, err, rtol, atol1, atS1, atS2);
+        // `bad`: a stage of this trial left the range of the cbrt/log series (|1 - x/x0| > emax; only at loose
+        // tolerances).  Fast kernel: if the trial fails error control anyway (the usual case: an overshoot while the
+        // step size ramps up) it is an ordinary rejection (the estimate is inaccurate there, but it only sets the step-size
+        // factor; a non-finite one gives the smallest factor); if it would be ACCEPTED, its slopes
+        // cannot be trusted and the system is handed to the redo pass, which evaluates both functions over a wide
+        // range.  Redo kernel: `bad` means omega more than doubled inside one step: rejected.
+        if (!SLOW) {
+            if (idx >= 0 && bad && E2 <= 1.0f) {
+                p.redo_list[atomicAdd(p.redo_count, 1u)] = idx;
+                idx = -1;
+            }
+            E2 = (bad && !(E2 <= FLT_MAX)) ? 1e30f : E2;      // keep a finite estimate: it sets the factor of the rejection
+        } else {
+            E2 = bad ? 1e30f : E2;
+        }
 
         // ---------------- per-lane decision as straight-line selects ----------------
         // controller factor 0.9 (E^2)^{-1/10} on the FP32 special-function unit (R8)
@@ -327,7 +335,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         // priority by overwrite order, all selects, one branch
         const real h_floor = pn_max(PnLimits<real>::tiny(), (real)(2.3e-16 * t));   // independent of the controller chain
         int code = 0;
-        code = !(pn_abs(h_next) > h_floor) ? PN_F_HUNDERFLOW : code;
+        // step-size underflow as the oracle defines it (t + h == t, or h not above 1e-300): h_floor = one ulp of t is a
+        // cheap screen that never misses; the exact test runs only when the screen fires (a landing correction of a long
+        // inspiral is a few 1e-11 of time at t ~ 2e5, the size of that ulp)
+        bool underflow = !(pn_abs(h_next) > h_floor);
+        if (underflow) underflow = !(pn_abs(h_next) > PnLimits<real>::tiny()) || (t + (double)h_next == t);
+        code = underflow ? PN_F_HUNDERFLOW : code;
         code = (steps >= p.max_steps) ? PN_F_MAXSTEPS : code;
         code = (nland > 50) ? PN_F_LANDING : code;
         code = landed ? steps : code;
@@ -409,6 +422,7 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
     PnBase<real> base, base_new;
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
+    u.emax = (real)p.emax;
     pn_base_init(c.M * y[0], base);
     const real h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
     real r_tmp, l_tmp;

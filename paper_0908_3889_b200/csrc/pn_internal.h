@@ -16,6 +16,7 @@ struct PnKernelParams {
     int n;
     double omega0;       // > 0: every initial omega must match it to 1e-12 relative
     double omegaf, rtol, atol, h0, tau;
+    double emax;         // FP64 fast kernel: range of the cbrt/log series, |1 - x/x0| <= emax (pn_rhs.cuh)
     int max_steps;
     int fixed_steps;
     unsigned mask;
