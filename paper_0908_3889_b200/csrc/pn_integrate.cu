@@ -333,13 +333,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         const real h_next = h * ratio;
         // rare exits: finished, non-finite, landing failure, max_steps, step-size underflow (t + h == t);
         // priority by overwrite order, all selects, one branch
-        const real h_floor = pn_max(PnLimits<real>::tiny(), (real)(2.3e-16 * t));   // independent of the controller chain
+        // step-size underflow exactly as the oracle defines it: t + h == t, or h not above 1e-300 (a landing correction of
+        // a long inspiral can be one ulp of t ~ 2e5; a coarser test mistakes that for stagnation)
+        const bool underflow = !(pn_abs(h_next) > PnLimits<real>::tiny()) || (t + (double)h_next == t);
         int code = 0;
-        // step-size underflow as the oracle defines it (t + h == t, or h not above 1e-300): h_floor = one ulp of t is a
-        // cheap screen that never misses; the exact test runs only when the screen fires (a landing correction of a long
-        // inspiral is a few 1e-11 of time at t ~ 2e5, the size of that ulp)
-        bool underflow = !(pn_abs(h_next) > h_floor);
-        if (underflow) underflow = !(pn_abs(h_next) > PnLimits<real>::tiny()) || (t + (double)h_next == t);
         code = underflow ? PN_F_HUNDERFLOW : code;
         code = (steps >= p.max_steps) ? PN_F_MAXSTEPS : code;
         code = (nland > 50) ? PN_F_LANDING : code;
