@@ -268,8 +268,8 @@ def run_ours(args, cfg):
         "roofline": {"bound": "alu", "kernel": "pn_integrate_adaptive_kernel", "achieved": achieved, "peak": peak_nominal,
                      "unit": "TFLOP/s", "frac": achieved / peak_nominal,
                      # dram__bytes_read + dram__bytes_write of this kernel per launch, from the ncu --set full capture of
-                     # the same workload and size (profiles/r1_v9_ncu_integrator.md); algorithmic bytes: 445 MB
-                     "traffic": 435.0e6 if (cfg.name == "C2" and n == (1 << 20)) else None, "traffic_unit": "bytes/launch",
+                     # the same workload and size (profiles/r1_v10_ncu_integrator.md); algorithmic bytes: 445 MB
+                     "traffic": 431.4e6 if (cfg.name == "C2" and n == (1 << 20)) else None, "traffic_unit": "bytes/launch",
                      "peak_source": f"nominal {sms} SMs x {lanes} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md 6.3)",
                      "peak_measured_fma": peak_meas, "peak_measured_sm_mhz": peak_mhz,
                      "frac_of_measured_fma": achieved / peak_meas if peak_meas > 0 else None,
