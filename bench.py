@@ -57,7 +57,7 @@ class ClockSampler(threading.Thread):
                 self.samples.append([t.strip() for t in out.split(",")])
             except Exception:
                 pass
-            self._stop_evt.wait(0.2)
+            self._stop_evt.wait(0.02)
 
     def stop(self):
         self._stop_evt.set()
