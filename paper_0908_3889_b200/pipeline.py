@@ -1,0 +1,45 @@
+"""Seed in, statistics out: pn_generate -> pn_integrate -> pn_statistics (-> pn_selfcheck) on device buffers.
+
+Orchestration only: every step is one call of the C ABI (include/pn.h) through binding.py; nothing is computed here.
+One ensemble or a sweep of ensembles, n systems each, all on the current CUDA device.
+"""
+from __future__ import annotations
+
+from . import binding as B
+
+
+def run_ensembles(ensembles, n, omegaf, *, rtol=1e-10, atol=1e-12, precision=B.PN_FP64, bins1=50, bins2=79,
+                  check_fraction=0.0, check_key=(0, 0), keep_states=False):
+    """ensembles: list of dicts for binding.make_ensemble (key, omega0, q, chi1, chi2, m1_fixed, s1_tilt_deg).
+
+    Returns a dict of numpy arrays: pearson_r[G,3], moments[G,3,6], n_skipped[G,3], hist1[G,3,bins1],
+    hist2[G,3,bins2,bins2], hist2_max[G,3], steps_mean[G], status, and, if check_fraction > 0, `check`
+    (pn_selfcheck's report: the paper's random double-precision cross-check)."""
+    import torch
+
+    ens = ensembles if isinstance(ensembles, (list, tuple)) else [ensembles]
+    G, N = len(ens), len(ens) * int(n)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    f64 = dict(dtype=torch.float64, device=dev)
+    i64 = dict(dtype=torch.int64, device=dev)
+    y0, m = torch.empty(N, 10, **f64), torch.empty(N, 2, **f64)
+    B.pn_generate([B.make_ensemble(**e) for e in ens], int(n), y0, m)
+    yf = torch.empty_like(y0)
+    steps = torch.empty(N, dtype=torch.int32, device=dev)
+    times = torch.empty(N, **f64)
+    status = B.pn_integrate(y0, m, 0.0, omegaf, rtol, atol, precision, yf, steps, out_time=times, allow_failures=True)
+    out = dict(pearson_r=torch.zeros(G, 3, **f64), moments=torch.zeros(G, 3, 6, **f64), n_skipped=torch.zeros(G, 3, **i64))
+    if bins1 > 0:
+        out["hist1"] = torch.zeros(G, 3, bins1, **i64)
+    if bins2 > 0:
+        out["hist2"] = torch.zeros(G, 3, bins2, bins2, **i64)
+        out["hist2_max"] = torch.zeros(G, 3, **i64)
+    B.pn_statistics(y0, yf, steps, group_size=int(n), bins1=bins1, bins2=bins2, **out)
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    res["status"] = status
+    res["steps_mean"] = steps.view(G, int(n)).clamp(min=0).double().mean(dim=1).cpu().numpy()
+    if check_fraction > 0:
+        res["check"] = B.pn_selfcheck(y0, m, yf, omegaf, fraction=check_fraction, key=check_key, times=times, allow_failures=True)
+    if keep_states:
+        res.update(init_states=y0, masses=m, final_states=yf, steps=steps, times=times)
+    return res

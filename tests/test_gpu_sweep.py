@@ -61,3 +61,22 @@ def test_sweep_one_launch_against_oracle_chain(oracle):
     assert np.all(r[4:, 0] > 0.98)
     assert np.abs(r[4:, 1] - r[4:, 2]).max() < 0.03
     assert np.ptp(np.concatenate([r[4:, 1], r[:1, 1]])) > 0.05
+
+
+def test_run_ensembles_pipeline(oracle):
+    """The orchestration helper gives what the separate calls give, and its cross-check agrees with the FP32 bar."""
+    import paper_0908_3889_b200 as pn
+
+    sp = specs()[:2]
+    res = pn.run_ensembles(sp, 4000, OMEGAF, rtol=1e-5, atol=1e-7, precision=pn.PN_FP32, bins1=20, bins2=16,
+                           check_fraction=0.05, check_key=(5, 6))
+    assert res["status"] == 0 and res["pearson_r"].shape == (2, 3) and res["hist2"].shape == (2, 3, 16, 16)
+    assert np.all(res["moments"][..., 0] == 4000) and np.all(res["hist1"].sum(axis=2) == 4000)
+    assert 0.97 < res["pearson_r"][0, 0] < 1.0 and res["pearson_r"][1, 0] < res["pearson_r"][0, 0]
+    chk = res["check"]
+    assert 300 < chk["n_checked"] < 500 and chk["n_failed_ref"] == 0 and 0 < max(chk["max_dot_dev"]) < 1e-2
+    # the same ensembles through the oracle chain: r to the FP32 accuracy
+    for e, s in enumerate(sp):
+        y0, m = G.generate(G.make_spec(**s), 4000)
+        o = oracle.integrate(y0, m, OMEGAF, 1e-10, 1e-12)
+        assert np.abs(S.statistics(y0, o["final"])["r"][0] - res["pearson_r"][e]).max() < 5e-4
