@@ -5,11 +5,15 @@ One "step" = one pass of the whole hot path over one batch of synthetic inspiral
 (default: C2 of BASELINE.json, 2^20 equal-mass maximally spinning inspirals, FP64, omega 0.005->0.05,
 rtol 1e-10): stage-in, persistent DP5(4) integrator, stage-out, histogram kernel.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference] [--scaling weak|strong]
 
-Prints ONE JSON line (see DESIGN.md 6 for every field).  Multi-GPU: the batch dimension is sharded
-(every rank integrates its own seeded batch of the same size: weak scaling); the only exchange is the
-all-reduce of the 3 x bins histogram counters.
+Prints ONE JSON line (see DESIGN.md 6 for every field).  Multi-GPU: one process per GPU.  Started
+under torchrun (RANK / LOCAL_RANK / WORLD_SIZE / MASTER_* in the environment) it uses those ranks; started as
+plain `python bench.py --gpus N` with N > 1 it re-executes itself under `python -m torch.distributed.run
+--nproc-per-node N` on 127.0.0.1.  The batch dimension is sharded: weak scaling (default) gives every rank its own
+seeded batch of the full workload size, strong scaling splits ONE batch into contiguous slices
+(sharding.shard_range); the only exchange is the all-reduce of the 3 x bins histogram counters.
+`--dry` runs the launch, sharding and exchange logic on the CPU (gloo, no CUDA, no kernels): for the CPU tests.
 """
 from __future__ import annotations
 
@@ -75,12 +79,27 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_throughput(cfg, target_seconds=15.0, n_threads=0):
-    """Times the CPU oracle, as it stands, on a bounded seeded sample of the workload."""
+def cpu_model():
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_throughput(cfg, target_seconds=15.0, n_threads=0, single_thread=False):
+    """Times the CPU oracle, as it stands, on a bounded seeded sample of the workload: a random-permutation prefix of
+    the batch (so the q / chi mix is the workload's), sized from a 256-system probe for about target_seconds."""
     from oracle import pn_oracle
 
     pn_oracle.build()
+    # torchrun exports OMP_NUM_THREADS=1 to its ranks: ask for the host's cores explicitly
+    n_threads = n_threads if n_threads > 0 else (os.cpu_count() or 1)
     y0, m = W.generate(W.with_size(cfg, min(cfg.n, 1 << 19)))
+    perm = np.random.Generator(np.random.Philox(20090826)).permutation(y0.shape[0])
+    y0, m = np.ascontiguousarray(y0[perm]), np.ascontiguousarray(m[perm])
     probe = min(256, y0.shape[0])
     t0 = time.perf_counter()
     pn_oracle.integrate(y0[:probe], m[:probe], cfg.omegaf, 1e-10, 1e-12, n_threads=n_threads)
@@ -90,12 +109,17 @@ def oracle_throughput(cfg, target_seconds=15.0, n_threads=0):
     r = pn_oracle.integrate(y0[:k], m[:k], cfg.omegaf, 1e-10, 1e-12, n_threads=n_threads)
     pn_oracle.histogram(r["final"], cfg.bins)
     dt = time.perf_counter() - t0
-    cores = n_threads if n_threads > 0 else pn_oracle.num_threads()
-    return {"value": k / dt, "unit": "inspirals/s", "cores": cores, "kind": "oracle",
-            "sample": f"first {k} systems of the seeded {cfg.name} batch (FP64 oracle, rtol 1e-10, atol 1e-12), "
-                      f"{dt:.1f} s wall on {cores} threads, {os.cpu_count()} logical CPUs",
-            "rhs_evals_per_s": float((6 * r["steps"].astype(np.int64) + 1).sum() / dt), "seconds": dt,
-            "mean_steps": float(r["steps"].mean())}
+    out = {"value": k / dt, "unit": "inspirals/s", "cores": n_threads, "kind": "oracle", "cpu_model": cpu_model(),
+           "sample": f"random-permutation prefix of {k} systems of the seeded {cfg.name} batch (FP64 oracle, rtol 1e-10, atol 1e-12), "
+                     f"{dt:.1f} s wall on {n_threads} threads, {os.cpu_count()} logical CPUs",
+           "rhs_evals_per_s": float((6 * r["steps"].astype(np.int64) + 1).sum() / dt), "seconds": dt,
+           "mean_steps": float(r["steps"].mean())}
+    if single_thread:
+        # one thread on 256 systems: the figure comparable with the paper's single-core number
+        t0 = time.perf_counter()
+        pn_oracle.integrate(y0[:probe], m[:probe], cfg.omegaf, 1e-10, 1e-12, n_threads=1)
+        out["single_thread"] = {"value": probe / (time.perf_counter() - t0), "unit": "inspirals/s", "systems": probe}
+    return out
 
 
 def run_reference(args, cfg):
@@ -112,13 +136,69 @@ def run_reference(args, cfg):
     line = {"impl": "reference", "metric": "inspirals_per_sec", "value": value, "unit": "inspirals/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([p["seconds"] for p in per_step])),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "n_inspirals": cfg.n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
-                       "rtol": 1e-10, "atol": 1e-12, "note": "each step is a bounded sample of the workload"},
-            "cpu_baseline": {k: last[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "config": {"workload": cfg.name, "n_inspirals": cfg.n, "n_inspirals_per_gpu": cfg.n, "omega0": cfg.omega0,
+                       "omegaf": cfg.omegaf, "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins,
+                       "note": "each step is a bounded sample of the workload"},
+            "cpu_baseline": {k: last[k] for k in ("value", "unit", "cores", "kind", "sample", "cpu_model")},
             "e2e": {"value": value, "unit": "inspirals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "rhs_evals_per_sec": float(np.mean([p["rhs_evals_per_s"] for p in per_step])), "gpu_launches": 0}
     line["cpu_baseline"]["value"] = value
     print(json.dumps(line))
+
+
+def spawn_ranks_if_needed(args):
+    """`python bench.py --gpus N` (N > 1, no torchrun environment): re-execute under torch.distributed.run with N ranks on
+    this node.  Under torchrun a WORLD_SIZE that disagrees with --gpus is an error, never a silently mislabelled run."""
+    if "WORLD_SIZE" in os.environ:
+        world = int(os.environ["WORLD_SIZE"])
+        if args.gpus != world:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with --nproc-per-node {args.gpus}")
+        return
+    if args.gpus <= 1:
+        return
+    import socket
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def rank_shard(cfg, rank, world, scaling):
+    """This rank's share of the workload: (config to generate, slice of the generated batch, systems of the whole job)."""
+    from paper_0908_3889_b200 import sharding
+
+    if scaling == "strong":
+        lo, hi = sharding.shard_range(cfg.n, rank, world)          # one batch, contiguous balanced slices
+        return cfg, slice(lo, hi), cfg.n
+    return sharding.rank_config(cfg, rank), slice(0, cfg.n), cfg.n * world     # every rank its own full-size batch
+
+
+def run_dry(args, cfg):
+    """--dry: the multi-rank launch, sharding and exchange logic on the CPU with gloo; no CUDA, no kernels, no timing
+    claims.  Every rank contributes its shard size to the same all-reduce and max-reduction the real run uses."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_0908_3889_b200 import sharding
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    gen_cfg, sl, total = rank_shard(cfg, rank, world, args.scaling)
+    n_mine = len(range(*sl.indices(gen_cfg.n)))
+    counts = torch.zeros(3, cfg.bins, dtype=torch.int64)
+    counts[:, rank % cfg.bins] = n_mine                          # stand-in for this rank's histogram
+    sharding.allreduce_counts(counts, dist if world > 1 else None)
+    slowest = sharding.max_over_ranks(float(rank + 1), torch.device("cpu"), dist if world > 1 else None)
+    if rank == 0:
+        print(json.dumps({"dry": True, "n_gpus": world, "scaling": args.scaling, "seed_rank0": gen_cfg.seed,
+                          "systems_rank0": n_mine, "systems_all_ranks": int(counts[0].sum().item()), "systems_expected": total,
+                          "max_over_ranks": slowest, "config": {"workload": cfg.name}}))
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def run_ours(args, cfg):
@@ -138,10 +218,12 @@ def run_ours(args, cfg):
         dist.init_process_group("nccl", device_id=dev)
     prec = {"fp32": pn.PN_FP32, "mixed": pn.PN_MIXED}.get(cfg.precision, pn.PN_FP64)
 
-    # every rank integrates its own seeded batch of the full workload size (weak scaling)
+    # weak scaling: every rank integrates its own seeded batch of the full workload size; strong: its slice of one batch
     from paper_0908_3889_b200 import sharding
-    y0, m = W.generate(sharding.rank_config(cfg, rank))
-    n = cfg.n
+    gen_cfg, sl, total_inspirals = rank_shard(cfg, rank, world, args.scaling)
+    y0, m = W.generate(gen_cfg)
+    y0, m = np.ascontiguousarray(y0[sl]), np.ascontiguousarray(m[sl])
+    n = y0.shape[0]
     h_y0 = torch.from_numpy(y0).pin_memory(); h_m = torch.from_numpy(m).pin_memory()
     d_y0, d_m = h_y0.to(dev), h_m.to(dev)
     d_yf = torch.empty_like(d_y0)
@@ -182,6 +264,11 @@ def run_ours(args, cfg):
     ms_total = ev0.elapsed_time(ev1)
     ms_step = sharding.max_over_ranks(ms_total, dev, dist if world > 1 else None) / args.steps
     counters = pn.pn_last_counters()
+    # RHS evaluations of the whole job per step (6 per trial step + the seed evaluation), summed over ranks on the device
+    rhs_mine = torch.tensor([6.0 * float(np.mean(trial_steps)) + n], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(rhs_mine)
+    rhs_all_ranks = float(rhs_mine.item())
 
     # end to end through the C ABI with HOST buffers: H2D of inputs and D2H of results inside the timed region
     h_yf = torch.empty(n, 10, dtype=torch.float64).pin_memory()
@@ -249,27 +336,35 @@ def run_ours(args, cfg):
     peak_nominal = sms * lanes * 2 * sm_max * 1e6 / 1e12
     peak_prec = pn.PN_FP64 if prec == pn.PN_FP64 else pn.PN_FP32       # the pipe the slopes are computed on
     peak_meas, peak_mhz = pn.pn_measure_fma_peak(peak_prec, 0.5)
+    traffic, traffic_src = None, None
+    tj = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tj):
+        ent = json.load(open(tj)).get(f"{cfg.name}:{n}")
+        if ent:
+            traffic, traffic_src = float(ent["dram_bytes_read"]) + float(ent["dram_bytes_write"]), ent["source"]
     flops_launch = float(np.mean(trial_steps)) * F_STEP + n * F_RHS
     k_ms = float(np.mean(kern_ms))
     achieved = flops_launch / (k_ms * 1e-3) / 1e12
-    total_inspirals = n * world
     line = {
         "metric": "inspirals_per_sec", "value": total_inspirals / (ms_step * 1e-3), "unit": "inspirals/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
         "dtype": {pn.PN_FP32: "f32", pn.PN_MIXED: "f32 slopes + f64 state"}.get(prec, "f64"), "data": "synthetic",
-        "config": {"workload": cfg.name, "n_inspirals_per_gpu": n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
+        "comm": {"backend": "nccl" if world > 1 else None, "nranks": world, "exchange": "all-reduce of 3 x bins int64 counters per step"},
+        "config": {"workload": cfg.name, "n_inspirals": cfg.n, "n_inspirals_per_gpu": n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
                    "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "queue": "input order" if args.input_order else "longest-expected-first", "parallelism": f"batch-sharded x{world}",
                    "l2": "256 MiB memset between steps, inside the timed region (<0.1 % of a step)"},
-        "rhs_evals_per_sec": world * (6 * float(np.mean(trial_steps)) + n) / (ms_step * 1e-3),
+        "rhs_evals_per_sec": rhs_all_ranks / (ms_step * 1e-3),
         "trial_steps_per_inspiral": float(np.mean(trial_steps)) / n,
         "counters_last_step": counters,
         "kernel_ms": {"integrate": k_ms, "histogram": float(np.mean(hist_ms))},
         "roofline": {"bound": "alu", "kernel": "pn_integrate_adaptive_kernel", "achieved": achieved, "peak": peak_nominal,
                      "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-                     # dram__bytes_read + dram__bytes_write of this kernel per launch, from the ncu --set full capture of
-                     # the same workload and size (profiles/r1_v10_ncu_integrator.md); algorithmic bytes: 445 MB
-                     "traffic": 431.4e6 if (cfg.name == "C2" and n == (1 << 20)) else None, "traffic_unit": "bytes/launch",
+                     # dram__bytes_read + dram__bytes_write of this kernel per launch, from the committed ncu --set full
+                     # capture of the same workload and size (profiles/traffic.json names the capture); null if none.
+                     # algorithmic bytes: 96 B in + 100 B out (state, steps, time) per inspiral
+                     "traffic": traffic, "traffic_unit": "bytes/launch", "traffic_source": traffic_src,
+                     "algorithmic_bytes": 196 * n,
                      "peak_source": f"nominal {sms} SMs x {lanes} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md 6.3)",
                      "peak_measured_fma": peak_meas, "peak_measured_sm_mhz": peak_mhz,
                      "frac_of_measured_fma": achieved / peak_meas if peak_meas > 0 else None,
@@ -284,8 +379,8 @@ def run_ours(args, cfg):
     if widened:
         line["widened"] = widened
     if world == 1 and not args.no_cpu_baseline:
-        cb = oracle_throughput(cfg, target_seconds=args.cpu_seconds)
-        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        cb = oracle_throughput(cfg, target_seconds=args.cpu_seconds, single_thread=True)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "cpu_model", "single_thread")}
         line["cpu_baseline"]["rhs_evals_per_s"] = cb["rhs_evals_per_s"]
         line["paper_context"] = "paper: 0.057 inspirals/ms on 1 Xeon E5410 core (double) vs 2.7 inspirals/ms on 1 Tesla S1070 GPU (single), 'factor 50' (PAPER.md:86-96)"
     print(json.dumps(line))
@@ -304,11 +399,17 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--input-order", type=int, default=0, help="1: issue the work queue in input order instead of longest-expected-first")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: every rank its own full-size batch; strong: one batch split over the ranks")
+    ap.add_argument("--dry", action="store_true", help="launch / sharding / exchange logic only, on the CPU with gloo (tests)")
     args = ap.parse_args()
     cfg = W.CONFIGS[args.workload]
     if args.n > 0:
         cfg = W.with_size(cfg, args.n)
-    if args.impl == "reference":
+    spawn_ranks_if_needed(args)
+    if args.dry:
+        run_dry(args, cfg)
+    elif args.impl == "reference":
         run_reference(args, cfg)
     else:
         run_ours(args, cfg)

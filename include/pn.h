@@ -23,7 +23,12 @@
  *     arrays, work counter, status word) that pn_shutdown() frees.
  *   - Calls are synchronous: on return the outputs are complete (the stream has been synchronised).
  *     If pn_options.async != 0 and device pointers are used, the call only enqueues on
- *     pn_options.stream and the per-call status is collected by pn_stream_status().
+ *     pn_options.stream; pn_stream_status(stream) later returns the worst status of ALL async calls
+ *     enqueued on that stream since the last pn_stream_status.  Any number of async calls may be in
+ *     flight, on one stream or several: the library keeps one scratch context (staging arrays, work
+ *     counters, status words) per stream, and calls on one stream are ordered by the stream.  The
+ *     caller's own buffers must of course not be reused by a second call before the first has finished
+ *     unless both calls are on the same stream.
  *   - N = 0 is a successful no-op.  Not thread-safe: one caller thread per process.
  */
 #ifndef PN_B200_H
@@ -95,6 +100,9 @@ typedef struct pn_options {
     void* stream;          /* cudaStream_t, or NULL for the default stream */
     int block_threads;     /* tuning: threads per block of the integrator (0: default) */
     int grid_blocks;       /* tuning: blocks of the persistent grid (0: SMs x resident blocks) */
+    int variant;           /* tests / tuning: kernel selection bits, results are unchanged.  1: always the generic FP64
+                              kernel (per-lane constants) even for uniform-mass batches; 2: always the
+                              scalar FP32 kernel instead of the packed two-systems-per-lane one */
 } pn_options;
 
 /* Same as pn_integrate with explicit options (opt == NULL: defaults). */
@@ -228,7 +236,9 @@ int pn_selfcheck(const double* init_states, const double* masses, const double* 
                  double atol_ref, pn_check_out* out, long long* checked_indices, long long max_indices,
                  const struct pn_options* opt);
 
-/* Worst pn_status of the async calls enqueued on `stream` since the last pn_stream_status; synchronises it. */
+/* Worst pn_status of the async calls enqueued on `stream` since the last pn_stream_status (a later call never
+ * erases an earlier call's status); synchronises the stream.  pn_last_counters() then refers to the last call
+ * enqueued on that stream. */
 int pn_stream_status(void* stream);
 
 /*

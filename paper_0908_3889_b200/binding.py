@@ -27,7 +27,7 @@ class PnOptions(C.Structure):
     _fields_ = [("size", C.c_int), ("fixed_steps", C.c_int), ("h0", C.c_double), ("max_steps", C.c_int),
                 ("term_mask", C.c_uint), ("tau_land", C.c_double), ("layout", C.c_int), ("host_buffers", C.c_int),
                 ("async_", C.c_int), ("input_order", C.c_int), ("out_time", C.c_void_p), ("out_rejected", C.c_void_p),
-                ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int)]
+                ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int), ("variant", C.c_int)]
 
 
 class PnStatsOut(C.Structure):
@@ -121,16 +121,49 @@ def _is_host(a) -> bool:
     return isinstance(a, np.ndarray) or (hasattr(a, "is_cuda") and not a.is_cuda)
 
 
+_DTYPES = {"f64": ("float64",), "i32": ("int32",), "i64": ("int64", "uint64")}
+
+
+def _require(name, a, dtype, shape=None, host=None, at_least=False):
+    """The C ABI takes raw pointers: a wrong dtype, a non-contiguous view, a short array or a tensor on another device
+    would be read or written out of bounds by the kernels.  Checked here, before the call (None passes).
+    at_least: an output that only has to be large enough (element count), whatever its shape."""
+    if a is None:
+        return
+    dt = str(a.dtype).replace("torch.", "")
+    if dt not in _DTYPES[dtype]:
+        raise ValueError(f"{name}: dtype {dt}, expected {_DTYPES[dtype][0]}")
+    contiguous = a.flags["C_CONTIGUOUS"] if isinstance(a, np.ndarray) else a.is_contiguous()
+    if not contiguous:
+        raise ValueError(f"{name}: array is not contiguous")
+    if shape is not None and at_least:
+        need = int(np.prod([int(w) for w in shape])) if len(shape) else 1
+        have = int(np.prod([int(x) for x in a.shape])) if len(a.shape) else 1
+        if have < need:
+            raise ValueError(f"{name}: {have} elements, the call writes {need}")
+    elif shape is not None:
+        got = tuple(int(x) for x in a.shape)
+        if len(got) != len(shape) or any(w is not None and g != w for g, w in zip(got, shape)):
+            raise ValueError(f"{name}: shape {got}, expected {tuple('*' if w is None else w for w in shape)}")
+    if host is not None and _is_host(a) != host:
+        raise ValueError(f"{name}: all arrays of one call must live on the same side (host or device)")
+    if not _is_host(a):
+        import torch
+
+        if a.device.index != torch.cuda.current_device():
+            raise ValueError(f"{name}: tensor is on cuda:{a.device.index}, the current device is cuda:{torch.cuda.current_device()}")
+
+
 def make_options(*, fixed_steps=0, h0=0.0, max_steps=0, term_mask=0, tau_land=0.0, layout=0, host_buffers=False,
                  async_=False, input_order=False, out_time=None, out_rejected=None, stream=None, block_threads=0,
-                 grid_blocks=0) -> PnOptions:
+                 grid_blocks=0, variant=0) -> PnOptions:
     o = PnOptions()
     o.size = C.sizeof(PnOptions)
     o.fixed_steps, o.h0, o.max_steps, o.term_mask, o.tau_land = int(fixed_steps), float(h0), int(max_steps), int(term_mask), float(tau_land)
     o.layout, o.host_buffers, o.async_, o.input_order = int(layout), int(bool(host_buffers)), int(bool(async_)), int(bool(input_order))
     o.out_time, o.out_rejected = _ptr(out_time), _ptr(out_rejected)
     o.stream = None if stream is None else int(getattr(stream, "cuda_stream", stream))
-    o.block_threads, o.grid_blocks = int(block_threads), int(grid_blocks)
+    o.block_threads, o.grid_blocks, o.variant = int(block_threads), int(grid_blocks), int(variant)
     return o
 
 
@@ -142,9 +175,13 @@ def pn_integrate(init_states, masses, omega0, omegaf, rtol, atol, precision, out
     lib = load()
     n = int(out_steps.shape[0])
     host = _is_host(init_states)
-    for a in (masses, out_final, out_steps, opts.get("out_time"), opts.get("out_rejected")):
-        if a is not None and _is_host(a) != host:
-            raise ValueError("all arrays of one call must live on the same side (host or device)")
+    soa = opts.get("layout", 0) == 1
+    _require("init_states", init_states, "f64", (10, n) if soa else (n, 10), host)
+    _require("masses", masses, "f64", (2, n) if soa else (n, 2), host)
+    _require("out_final", out_final, "f64", (10, n) if soa else (n, 10), host)
+    _require("out_steps", out_steps, "i32", (n,), host)
+    _require("out_time", opts.get("out_time"), "f64", (n,), host)
+    _require("out_rejected", opts.get("out_rejected"), "i32", (n,), host)
     if host:
         opts["host_buffers"] = True
     o = make_options(**opts)
@@ -156,9 +193,16 @@ def pn_integrate(init_states, masses, omega0, omegaf, rtol, atol, precision, out
 def pn_histogram(final_states, bins, counts, n_skipped=None, *, n=None, **opts):
     """pn_histogram_ex of include/pn.h: counts[3, bins] uint64 (torch int64 storage is accepted)."""
     lib = load()
+    soa = opts.get("layout", 0) == 1
     if n is None:
-        n = int(final_states.shape[1] if opts.get("layout", 0) == 1 else final_states.shape[0])
-    if _is_host(final_states):
+        n = int(final_states.shape[1] if soa else final_states.shape[0])
+    host = _is_host(final_states)
+    _require("final_states", final_states, "f64", (10, None) if soa else (None, 10), host)
+    if int(final_states.shape[1 if soa else 0]) < n:
+        raise ValueError("final_states holds fewer than n systems")
+    _require("counts", counts, "i64", (3, max(int(bins), 0)), host, at_least=True)
+    _require("n_skipped", n_skipped, "i64", (3,), host, at_least=True)
+    if host:
         opts["host_buffers"] = True
     o = make_options(**opts)
     return _check(lib.pn_histogram_ex(_ptr(final_states), int(n), int(bins), _ptr(counts), _ptr(n_skipped), C.byref(o)))
@@ -170,7 +214,20 @@ def pn_statistics(init_states, final_states, steps=None, *, group_size=0, bins1=
     the inputs are on the host); any of them may be None.  init_states may be None (final-only mode)."""
     lib = load()
     n = int(final_states.shape[0])
-    if _is_host(final_states):
+    host = _is_host(final_states)
+    gs = int(group_size) if int(group_size) > 0 else max(n, 1)
+    G = n // gs if n else 0
+    _require("final_states", final_states, "f64", (n, 10), host)
+    _require("init_states", init_states, "f64", (n, 10), host)
+    _require("steps", steps, "i32", (n,), host)
+    _require("pearson_r", pearson_r, "f64", (G, 3), host, at_least=True)
+    _require("moments", moments, "f64", (G, 3, 6), host, at_least=True)
+    _require("n_skipped", n_skipped, "i64", (G, 3), host, at_least=True)
+    _require("hist1", hist1, "i64", (G, 3, int(bins1)), host, at_least=True)
+    _require("hist2", hist2, "i64", (G, 3, int(bins2), int(bins2)), host, at_least=True)
+    _require("hist2_max", hist2_max, "i64", (G, 3), host, at_least=True)
+    _require("hist2_norm", hist2_norm, "f64", (G, 3, int(bins2), int(bins2)), host, at_least=True)
+    if host:
         opts["host_buffers"] = True
     o = make_options(**opts)
     out = PnStatsOut()
@@ -184,6 +241,9 @@ def pn_statistics(init_states, final_states, steps=None, *, group_size=0, bins1=
 def pn_merge_statistics(parts, moments=None, pearson_r=None, **opts):
     """pn_merge_statistics of include/pn.h: parts [R, G, 3, 6] (torch CUDA float64) -> moments [G, 3, 6], pearson_r [G, 3]."""
     lib = load()
+    _require("parts", parts, "f64", (None, None, 3, 6), False)
+    _require("moments", moments, "f64", (int(parts.shape[1]), 3, 6), False, at_least=True)
+    _require("pearson_r", pearson_r, "f64", (int(parts.shape[1]), 3), False, at_least=True)
     o = make_options(**opts)
     return _check(lib.pn_merge_statistics(_ptr(parts), int(parts.shape[0]), int(parts.shape[1]), _ptr(moments), _ptr(pearson_r),
                                           C.byref(o)))
@@ -196,7 +256,10 @@ def pn_generate(ensembles, n_total, init_states, masses, *, first=0, count=None,
     ens = ensembles if isinstance(ensembles, (list, tuple)) else [ensembles]
     arr = (PnEnsemble * len(ens))(*ens)
     count = int(n_total) - int(first) if count is None else int(count)
-    if _is_host(init_states):
+    host = _is_host(init_states)
+    _require("init_states", init_states, "f64", (len(ens) * max(count, 0), 10), host)
+    _require("masses", masses, "f64", (len(ens) * max(count, 0), 2), host)
+    if host:
         opts["host_buffers"] = True
     o = make_options(**opts)
     return _check(lib.pn_generate(arr, len(ens), int(n_total), int(first), count, _ptr(init_states), _ptr(masses), C.byref(o)))
@@ -207,7 +270,13 @@ def pn_selfcheck(init_states, masses, final_states, omegaf, *, fraction=0.01, ke
     """pn_selfcheck of include/pn.h (the paper's 1 % double-precision cross-check).  Returns a dict."""
     lib = load()
     n = int(final_states.shape[0])
-    if _is_host(final_states):
+    host = _is_host(final_states)
+    _require("init_states", init_states, "f64", (n, 10), host)
+    _require("masses", masses, "f64", (n, 2), host)
+    _require("final_states", final_states, "f64", (n, 10), host)
+    _require("times", times, "f64", (n,), host)
+    _require("checked_indices", checked_indices, "i64", (None,), host)
+    if host:
         opts["host_buffers"] = True
     o = make_options(**opts)
     out = PnCheckOut()

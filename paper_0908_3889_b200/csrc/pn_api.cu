@@ -42,22 +42,46 @@ struct Buf {
         return PN_OK;
     }
 };
-static Buf g_soa_in, g_soa_m, g_soa_out, g_small, g_redo, g_seed, g_sort_keys, g_sort_idx, g_sort_tmp, g_h_init, g_h_m, g_h_final, g_h_steps, g_h_time, g_h_rej, g_h_counts, g_st_scratch, g_st_in, g_st_out, g_gen_specs, g_gen_y, g_gen_m, g_ck_idx, g_ck_tmp, g_ck_sub, g_ck_out, g_ck_in;
-static cudaEvent_t g_ev[5];
-static bool g_ev_ok = false;
+// One scratch context per stream: two calls in flight on different streams never share a buffer, a work counter or
+// a status word (the single global set was aliased by concurrent async calls).  Calls on ONE stream are
+// ordered by the stream, so they may share their context's buffers; what they must not share is the status word:
+// every call owns the status in its (re-zeroed) Small block and async calls fold it into the context's sticky word
+// with a one-thread kernel at the end, which only pn_stream_status reads and clears.
+struct Ctx {
+    Buf soa_in, soa_m, soa_out, small, sticky, redo, seed, keys, order, ord_scr, h_init, h_m, h_final, h_steps, h_time, h_rej,
+        h_counts, st_scratch, st_in, st_out, gen_specs, gen_y, gen_m, ck_idx, ck_tmp, ck_sub, ck_out, ck_in;
+    cudaEvent_t ev[5];
+    bool ev_ok = false;
+    bool async_pending = false;
+    int slot = -1;              // row of the __constant__ table of the uniform-mass kernel; -1: none left (generic kernel only)
+    Buf* all[28] = {&soa_in, &soa_m, &soa_out, &small, &sticky, &redo, &seed, &keys, &order, &ord_scr, &h_init, &h_m, &h_final,
+                    &h_steps, &h_time, &h_rej, &h_counts, &st_scratch, &st_in, &st_out, &gen_specs, &gen_y, &gen_m, &ck_idx,
+                    &ck_tmp, &ck_sub, &ck_out, &ck_in};
+};
+static std::map<void*, Ctx*> g_ctx;
+static int g_next_slot = 0;
 static float g_ms[4] = {0, 0, 0, 0};
 static unsigned long long g_counters[4] = {0, 0, 0, 0};
 static unsigned g_redo_count = 0;   // systems that went through the redo pass in the last synchronous call
-static std::map<void*, int> g_stream_status;
+
+static Ctx* ctx_for(void* stream)
+{
+    auto it = g_ctx.find(stream);
+    if (it != g_ctx.end()) return it->second;
+    Ctx* c = new Ctx();
+    c->slot = g_next_slot < PN_UNI_SLOTS ? g_next_slot++ : -1;
+    g_ctx[stream] = c;
+    return c;
+}
 
 // layout of g_small: [0..3] counters (u64), then queue (u32), status (i32)
 struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned int queue2; unsigned int redo_count; unsigned long long skipped[3]; int nonuniform; int pad; };
 
-static int ensure_events()
+static int ensure_events(Ctx& c)
 {
-    if (!g_ev_ok) {
-        for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&g_ev[i]));
-        g_ev_ok = true;
+    if (!c.ev_ok) {
+        for (int i = 0; i < 5; ++i) CK(cudaEventCreate(&c.ev[i]));
+        c.ev_ok = true;
     }
     return PN_OK;
 }
@@ -90,9 +114,10 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     if (o.async && o.host_buffers) return PN_EINVAL;
     if (o.block_threads != 0 && o.block_threads != 128 && o.block_threads != 256) return PN_EINVAL;
     cudaStream_t s = (cudaStream_t)o.stream;
+    Ctx& c = *ctx_for(o.stream);
     const int n = (int)N;
     int rc;
-    if ((rc = ensure_events()) != PN_OK) return rc;
+    if ((rc = ensure_events(c)) != PN_OK) return rc;
 
     // ---- host buffers: stage through device scratch ----
     const double* d_init = init_states;
@@ -102,50 +127,47 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     double* d_time = o.out_time;
     int* d_rej = o.out_rejected;
     if (o.host_buffers) {
-        if ((rc = g_h_init.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_h_m.ensure(sizeof(double) * 2 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_h_final.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_h_steps.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
-        if (o.out_time && (rc = g_h_time.ensure(sizeof(double) * (size_t)n)) != PN_OK) return rc;
-        if (o.out_rejected && (rc = g_h_rej.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
-        CK(cudaMemcpyAsync(g_h_init.p, init_states, sizeof(double) * 10 * (size_t)n, cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(g_h_m.p, masses, sizeof(double) * 2 * (size_t)n, cudaMemcpyHostToDevice, s));
-        d_init = (const double*)g_h_init.p; d_m = (const double*)g_h_m.p;
-        d_final = (double*)g_h_final.p; d_steps = (int*)g_h_steps.p;
-        d_time = o.out_time ? (double*)g_h_time.p : nullptr;
-        d_rej = o.out_rejected ? (int*)g_h_rej.p : nullptr;
+        if ((rc = c.h_init.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.h_m.ensure(sizeof(double) * 2 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.h_final.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.h_steps.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+        if (o.out_time && (rc = c.h_time.ensure(sizeof(double) * (size_t)n)) != PN_OK) return rc;
+        if (o.out_rejected && (rc = c.h_rej.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+        CK(cudaMemcpyAsync(c.h_init.p, init_states, sizeof(double) * 10 * (size_t)n, cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(c.h_m.p, masses, sizeof(double) * 2 * (size_t)n, cudaMemcpyHostToDevice, s));
+        d_init = (const double*)c.h_init.p; d_m = (const double*)c.h_m.p;
+        d_final = (double*)c.h_final.p; d_steps = (int*)c.h_steps.p;
+        d_time = o.out_time ? (double*)c.h_time.p : nullptr;
+        d_rej = o.out_rejected ? (int*)c.h_rej.p : nullptr;
     }
 
-    // ---- SoA staging ----
-    if ((rc = g_small.ensure(sizeof(Small))) != PN_OK) return rc;
-    Small* small = (Small*)g_small.p;
+    // ---- per-call work counters and status (stream-ordered: an earlier call on this stream has finished with them) ----
+    if ((rc = c.small.ensure(sizeof(Small))) != PN_OK) return rc;
+    Small* small = (Small*)c.small.p;
     CK(cudaMemsetAsync(small, 0, sizeof(Small), s));
     PnKernelParams p;
     memset(&p, 0, sizeof p);
-    CK(cudaEventRecord(g_ev[0], s));
+    CK(cudaEventRecord(c.ev[0], s));
+    // ---- SoA staging ----
     if (o.layout == 0) {
-        if ((rc = g_soa_in.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_soa_m.ensure(sizeof(double) * 2 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_soa_out.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
-        CK(pn_launch_aos_to_soa(d_init, (double*)g_soa_in.p, n, 10, s));
-        CK(pn_launch_aos_to_soa(d_m, (double*)g_soa_m.p, n, 2, s));
-        p.y0 = (const double*)g_soa_in.p; p.masses = (const double*)g_soa_m.p; p.yf = (double*)g_soa_out.p;
+        if ((rc = c.soa_in.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.soa_m.ensure(sizeof(double) * 2 * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.soa_out.ensure(sizeof(double) * 10 * (size_t)n)) != PN_OK) return rc;
+        CK(pn_launch_aos_to_soa(d_init, (double*)c.soa_in.p, n, 10, s));
+        CK(pn_launch_aos_to_soa(d_m, (double*)c.soa_m.p, n, 2, s));
+        p.y0 = (const double*)c.soa_in.p; p.masses = (const double*)c.soa_m.p; p.yf = (double*)c.soa_out.p;
     } else {
         p.y0 = d_init; p.masses = d_m; p.yf = d_final;
     }
-    p.order = nullptr;
     if (!o.input_order && !fixed && n > 1024) {
-        // longest-expected-first queue order; part of the stage-in time
-        const size_t tb = pn_cost_order_temp_bytes(n);
-        if ((rc = g_sort_keys.ensure(sizeof(float) * 2 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_sort_idx.ensure(sizeof(int) * 2 * (size_t)n)) != PN_OK) return rc;
-        if ((rc = g_sort_tmp.ensure(tb)) != PN_OK) return rc;
-        float* keys = (float*)g_sort_keys.p;
-        int* idx = (int*)g_sort_idx.p;
-        CK(pn_launch_cost_order(p.y0, p.masses, n, omegaf, keys, keys + n, idx, idx + n, g_sort_tmp.p, tb, s));
-        p.order = idx + n;
+        // longest-expected-first queue order: keys from the seed kernel, then a bucket sort
+        if ((rc = c.keys.ensure(sizeof(float) * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.order.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+        if ((rc = c.ord_scr.ensure(sizeof(unsigned) * (PN_ORDER_BUCKETS + 2))) != PN_OK) return rc;
+        p.keys = (float*)c.keys.p; p.order_out = (int*)c.order.p; p.order = p.order_out;
+        p.order_scratch = (unsigned*)c.ord_scr.p;
     }
-    CK(cudaEventRecord(g_ev[1], s));
+    CK(cudaEventRecord(c.ev[1], s));
     p.steps = d_steps; p.time = d_time; p.rejected = d_rej;
     p.n = n;
     p.omega0 = omega0; p.omegaf = omegaf; p.rtol = rtol; p.atol = atol; p.h0 = o.h0;
@@ -159,22 +181,26 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
     p.fixed_steps = fixed ? o.fixed_steps : 0;
     p.mask = o.term_mask;
-    if ((rc = g_redo.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
+    if ((rc = c.redo.ensure(sizeof(int) * (size_t)n)) != PN_OK) return rc;
     if (!fixed) {
-        if ((rc = g_seed.ensure((precision == PN_FP64 ? sizeof(double) : sizeof(float)) * 40 * (size_t)n)) != PN_OK) return rc;
-        p.seed = g_seed.p;
+        if ((rc = c.seed.ensure((precision == PN_FP64 ? sizeof(double) : sizeof(float)) * 40 * (size_t)n)) != PN_OK) return rc;
+        p.seed = c.seed.p;
     }
     p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
-    p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = (int*)g_redo.p;
+    p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = (int*)c.redo.p;
     p.nonuniform = &small->nonuniform;
-    CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s, !o.async));
-    CK(cudaEventRecord(g_ev[2], s));
-    if (o.layout == 0) CK(pn_launch_soa_to_aos((const double*)g_soa_out.p, d_final, n, 10, s));
-    CK(cudaEventRecord(g_ev[3], s));
+    p.uni_slot = c.slot;
+    CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s, o.variant));
+    CK(cudaEventRecord(c.ev[2], s));
+    if (o.layout == 0) CK(pn_launch_soa_to_aos((const double*)c.soa_out.p, d_final, n, 10, s));
+    CK(cudaEventRecord(c.ev[3], s));
 
     if (o.async) {
-        // status is collected by pn_stream_status(); the Small block must stay untouched until then
-        g_stream_status[o.stream] = PN_OK;
+        // the call's status is folded into the stream's sticky word, which pn_stream_status() reads and clears
+        if ((rc = c.sticky.ensure(sizeof(int))) != PN_OK) return rc;
+        if (!c.async_pending) CK(cudaMemsetAsync(c.sticky.p, 0, sizeof(int), s));
+        CK(pn_launch_fold_status(&small->status, (int*)c.sticky.p, s));
+        c.async_pending = true;
         return PN_OK;
     }
     if (o.host_buffers) {
@@ -187,7 +213,7 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     CK(cudaMemcpyAsync(&hs, small, sizeof hs, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
-    for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&g_ms[i], g_ev[i], g_ev[i + 1]));
+    for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&g_ms[i], c.ev[i], c.ev[i + 1]));
     memcpy(g_counters, hs.counters, sizeof g_counters);
     g_redo_count = hs.redo_count;
     return hs.status;
@@ -213,34 +239,35 @@ extern "C" int pn_histogram_ex(const double* final_states, long long N, int bins
     if (N > 0 && !final_states) return PN_EINVAL;
     if (o.async && o.host_buffers) return PN_EINVAL;
     cudaStream_t s = (cudaStream_t)o.stream;
+    Ctx& c = *ctx_for(o.stream);
     int rc;
-    if ((rc = ensure_events()) != PN_OK) return rc;
+    if ((rc = ensure_events(c)) != PN_OK) return rc;
     const double* d_st = final_states;
     unsigned long long* d_counts = counts;
     unsigned long long* d_skip = n_skipped;
     if (o.host_buffers) {
         if (N > 0) {
-            if ((rc = g_h_final.ensure(sizeof(double) * 10 * (size_t)N)) != PN_OK) return rc;
-            CK(cudaMemcpyAsync(g_h_final.p, final_states, sizeof(double) * 10 * (size_t)N, cudaMemcpyHostToDevice, s));
-            d_st = (const double*)g_h_final.p;
+            if ((rc = c.h_final.ensure(sizeof(double) * 10 * (size_t)N)) != PN_OK) return rc;
+            CK(cudaMemcpyAsync(c.h_final.p, final_states, sizeof(double) * 10 * (size_t)N, cudaMemcpyHostToDevice, s));
+            d_st = (const double*)c.h_final.p;
         }
-        if ((rc = g_h_counts.ensure(sizeof(unsigned long long) * (3 * (size_t)bins + 3))) != PN_OK) return rc;
-        d_counts = (unsigned long long*)g_h_counts.p;
+        if ((rc = c.h_counts.ensure(sizeof(unsigned long long) * (3 * (size_t)bins + 3))) != PN_OK) return rc;
+        d_counts = (unsigned long long*)c.h_counts.p;
         d_skip = d_counts + 3 * (size_t)bins;
     }
     // AoS, 16-byte aligned, moderate bin count: the bulk-copy streaming kernel of pn_stats.cu in its final-only mode
     // (3.1 TB/s at 2^22 systems); otherwise (SoA layout, odd alignment, huge bin counts) the plain kernel of pn_aux.cu
     const bool bulk = o.layout == 0 && N > 0 && bins <= 8192 && (((uintptr_t)d_st) & 15u) == 0;
-    if (bulk && (rc = g_st_scratch.ensure(pn_stats_scratch_bytes(N, 0, nullptr))) != PN_OK) return rc;
-    CK(cudaEventRecord(g_ev[3], s));
+    if (bulk && (rc = c.st_scratch.ensure(pn_stats_scratch_bytes(N, 0, nullptr))) != PN_OK) return rc;
+    CK(cudaEventRecord(c.ev[3], s));
     if (bulk) {
         if (d_skip) CK(cudaMemsetAsync(d_skip, 0, sizeof(unsigned long long) * 3, s));
-        CK(pn_launch_stats(nullptr, d_st, nullptr, N, 0, bins, 0, g_st_scratch.p, nullptr, nullptr, d_skip, d_counts, nullptr,
+        CK(pn_launch_stats(nullptr, d_st, nullptr, N, 0, bins, 0, c.st_scratch.p, nullptr, nullptr, d_skip, d_counts, nullptr,
                            nullptr, nullptr, s));
     } else {
         CK(pn_launch_histogram(d_st, o.layout, N, bins, d_counts, d_skip, s));
     }
-    CK(cudaEventRecord(g_ev[4], s));
+    CK(cudaEventRecord(c.ev[4], s));
     if (o.async) return PN_OK;
     if (o.host_buffers) {
         CK(cudaMemcpyAsync(counts, d_counts, sizeof(unsigned long long) * 3 * (size_t)bins, cudaMemcpyDeviceToHost, s));
@@ -248,7 +275,7 @@ extern "C" int pn_histogram_ex(const double* final_states, long long N, int bins
     }
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
-    CK(cudaEventElapsedTime(&g_ms[3], g_ev[3], g_ev[4]));
+    CK(cudaEventElapsedTime(&g_ms[3], c.ev[3], c.ev[4]));
     return PN_OK;
 }
 
@@ -283,9 +310,10 @@ extern "C" int pn_statistics(const double* init_states, const double* final_stat
     if (N == 0) return PN_OK;
     if (!o.host_buffers && (((uintptr_t)final_states & 15u) || ((uintptr_t)init_states & 15u))) return PN_EINVAL;
     cudaStream_t s = (cudaStream_t)o.stream;
+    Ctx& c = *ctx_for(o.stream);
     int rc;
-    if ((rc = ensure_events()) != PN_OK) return rc;
-    if ((rc = g_st_scratch.ensure(pn_stats_scratch_bytes(N, group_size, nullptr))) != PN_OK) return rc;
+    if ((rc = ensure_events(c)) != PN_OK) return rc;
+    if ((rc = c.st_scratch.ensure(pn_stats_scratch_bytes(N, group_size, nullptr))) != PN_OK) return rc;
 
     const double* d_init = init_states;
     const double* d_fin = final_states;
@@ -297,14 +325,14 @@ extern "C" int pn_statistics(const double* init_states, const double* final_stat
     const size_t b_h1 = sizeof(unsigned long long) * 3 * (size_t)bins1 * G, b_h2 = sizeof(unsigned long long) * 3 * (size_t)bins2 * bins2 * G;
     if (o.host_buffers) {
         const size_t in_bytes = row * (init_states ? 2 : 1) + (steps ? sizeof(int) * (size_t)N : 0);
-        if ((rc = g_st_in.ensure(in_bytes)) != PN_OK) return rc;
-        char* q = (char*)g_st_in.p;
+        if ((rc = c.st_in.ensure(in_bytes)) != PN_OK) return rc;
+        char* q = (char*)c.st_in.p;
         CK(cudaMemcpyAsync(q, final_states, row, cudaMemcpyHostToDevice, s));
         d_fin = (const double*)q; q += row;
         if (init_states) { CK(cudaMemcpyAsync(q, init_states, row, cudaMemcpyHostToDevice, s)); d_init = (const double*)q; q += row; }
         if (steps) { CK(cudaMemcpyAsync(q, steps, sizeof(int) * (size_t)N, cudaMemcpyHostToDevice, s)); d_steps = (const int*)q; }
-        if ((rc = g_st_out.ensure(b_r + b_m + 2 * b_sk + b_h1 + 2 * b_h2 + 64)) != PN_OK) return rc;
-        char* w = (char*)g_st_out.p;
+        if ((rc = c.st_out.ensure(b_r + b_m + 2 * b_sk + b_h1 + 2 * b_h2 + 64)) != PN_OK) return rc;
+        char* w = (char*)c.st_out.p;
         auto take = [&](size_t bytes) { char* r = w; w += (bytes + 15) & ~(size_t)15; return r; };
         if (out.pearson_r) d.pearson_r = (double*)take(b_r);
         if (out.moments) d.moments = (double*)take(b_m);
@@ -314,10 +342,10 @@ extern "C" int pn_statistics(const double* init_states, const double* final_stat
         if (out.hist2_max) d.hist2_max = (unsigned long long*)take(b_sk);
         if (out.hist2_norm) d.hist2_norm = (double*)take(b_h2);
     }
-    CK(cudaEventRecord(g_ev[3], s));
-    CK(pn_launch_stats(d_init, d_fin, d_steps, N, group_size, bins1, bins2, g_st_scratch.p, d.pearson_r, d.moments,
+    CK(cudaEventRecord(c.ev[3], s));
+    CK(pn_launch_stats(d_init, d_fin, d_steps, N, group_size, bins1, bins2, c.st_scratch.p, d.pearson_r, d.moments,
                        d.n_skipped, d.hist1, d.hist2, d.hist2_max, d.hist2_norm, s));
-    CK(cudaEventRecord(g_ev[4], s));
+    CK(cudaEventRecord(c.ev[4], s));
     if (o.async) return PN_OK;
     if (o.host_buffers) {
         if (out.pearson_r) CK(cudaMemcpyAsync(out.pearson_r, d.pearson_r, b_r, cudaMemcpyDeviceToHost, s));
@@ -330,7 +358,7 @@ extern "C" int pn_statistics(const double* init_states, const double* final_stat
     }
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
-    CK(cudaEventElapsedTime(&g_ms[3], g_ev[3], g_ev[4]));
+    CK(cudaEventElapsedTime(&g_ms[3], c.ev[3], c.ev[4]));
     return PN_OK;
 }
 
@@ -380,22 +408,23 @@ extern "C" int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_
         memcpy(h[e].v, v, sizeof v);
     }
     cudaStream_t s = (cudaStream_t)o.stream;
+    Ctx& c = *ctx_for(o.stream);
     int rc;
-    if ((rc = ensure_events()) != PN_OK) return rc;
-    if ((rc = g_gen_specs.ensure(sizeof(Spec) * (size_t)n_ensembles)) != PN_OK) return rc;
-    CK(cudaMemcpyAsync(g_gen_specs.p, h.data(), sizeof(Spec) * (size_t)n_ensembles, cudaMemcpyHostToDevice, s));
+    if ((rc = ensure_events(c)) != PN_OK) return rc;
+    if ((rc = c.gen_specs.ensure(sizeof(Spec) * (size_t)n_ensembles)) != PN_OK) return rc;
+    CK(cudaMemcpyAsync(c.gen_specs.p, h.data(), sizeof(Spec) * (size_t)n_ensembles, cudaMemcpyHostToDevice, s));
     CK(cudaStreamSynchronize(s));      // h is a local: the copy must have left it before we return
     const size_t rows = (size_t)n_ensembles * (size_t)count;
     double* d_y = init_states;
     double* d_m = masses;
     if (o.host_buffers) {
-        if ((rc = g_gen_y.ensure(sizeof(double) * 10 * rows)) != PN_OK) return rc;
-        if ((rc = g_gen_m.ensure(sizeof(double) * 2 * rows)) != PN_OK) return rc;
-        d_y = (double*)g_gen_y.p; d_m = (double*)g_gen_m.p;
+        if ((rc = c.gen_y.ensure(sizeof(double) * 10 * rows)) != PN_OK) return rc;
+        if ((rc = c.gen_m.ensure(sizeof(double) * 2 * rows)) != PN_OK) return rc;
+        d_y = (double*)c.gen_y.p; d_m = (double*)c.gen_m.p;
     }
-    CK(cudaEventRecord(g_ev[0], s));
-    CK(pn_launch_generate(g_gen_specs.p, n_ensembles, n_total, first, count, d_y, d_m, s));
-    CK(cudaEventRecord(g_ev[1], s));
+    CK(cudaEventRecord(c.ev[0], s));
+    CK(pn_launch_generate(c.gen_specs.p, n_ensembles, n_total, first, count, d_y, d_m, s));
+    CK(cudaEventRecord(c.ev[1], s));
     if (o.async) return PN_OK;
     if (o.host_buffers) {
         CK(cudaMemcpyAsync(init_states, d_y, sizeof(double) * 10 * rows, cudaMemcpyDeviceToHost, s));
@@ -403,7 +432,7 @@ extern "C" int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_
     }
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
-    CK(cudaEventElapsedTime(&g_ms[0], g_ev[0], g_ev[1]));
+    CK(cudaEventElapsedTime(&g_ms[0], c.ev[0], c.ev[1]));
     return PN_OK;
 }
 
@@ -429,12 +458,13 @@ extern "C" int pn_selfcheck(const double* init_states, const double* masses, con
     for (int k = 0; k < 3; ++k) { out->max_dot_dev[k] = 0.0; out->worst_index[k] = -1; }
     if (N == 0) return PN_OK;
     cudaStream_t s = (cudaStream_t)o.stream;
+    Ctx& c = *ctx_for(o.stream);
     int rc;
     const double* d_init = init_states; const double* d_m = masses; const double* d_fin = final_states; const double* d_t = times;
     if (o.host_buffers) {
         const size_t rows = sizeof(double) * (size_t)N;
-        if ((rc = g_ck_in.ensure(rows * 23)) != PN_OK) return rc;
-        double* q = (double*)g_ck_in.p;
+        if ((rc = c.ck_in.ensure(rows * 23)) != PN_OK) return rc;
+        double* q = (double*)c.ck_in.p;
         CK(cudaMemcpyAsync(q, init_states, rows * 10, cudaMemcpyHostToDevice, s)); d_init = q; q += 10 * N;
         CK(cudaMemcpyAsync(q, final_states, rows * 10, cudaMemcpyHostToDevice, s)); d_fin = q; q += 10 * N;
         CK(cudaMemcpyAsync(q, masses, rows * 2, cudaMemcpyHostToDevice, s)); d_m = q; q += 2 * N;
@@ -442,11 +472,11 @@ extern "C" int pn_selfcheck(const double* init_states, const double* masses, con
     }
     // 1. selection (sorted index list + count)
     const size_t tb = pn_check_select_temp_bytes(N);
-    if ((rc = g_ck_idx.ensure(sizeof(long long) * ((size_t)N + 1))) != PN_OK) return rc;
-    if ((rc = g_ck_tmp.ensure(tb)) != PN_OK) return rc;
-    long long* d_idx = (long long*)g_ck_idx.p;
+    if ((rc = c.ck_idx.ensure(sizeof(long long) * ((size_t)N + 1))) != PN_OK) return rc;
+    if ((rc = c.ck_tmp.ensure(tb)) != PN_OK) return rc;
+    long long* d_idx = (long long*)c.ck_idx.p;
     long long* d_cnt = d_idx + N;
-    CK(pn_launch_check_select(N, fraction, key[0], key[1], d_idx, d_cnt, g_ck_tmp.p, tb, s));
+    CK(pn_launch_check_select(N, fraction, key[0], key[1], d_idx, d_cnt, c.ck_tmp.p, s));
     long long m = 0;
     CK(cudaMemcpyAsync(&m, d_cnt, sizeof m, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -458,8 +488,8 @@ extern "C" int pn_selfcheck(const double* init_states, const double* masses, con
     }
     if (m == 0) { CK(cudaStreamSynchronize(s)); return PN_OK; }
     // 2. gather + FP64 reference integration of the subset (the library's own integrator)
-    if ((rc = g_ck_sub.ensure(sizeof(double) * 23 * (size_t)m + sizeof(int) * (size_t)m)) != PN_OK) return rc;
-    double* sub_init = (double*)g_ck_sub.p;
+    if ((rc = c.ck_sub.ensure(sizeof(double) * 23 * (size_t)m + sizeof(int) * (size_t)m)) != PN_OK) return rc;
+    double* sub_init = (double*)c.ck_sub.p;
     double* sub_fin = sub_init + 10 * m;
     double* sub_m = sub_fin + 10 * m;
     double* sub_t = sub_m + 2 * m;
@@ -473,10 +503,10 @@ extern "C" int pn_selfcheck(const double* init_states, const double* masses, con
     if (st == PN_ECUDA) return st;
     out->ms_reference = g_ms[1];
     // 3. comparison
-    if ((rc = g_ck_out.ensure(64)) != PN_OK) return rc;
-    CK(pn_launch_check_compare(d_idx, m, d_fin, d_t, sub_fin, sub_t, sub_steps, (double*)g_ck_out.p, s));
+    if ((rc = c.ck_out.ensure(64)) != PN_OK) return rc;
+    CK(pn_launch_check_compare(d_idx, m, d_fin, d_t, sub_fin, sub_t, sub_steps, (double*)c.ck_out.p, s));
     double h[8];
-    CK(cudaMemcpyAsync(h, g_ck_out.p, sizeof h, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(h, c.ck_out.p, sizeof h, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
     long long hi[8];
@@ -493,12 +523,15 @@ extern "C" int pn_stream_status(void* stream)
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
     int st = PN_OK;
-    if (g_small.p && g_stream_status.count(stream)) {
+    auto it = g_ctx.find(stream);
+    if (it != g_ctx.end() && it->second->async_pending) {
+        Ctx& c = *it->second;
         Small hs;
-        CK(cudaMemcpy(&hs, g_small.p, sizeof hs, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(&st, c.sticky.p, sizeof st, cudaMemcpyDeviceToHost));      // worst status since the last collection
+        CK(cudaMemcpy(&hs, c.small.p, sizeof hs, cudaMemcpyDeviceToHost));       // counters of the LAST call on the stream
         memcpy(g_counters, hs.counters, sizeof g_counters);
-        st = hs.status;
-        g_stream_status.erase(stream);
+        g_redo_count = hs.redo_count;
+        c.async_pending = false;
     }
     return st;
 }
@@ -557,10 +590,15 @@ extern "C" const char* pn_last_cuda_error(void) { return g_last_err.c_str(); }
 extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
-    Buf* all[] = {&g_soa_in, &g_soa_m, &g_soa_out, &g_small, &g_redo, &g_seed, &g_sort_keys, &g_sort_idx, &g_sort_tmp, &g_h_init, &g_h_m, &g_h_final, &g_h_steps, &g_h_time, &g_h_rej, &g_h_counts, &g_st_scratch, &g_st_in, &g_st_out, &g_gen_specs, &g_gen_y, &g_gen_m, &g_ck_idx, &g_ck_tmp, &g_ck_sub, &g_ck_out, &g_ck_in};
-    for (Buf* b : all) if (b->release() != PN_OK) rc = PN_ECUDA;
-    if (g_ev_ok) { for (int i = 0; i < 5; ++i) cudaEventDestroy(g_ev[i]); g_ev_ok = false; }
-    g_stream_status.clear();
+    if (cudaDeviceSynchronize() != cudaSuccess) rc = PN_ECUDA;
+    for (auto& kv : g_ctx) {
+        Ctx* c = kv.second;
+        for (Buf* b : c->all) if (b->release() != PN_OK) rc = PN_ECUDA;
+        if (c->ev_ok) for (int i = 0; i < 5; ++i) cudaEventDestroy(c->ev[i]);
+        delete c;
+    }
+    g_ctx.clear();
+    g_next_slot = 0;
     return rc;
 }
 

@@ -1,7 +1,7 @@
 // pn_aux.cu -- staging (AoS <-> SoA), dot-product histogram and FMA-peak kernels of libpn_b200.
 #include <cstdint>
-#include <cub/device/device_radix_sort.cuh>
 #include "pn_internal.h"
+#include "pn_dots.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // AoS [n][W]  <->  SoA [W][n], coalesced on both sides through a shared-memory tile (stage-in /
@@ -50,12 +50,6 @@ cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int widt
 // population count to a per-block shared-memory histogram; blocks flush with one 64-bit global atomic
 // per non-empty bin.  HBM-bound: 80 B read per system.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int pn_bin_of(double d, int bins)
-{
-    int b = (int)floor((d + 1.0) * (double)bins * 0.5);
-    return max(0, min(bins - 1, b));
-}
-
 template <bool SOA, bool SMEM_HIST>
 __global__ void __launch_bounds__(PN_TILE) pn_histogram_kernel(const double* __restrict__ st, long long n, int bins,
                                                                unsigned long long* __restrict__ counts,
@@ -89,18 +83,11 @@ __global__ void __launch_bounds__(PN_TILE) pn_histogram_kernel(const double* __r
         }
         int bin[3] = {-1, -1, -1};
         if (have) {
-            const double n1 = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-            const double n2 = sqrt(v[3] * v[3] + v[4] * v[4] + v[5] * v[5]);
-            const double nl = sqrt(v[6] * v[6] + v[7] * v[7] + v[8] * v[8]);
-            const double d[3] = {(v[0] * v[3] + v[1] * v[4] + v[2] * v[5]) / (n1 * n2),
-                                 (v[0] * v[6] + v[1] * v[7] + v[2] * v[8]) / (n1 * nl),
-                                 (v[3] * v[6] + v[4] * v[7] + v[5] * v[8]) / (n2 * nl)};
-            const bool ok[3] = {n1 > 0 && n2 > 0, n1 > 0 && nl > 0, n2 > 0 && nl > 0};
+            double d[3];
+            bool ok[3];
+            pn_unit_dots(v, d, ok);
 #pragma unroll
-            for (int hh = 0; hh < 3; ++hh) {
-                if (ok[hh] && isfinite(d[hh])) bin[hh] = pn_bin_of(d[hh], bins);
-                else bin[hh] = -2;   // skipped
-            }
+            for (int hh = 0; hh < 3; ++hh) bin[hh] = ok[hh] ? pn_bin_of(d[hh], bins) : -2;      // -2: skipped
         }
 #pragma unroll
         for (int hh = 0; hh < 3; ++hh) {
@@ -154,46 +141,126 @@ cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long 
 }
 
 // ------------------------------------------------------------------------------------------------
-// Queue ordering by expected cost (default; pn_options.input_order turns it off).  The number of trial steps of
-// an inspiral follows the number of precession cycles of the faster-precessing body,
-//     key = (4 + 3 m_big/m_small)/eta * (1/(M omega_0) - 1/(M omega_f))        (Eq. (4) over Eq. (1), leading order)
-// (log-correlation 0.98 with the measured step counts on C3 and C5).  Issuing the queue longest-first
-// (LPT) shortens the drain tail of the persistent grid; results do not depend on the order.
+// Queue ordering by expected cost (default; pn_options.input_order turns it off).  The seed kernel
+// writes key[i] (expected number of precession cycles, log-correlation 0.98 with the measured step counts on C3
+// and C5) and the range of the keys; issuing the queue longest-first (LPT) shortens the drain tail of the
+// persistent grid.  An LPT order only needs to be approximate, so it is a ONE-pass bucket sort on
+// PN_ORDER_BUCKETS equal-width buckets of [kmin, kmax], bucket 0 holding the largest keys:
+//   count (shared-memory histogram per block, one global add per non-empty bucket) ->
+//   exclusive scan of the 2048 counts (one block) ->
+//   scatter (rank inside the block from a shared-memory atomic, one global add per block and bucket reserves the
+//   block's range, then order[base + rank] = i).
+// Systems inside a bucket land in block-arrival order: the ORDER may differ from run to run, the results cannot
+// (every system's result is independent of its queue position; tested bit for bit).
 // ------------------------------------------------------------------------------------------------
-__global__ void pn_cost_key_kernel(const double* __restrict__ y0, const double* __restrict__ masses, int n,
-                                   double omegaf, float* __restrict__ keys, int* __restrict__ idx)
+#define PN_ORD_THREADS 256
+#define PN_ORD_ITEMS 8       /* systems per thread */
+__device__ __forceinline__ int pn_order_bucket(float key, float kmax, float scale)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double m1 = masses[i], m2 = masses[(size_t)n + i], M = m1 + m2;
-    const double eta = m1 * m2 / (M * M);
-    const double big = fmax(m1, m2), small = fmin(m1, m2);
-    double key = (4.0 + 3.0 * big / small) / eta * (1.0 / (M * y0[i]) - 1.0 / (M * omegaf));
-    if (!(key > 0.0) || !isfinite(key)) key = 0.0;      // bad inputs go last; they are rejected at refill
-    keys[i] = (float)key;
-    idx[i] = i;
+    const int b = (int)((kmax - key) * scale);
+    return max(0, min(PN_ORDER_BUCKETS - 1, b));
+}
+__device__ __forceinline__ void pn_order_range(const unsigned* scratch, float& kmax, float& scale)
+{
+    const unsigned lo = scratch[PN_ORDER_BUCKETS], hi = scratch[PN_ORDER_BUCKETS + 1];
+    const float kmin = lo == 0xffffffffu ? 0.0f : __uint_as_float(lo);
+    kmax = __uint_as_float(hi);
+    scale = kmax > kmin ? (float)(PN_ORDER_BUCKETS - 1) / (kmax - kmin) : 0.0f;     // all keys equal: one bucket
 }
 
-size_t pn_cost_order_temp_bytes(int n)
+__global__ void __launch_bounds__(PN_ORD_THREADS) pn_order_count_kernel(const float* __restrict__ keys, int n, unsigned* __restrict__ scratch)
 {
-    size_t bytes = 0;
-    cub::DeviceRadixSort::SortPairsDescending(nullptr, bytes, (const float*)nullptr, (float*)nullptr,
-                                              (const int*)nullptr, (int*)nullptr, n);
-    return bytes;
+    __shared__ unsigned cnt[PN_ORDER_BUCKETS];
+    for (int b = threadIdx.x; b < PN_ORDER_BUCKETS; b += PN_ORD_THREADS) cnt[b] = 0u;
+    float kmax, scale;
+    pn_order_range(scratch, kmax, scale);
+    __syncthreads();
+    const int base = blockIdx.x * (PN_ORD_THREADS * PN_ORD_ITEMS);
+#pragma unroll
+    for (int k = 0; k < PN_ORD_ITEMS; ++k) {
+        const int i = base + k * PN_ORD_THREADS + threadIdx.x;
+        if (i < n) atomicAdd(&cnt[pn_order_bucket(keys[i], kmax, scale)], 1u);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < PN_ORDER_BUCKETS; b += PN_ORD_THREADS)
+        if (cnt[b]) atomicAdd(&scratch[b], cnt[b]);
 }
 
-cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys_in,
-                                 float* keys_out, int* idx_in, int* idx_out, void* temp, size_t temp_bytes,
-                                 cudaStream_t s)
+// exclusive scan of the PN_ORDER_BUCKETS counts in place: scratch[b] becomes the first queue position of bucket b
+__global__ void __launch_bounds__(1024) pn_order_scan_kernel(unsigned* __restrict__ scratch)
+{
+    __shared__ unsigned warp_tot[32];
+    constexpr int PER = PN_ORDER_BUCKETS / 1024;
+    unsigned v[PER], run = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { v[k] = scratch[threadIdx.x * PER + k]; run += v[k]; }
+    unsigned inc = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, inc, o); if ((threadIdx.x & 31) >= o) inc += t; }
+    if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = inc;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        unsigned w = warp_tot[threadIdx.x], wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned t = __shfl_up_sync(0xffffffffu, wi, o); if (threadIdx.x >= o) wi += t; }
+        warp_tot[threadIdx.x] = wi - w;
+    }
+    __syncthreads();
+    unsigned start = warp_tot[threadIdx.x >> 5] + inc - run;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { scratch[threadIdx.x * PER + k] = start; start += v[k]; }
+}
+
+__global__ void __launch_bounds__(PN_ORD_THREADS) pn_order_scatter_kernel(const float* __restrict__ keys, int n, unsigned* __restrict__ scratch,
+                                                                          int* __restrict__ order)
+{
+    __shared__ unsigned cnt[PN_ORDER_BUCKETS];       // systems of this block per bucket, then the block's first position in it
+    for (int b = threadIdx.x; b < PN_ORDER_BUCKETS; b += PN_ORD_THREADS) cnt[b] = 0u;
+    float kmax, scale;
+    pn_order_range(scratch, kmax, scale);
+    __syncthreads();
+    const int base = blockIdx.x * (PN_ORD_THREADS * PN_ORD_ITEMS);
+    int bucket[PN_ORD_ITEMS];
+    unsigned rank[PN_ORD_ITEMS];
+#pragma unroll
+    for (int k = 0; k < PN_ORD_ITEMS; ++k) {
+        const int i = base + k * PN_ORD_THREADS + threadIdx.x;
+        bucket[k] = i < n ? pn_order_bucket(keys[i], kmax, scale) : -1;
+        rank[k] = bucket[k] >= 0 ? atomicAdd(&cnt[bucket[k]], 1u) : 0u;
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < PN_ORDER_BUCKETS; b += PN_ORD_THREADS)
+        if (cnt[b]) cnt[b] = atomicAdd(&scratch[b], cnt[b]);
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < PN_ORD_ITEMS; ++k)
+        if (bucket[k] >= 0) order[cnt[bucket[k]] + rank[k]] = base + k * PN_ORD_THREADS + threadIdx.x;
+}
+
+__global__ void pn_fold_status_kernel(const int* __restrict__ status, int* __restrict__ sticky) { if (*status > *sticky) *sticky = *status; }
+cudaError_t pn_launch_fold_status(const int* status, int* sticky, cudaStream_t s)
+{
+    pn_fold_status_kernel<<<1, 1, 0, s>>>(status, sticky);
+    ++g_pn_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t pn_launch_order_init(unsigned int* scratch, cudaStream_t s)
+{
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(scratch, 0, sizeof(unsigned) * (PN_ORDER_BUCKETS + 2), s)) != cudaSuccess) return e;
+    return cudaMemsetAsync(scratch + PN_ORDER_BUCKETS, 0xff, sizeof(unsigned), s);      // running minimum starts at 0xffffffff
+}
+
+cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch, int* order, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
-    pn_cost_key_kernel<<<(n + 255) / 256, 256, 0, s>>>(y0_soa, m_soa, n, omegaf, keys_in, idx_in);
-    ++g_pn_launches;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    e = cub::DeviceRadixSort::SortPairsDescending(temp, temp_bytes, keys_in, keys_out, idx_in, idx_out, n, 0, 32, s);
-    g_pn_launches += 3;   // cub's histogram + onesweep passes (library kernels, counted approximately)
-    return e;
+    const int per = PN_ORD_THREADS * PN_ORD_ITEMS, grid = (n + per - 1) / per;
+    pn_order_count_kernel<<<grid, PN_ORD_THREADS, 0, s>>>(keys, n, scratch);
+    pn_order_scan_kernel<<<1, 1024, 0, s>>>(scratch);
+    pn_order_scatter_kernel<<<grid, PN_ORD_THREADS, 0, s>>>(keys, n, scratch, order);
+    g_pn_launches += 3;
+    return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -202,9 +269,13 @@ cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int 
 // the ALU roofline at the clocks the device actually holds.  MODE 1: a = a*x + U (two
 // distinct register sources).  MODE 2: a = a*x + z (three distinct register sources).  On sm_100a a DFMA
 // issues every 2 cycles per scheduler with <= 2 register sources and every 3 cycles with 3.
+// Clock: every block measures its own clock64() span and the LONGEST span is kept (atomicMax).  Co-resident
+// blocks are not served evenly: the warp arbiter runs the blocks of an SM almost one after the other (measured:
+// with 4 resident blocks the first finishes after 1/4 of the kernel's duration, the last spans all of it), so
+// the span of one fixed block is not the duration of the kernel -- r1 read block 0's and got 1/4 of the SM clock.
 // ------------------------------------------------------------------------------------------------
 template <typename real, int CHAINS, int MODE>
-__global__ void __launch_bounds__(256) pn_fma_peak_kernel(real* out, int iters, long long* clocks, real m, real b)
+__global__ void __launch_bounds__(256) pn_fma_peak_kernel(real* out, int iters, unsigned long long* clocks, real m, real b)
 {
     real a[CHAINS], x[CHAINS], z[CHAINS];
 #pragma unroll
@@ -229,7 +300,7 @@ __global__ void __launch_bounds__(256) pn_fma_peak_kernel(real* out, int iters, 
 #pragma unroll
     for (int i = 0; i < CHAINS; ++i) s += a[i];
     if (s == (real)123.456) out[0] = s;
-    if (blockIdx.x == 0 && threadIdx.x == 0) clocks[0] = c1 - c0;
+    if (threadIdx.x == 0) atomicMax(clocks, (unsigned long long)(c1 - c0));
 }
 
 cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
@@ -240,15 +311,26 @@ cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tfl
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     void* scratch = nullptr;
-    long long* dclk = nullptr;
+    unsigned long long* dclk = nullptr;
     cudaError_t e;
     if ((e = cudaMalloc(&scratch, 64)) != cudaSuccess) return e;
     if ((e = cudaMemset(scratch, 0, 64)) != cudaSuccess) { cudaFree(scratch); return e; }
-    if ((e = cudaMalloc((void**)&dclk, sizeof(long long))) != cudaSuccess) { cudaFree(scratch); return e; }
+    if ((e = cudaMalloc((void**)&dclk, sizeof(unsigned long long))) != cudaSuccess) { cudaFree(scratch); return e; }
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const int block = 256, grid = sms * 4;      // 4 resident blocks per SM = 8 warps per scheduler, one wave
+    // 4 resident blocks of 8 warps per SM = 8 warps per scheduler, one wave; checked against the occupancy the
+    // runtime reports for this instantiation (fewer resident blocks -> a smaller grid, still one wave)
+    const int block = 256;
+    int occ = 0;
+#define PN_PEAK_OCC(T, M) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pn_fma_peak_kernel<T, CH, M>, block, 0)
+    if (precision == 0) { if (mode == 0) PN_PEAK_OCC(double, 0); else if (mode == 1) PN_PEAK_OCC(double, 1); else PN_PEAK_OCC(double, 2); }
+    else { if (mode == 0) PN_PEAK_OCC(float, 0); else if (mode == 1) PN_PEAK_OCC(float, 1); else PN_PEAK_OCC(float, 2); }
+#undef PN_PEAK_OCC
+    const int resident = occ >= 4 ? 4 : (occ >= 1 ? occ : 1);
+    const int grid = sms * resident;
+    const double warps_per_scheduler = resident * (block / 32) / 4.0;
     auto run = [&](int iters, float* ms) {
+        cudaMemsetAsync(dclk, 0, sizeof(unsigned long long));
         cudaEventRecord(e0);
 #define PN_PEAK(T, M) pn_fma_peak_kernel<T, CH, M><<<grid, block>>>((T*)scratch, iters, dclk, (T)0.999999, (T)1e-7)
         if (precision == 0) { if (mode == 0) PN_PEAK(double, 0); else if (mode == 1) PN_PEAK(double, 1); else PN_PEAK(double, 2); }
@@ -273,11 +355,11 @@ cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tfl
         if (e == cudaSuccess) {
             const double fl = 2.0 * 8.0 * CH * (double)iters * (double)grid * block;
             if (tflops) *tflops = fl / (ms * 1e-3) / 1e12;
-            long long clk = 0;
+            unsigned long long clk = 0;
             cudaMemcpy(&clk, dclk, sizeof clk, cudaMemcpyDeviceToHost);
             if (sm_mhz) *sm_mhz = (double)clk / (ms * 1e-3) / 1e6;
-            // warp instructions per scheduler = iters*8*CH per warp x 8 warps per scheduler
-            if (cycles_per_warp_inst) *cycles_per_warp_inst = (double)clk / ((double)iters * 8.0 * CH * 8.0);
+            // warp instructions per scheduler = iters*8*CH per warp x resident warps per scheduler
+            if (cycles_per_warp_inst) *cycles_per_warp_inst = (double)clk / ((double)iters * 8.0 * CH * warps_per_scheduler);
         }
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);

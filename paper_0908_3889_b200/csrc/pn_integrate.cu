@@ -7,8 +7,7 @@
 // cost only the short refill section.  All state (y, k1..k7, per-system constants) lives in
 // registers; global memory is touched only at refill and at finish.  (DESIGN.md 2, 7.)
 #include <cfloat>
-#include <cstdlib>
-#include "pn_dp5_smem.cuh"
+#include "pn_dp5.cuh"
 #include "pn_internal.h"
 
 #define PN_ST_EINVAL 1
@@ -115,21 +114,44 @@ template <typename real>
 __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
 {
     const int i = blockIdx.x * 128 + threadIdx.x;
-    if (i >= p.n) return;
+    const bool in = i < p.n;
+    const int ii = in ? i : p.n - 1;            // out-of-range threads shadow the last system up to the key reduction
     double y0[10];
 #pragma unroll
-    for (int j = 0; j < 10; ++j) y0[j] = p.y0[(size_t)j * p.n + i];
-    const double m1 = p.masses[i], m2 = p.masses[(size_t)p.n + i];
+    for (int j = 0; j < 10; ++j) y0[j] = p.y0[(size_t)j * p.n + ii];
+    const double m1 = p.masses[ii], m2 = p.masses[(size_t)p.n + ii];
+    const bool bad_input = !(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
+                           (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0));
+    if (p.keys) {
+        // expected cost: the number of precession cycles of the faster-precessing body,
+        //   key = (4 + 3 m_big/m_small)/eta (1/(M omega_0) - 1/(M omega_f))      (Eq. (4) over Eq. (1) at leading order);
+        // the bucket sort that follows issues the queue longest-expected-first.  Positive floats order like their bit
+        // patterns, so the range of the keys is found with integer atomics: one pair per warp.  Bad inputs get key 0
+        // (last in the queue; the refill skips them) and stay out of the range.
+        const double M = m1 + m2, eta = m1 * m2 / (M * M);
+        double key = (4.0 + 3.0 * fmax(m1, m2) / fmin(m1, m2)) / eta * (1.0 / (M * y0[0]) - 1.0 / (M * p.omegaf));
+        const bool key_ok = !bad_input && key > 0.0 && key < 3e38;
+        const float kf = key_ok ? (float)key : 0.0f;
+        if (in) p.keys[i] = kf;
+        const unsigned kb = __float_as_uint(kf);
+        const unsigned lo = __reduce_min_sync(0xffffffffu, key_ok ? kb : 0xffffffffu);
+        const unsigned hi = __reduce_max_sync(0xffffffffu, key_ok ? kb : 0u);
+        if ((threadIdx.x & 31) == 0) {
+            if (lo != 0xffffffffu) atomicMin(p.order_scratch + PN_ORDER_BUCKETS, lo);
+            if (hi != 0u) atomicMax(p.order_scratch + PN_ORDER_BUCKETS + 1, hi);
+        }
+    }
+    if (!in) return;
     real* rec = (real*)p.seed + (size_t)i * PN_REC;
     real y[10], k1[10];
 #pragma unroll
     for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
-    if (!(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
-        (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0))) {
+    if (bad_input) {
         pn_store_result(p, i, y, PN_F_BADINPUT, 0.0, 0);
         atomicMax(p.status, PN_ST_EINVAL);
         atomicAdd(p.counters + 3, 1ull);
         rec[38] = (real)-1;
+        if (i == 0) *p.nonuniform = 1;          // the uniform-mass kernel takes its constants from system 0's record
         return;
     }
     if (m1 != p.masses[0] || m2 != p.masses[p.n]) *p.nonuniform = 1;      // benign race: every writer stores 1
@@ -175,26 +197,30 @@ __device__ __forceinline__ void pn_load_record(const void* seed, int i, real (&o
     for (int j = 0; j < PN_REC / W; ++j) PnVec<real>::unpack(__ldg(src + j), &out[j * W]);
 }
 
-// SMEM = true (FP64 only): k2..k5 and the error partial live in dynamic shared memory (pn_dp5_smem.cuh)
 // SLOW = true: the redo pass.  Systems whose step left the range of the cbrt/log series in the fast kernel
 // are re-integrated from their initial state with the wide-range evaluation (pn_rhs.cuh) in every stage.
 // MIXED = true (real = float only; PN_MIXED): slopes, RHS, stage sums and error norm in float, but the
 // state itself is carried in double: an accepted step adds the float increment dy = sum b_s K_s to the double copy,
 // so the per-step rounding error is eps32 |dy| instead of eps32 |y| ("only a few critical computations in
 // double"); omega is compared with omega_f in double.
-// UNI = true (FP64): every system of the batch has the masses of system 0 (checked by the seed kernel), so the 15
-// mass-dependent constants are kernel parameters: constant-bank operands instead of per-lane registers.
-template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false, bool UNI = false>
+// UNI >= 0 (FP64): every system of the batch has the masses of system 0 (checked by the seed kernel), so the 15
+// mass-dependent constants come from row UNI of a __constant__ table (uniform-register operands instead of per-lane
+// registers; the row must be a compile-time constant for that, a run-time row index makes ptxas load the values into
+// per-lane registers again, so there is one instantiation per row and one row per stream context, PN_UNI_SLOTS in all).
+// The launcher copies system 0's record into the row on the stream and launches BOTH the uniform-mass and the generic
+// kernel (p.uni_slot >= 0 marks such a pair); each looks at the seed kernel's verdict and the one that does not apply
+// returns at once, so no host synchronisation is needed and async calls keep the fast path.
+__constant__ double pn_uni_table[PN_UNI_SLOTS][16];
+template <typename real, int BLOCK, int MINB, bool SLOW, bool MIXED = false, int UNI = -1>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
 {
+    if (UNI >= 0) { if (*p.nonuniform != 0) return; }
+    else if (!SLOW && p.uni_slot >= 0) { if (*p.nonuniform == 0) return; }
     const unsigned n_queue = SLOW ? *p.redo_count : (unsigned)p.n;     // length of the work queue
     const int* order = SLOW ? p.redo_list : p.order;
     if (SLOW && n_queue == 0u) return;
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    extern __shared__ double pn_dyn_smem[];
-    PnSmem<BLOCK> sm;
-    sm.addr = SMEM ? (unsigned)__cvta_generic_to_shared(pn_dyn_smem) + threadIdx.x * 8u : 0u;
 
     // lane state.  k1 holds the SCALED slope h*f(y).  Idle lanes are frozen (h = 0, k1 = 0) on a benign
     // dummy state, so the lock-step arithmetic stays finite and never leaves the series' range.
@@ -206,10 +232,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     pn_make_uni<real>(p.mask, u);
     u.emax = (real)p.emax;
     pn_make_consts<real>(0.5, 0.5, 0u, c);
-    if constexpr (UNI) {
-        c.M = (real)p.uc[0]; c.c2 = (real)p.uc[1]; c.c4 = (real)p.uc[2]; c.c5 = (real)p.uc[3]; c.c6 = (real)p.uc[4]; c.c7 = (real)p.uc[5];
-        c.p1 = (real)p.uc[6]; c.p2 = (real)p.uc[7]; c.q1 = (real)p.uc[8]; c.q2 = (real)p.uc[9]; c.K0 = (real)p.uc[10];
-        c.A1 = (real)p.uc[11]; c.A2 = (real)p.uc[12]; c.Bc = (real)p.uc[13]; c.G = (real)p.uc[14];
+    if constexpr (UNI >= 0) {
+        const double* uc = pn_uni_table[UNI];
+        c.M = (real)uc[0]; c.c2 = (real)uc[1]; c.c4 = (real)uc[2]; c.c5 = (real)uc[3]; c.c6 = (real)uc[4]; c.c7 = (real)uc[5];
+        c.p1 = (real)uc[6]; c.p2 = (real)uc[7]; c.q1 = (real)uc[8]; c.q2 = (real)uc[9]; c.K0 = (real)uc[10];
+        c.A1 = (real)uc[11]; c.A2 = (real)uc[12]; c.Bc = (real)uc[13]; c.G = (real)uc[14];
     }
 #pragma unroll
     for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; yd[i] = 0.0; }
@@ -252,7 +279,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                         if constexpr (MIXED)
 #pragma unroll
                             for (int j = 0; j < 10; ++j) yd[j] = __ldg(p.y0 + (size_t)j * p.n + i);
-                        if constexpr (!UNI) {
+                        if constexpr (UNI < 0) {
                             c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
                             c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
                             c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
@@ -275,8 +302,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         real ynew[10], k7[10], err[10], dy[10];
         PnBase<real> base_new;
         bool bad = false;
-        if constexpr (SMEM) pn_dp5_trial_smem<SLOW, BLOCK>(y, k1, h, c, u, base, sm, ynew, k7, err, base_new, bad);
-        else if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad, dy);
+        if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad, dy);
         else pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
         // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|), E^2 = mean (err_j/sc_j)^2.
         // It only decides accept/reject and the next step size, so ~1e-6 relative accuracy is ample:
@@ -284,6 +310,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         // MUFU seed (rcp.approx.ftz.f64, ~2^-23, no Newton step): 3 FP64 instructions per component and no
         // F64<->F32 conversions (which issue at 1/8 rate and put a long serial tail at the end of the step).
         float E2 = pn_err_norm2(y, ynew, err, rtol, atol1, atS1, atS2);
+        // a huge but finite error ratio (atol = 0 and a tiny scale) overflows the float to +inf: that is a rejection with
+        // the smallest step factor, not a non-finite state; only NaN is reported as PN_FAIL_NONFINITE
+        E2 = (E2 > FLT_MAX) ? 1e30f : E2;
         // `bad`: a stage of this trial left the range of the cbrt/log series (|1 - x/x0| > emax; only at loose
         // tolerances).  Fast kernel: if the trial fails error control anyway (the usual case: an overshoot while the
         // step size ramps up) it is an ordinary rejection (the estimate is inaccurate there, but it only sets the step-size
@@ -447,33 +476,33 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
 
 unsigned long long g_pn_launches = 0;
 
-template <typename real, int BLOCK, int MINB, bool SMEM, bool SLOW, bool MIXED = false, bool UNI = false>
+template <typename real, int BLOCK, int MINB, bool SLOW, bool MIXED = false, int UNI = -1>
 static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
-    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SMEM, SLOW, MIXED, UNI>;
-    const int shm = SMEM ? PN_SM_SLOTS * BLOCK * (int)sizeof(double) : 0;
-    int dev = 0, sms = 0, per_sm = 0;
+    auto kern = pn_integrate_adaptive_kernel<real, BLOCK, MINB, SLOW, MIXED, UNI>;
+    // SMs x resident blocks, looked up once per (kernel, device): the occupancy query is a host-side call per launch otherwise
+    static int grid_full[64] = {0};
+    int dev = 0;
     cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if (SMEM) {
-        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, shm)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                      cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
+    int& gf = grid_full[dev & 63];
+    if (gf == 0) {
+        int sms = 0, per_sm = 0;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BLOCK, 0)) != cudaSuccess) return e;
+        gf = sms * (per_sm < 1 ? 1 : per_sm);
     }
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BLOCK, shm)) != cudaSuccess) return e;
-    if (per_sm < 1) per_sm = 1;
-    int grid = grid_blocks > 0 ? grid_blocks : sms * per_sm;
+    int grid = grid_blocks > 0 ? grid_blocks : gf;
     const long long need = ((long long)p.n + BLOCK - 1) / BLOCK;
     if (need < grid) grid = (int)need;
     if (grid < 1) grid = 1;
-    kern<<<grid, BLOCK, shm, s>>>(p);
+    kern<<<grid, BLOCK, 0, s>>>(p);
     ++g_pn_launches;
     return cudaGetLastError();
 }
 
 cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
-                                cudaStream_t s, bool may_sync)
+                                cudaStream_t s, int variant)
 {
     if (p.n <= 0) return cudaSuccess;
     if (p.fixed_steps > 0) {
@@ -489,42 +518,44 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
         ++g_pn_launches;
         return cudaGetLastError();
     }
+    cudaError_t e;
     {
-        // stage-in: per-system seed records (constants, base powers, K1 = h0 f(y0)); bad inputs fail here
+        // stage-in: per-system seed records (constants, base powers, K1 = h0 f(y0)), expected-cost keys; bad inputs fail here
         const int grid = (p.n + 127) / 128;
+        if (p.keys && (e = pn_launch_order_init(p.order_scratch, s)) != cudaSuccess) return e;
         if (precision == 0) pn_seed_kernel<double><<<grid, 128, 0, s>>>(p);
         else pn_seed_kernel<float><<<grid, 128, 0, s>>>(p);
         ++g_pn_launches;
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        // queue order: longest expected first
+        if (p.keys && (e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s)) != cudaSuccess) return e;
     }
+    const int slot = (precision == 0 && block_threads != 256 && !(variant & 1)) ? p.uni_slot : -1;
+    p.uni_slot = -1;                 // >= 0 only for the kernel pair below
     if (precision == 0) {
-        cudaError_t e;
-        const char* v = getenv("PN_DEV_VARIANT");   // development switch, not part of the ABI
-        if (block_threads == 256) e = launch_adaptive<double, 256, 1, false, false>(p, grid_blocks, s);
-        else if (v && v[0] == 's') e = launch_adaptive<double, 128, 3, true, false>(p, grid_blocks, s);
+        if (block_threads == 256) e = launch_adaptive<double, 256, 1, false>(p, grid_blocks, s);
+        else if (slot < 0) e = launch_adaptive<double, 128, 2, false>(p, grid_blocks, s);
         else {
-            // uniform-mass fast path: needs the seed kernel's verdict on the host (one small copy + sync, ~10 us)
-            bool uni = false;
-            if (may_sync && !getenv("PN_NO_UNIFORM")) {
-                int flag = 1;
-                double rec0[PN_REC];          // the constants come from system 0's seed record: bitwise what the generic path uses
-                if ((e = cudaMemcpyAsync(&flag, p.nonuniform, sizeof flag, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return e;
-                if ((e = cudaMemcpyAsync(rec0, p.seed, sizeof rec0, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return e;
-                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return e;
-                if (flag == 0 && rec0[38] >= 0.0) {
-                    for (int k = 0; k < 15; ++k) p.uc[k] = rec0[20 + k];
-                    uni = true;
-                }
-            }
-            if (uni) e = launch_adaptive<double, 128, 2, false, false, false, true>(p, grid_blocks, s);
-            else e = launch_adaptive<double, 128, 2, false, false>(p, grid_blocks, s);
+            p.uni_slot = slot;
+            // uniform-mass fast path, decided on the device: system 0's constants (bitwise those of its seed record) go
+            // into the __constant__ table on the stream, then both kernels of the pair are launched
+            if ((e = cudaMemcpyToSymbolAsync(pn_uni_table, (const double*)p.seed + 20, 15 * sizeof(double),
+                                             (size_t)p.uni_slot * 16 * sizeof(double), cudaMemcpyDeviceToDevice, s)) != cudaSuccess)
+                return e;
+            static_assert(PN_UNI_SLOTS == 4, "one instantiation of the uniform-mass kernel per table row");
+            if (slot == 0) e = launch_adaptive<double, 128, 2, false, false, 0>(p, grid_blocks, s);
+            else if (slot == 1) e = launch_adaptive<double, 128, 2, false, false, 1>(p, grid_blocks, s);
+            else if (slot == 2) e = launch_adaptive<double, 128, 2, false, false, 2>(p, grid_blocks, s);
+            else e = launch_adaptive<double, 128, 2, false, false, 3>(p, grid_blocks, s);
+            if (e != cudaSuccess) return e;
+            e = launch_adaptive<double, 128, 2, false>(p, grid_blocks, s);
+            p.uni_slot = -1;
         }
         if (e != cudaSuccess) return e;
         // redo pass for systems that left the series' range; its queue length is read on the device
-        return launch_adaptive<double, 128, 2, false, true>(p, grid_blocks, s);
+        return launch_adaptive<double, 128, 2, true>(p, grid_blocks, s);
     }
-    if (precision == 2) return launch_adaptive<float, 128, 3, false, false, true>(p, grid_blocks, s);   // PN_MIXED
-    if (block_threads == 128) return launch_adaptive<float, 128, 4, false, false>(p, grid_blocks, s);
-    return launch_adaptive<float, 256, 2, false, false>(p, grid_blocks, s);
+    if (precision == 2) return launch_adaptive<float, 128, 3, false, true>(p, grid_blocks, s);   // PN_MIXED
+    if (block_threads == 128) return launch_adaptive<float, 128, 4, false>(p, grid_blocks, s);
+    return launch_adaptive<float, 256, 2, false>(p, grid_blocks, s);
 }

@@ -2,6 +2,9 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#define PN_ORDER_BUCKETS 2048
+#define PN_UNI_SLOTS 4
+
 // Arguments of the integrator kernels.  All arrays are DEVICE pointers in SoA layout with stride n:
 // y0[c*n + i], masses[j*n + i], yf[c*n + i].
 struct PnKernelParams {
@@ -26,23 +29,29 @@ struct PnKernelParams {
     unsigned int* redo_count;
     unsigned long long* counters;   // [0] trial steps [1] rejected [2] landing trials [3] failed systems
     int* status;                    // worst pn_status seen on the device (atomicMax)
-    int* nonuniform;                // set by the seed kernel if some system's masses differ from system 0's
-    double uc[15];                  // FP64 uniform-mass path: the PnConsts of (masses[0]) as kernel parameters (constant bank)
+    int* nonuniform;                // set by the seed kernel if some system's masses differ from system 0's (or system 0 is bad)
+    int uni_slot;                   // FP64 uniform-mass path: slot of the __constant__ table that holds system 0's PnConsts; < 0: off
+    float* keys;                    // [n] or null: expected-cost keys written by the seed kernel (queue ordering)
+    unsigned int* order_scratch;    // [PN_ORDER_BUCKETS + 2]: bucket cursors, then the bit patterns of the smallest / largest key
+    int* order_out;                 // [n]: the queue order the bucket sort writes (= order when keys != null)
 };
 
 // launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults
+// variant bits (pn_options.variant): 1 = always the generic FP64 kernel (per-lane constants), 2 = always the scalar FP32 kernel
 cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
-                                cudaStream_t s, bool may_sync);
+                                cudaStream_t s, int variant);
 // staging + histogram + peak (pn_aux.cu)
 cudaError_t pn_launch_aos_to_soa(const double* aos, double* soa, int n, int width, cudaStream_t s);
 cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int width, cudaStream_t s);
 cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long n, int bins,
                                 unsigned long long* counts /*[3][bins]*/, unsigned long long* skipped /*[3]*/,
                                 cudaStream_t s);
-size_t pn_cost_order_temp_bytes(int n);
-cudaError_t pn_launch_cost_order(const double* y0_soa, const double* m_soa, int n, double omegaf, float* keys_in,
-                                 float* keys_out, int* idx_in, int* idx_out, void* temp, size_t temp_bytes,
-                                 cudaStream_t s);
+// queue order, longest expected first (pn_aux.cu): bucket sort of the keys the seed kernel wrote.
+// scratch: PN_ORDER_BUCKETS + 2 unsigned: bucket cursors (0), then min / max key bits (0xffffffff / 0), set by the init call
+// async calls: *sticky = max(*sticky, *status), one thread (pn_api.cu folds a call's status into its stream's sticky word)
+cudaError_t pn_launch_fold_status(const int* status, int* sticky, cudaStream_t s);
+cudaError_t pn_launch_order_init(unsigned int* scratch, cudaStream_t s);
+cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch, int* order, cudaStream_t s);
 // ensemble statistics (pn_stats.cu)
 size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out);
 cudaError_t pn_launch_stats_merge(const double* parts, int n_parts, int n_groups, double* mom_out, double* r_out, cudaStream_t s);
@@ -57,7 +66,7 @@ cudaError_t pn_launch_generate(const void* specs_dev, int n_ens, long long n_tot
 // cross-check (pn_check.cu)
 size_t pn_check_select_temp_bytes(long long n);
 cudaError_t pn_launch_check_select(long long n, double fraction, unsigned long long k0, unsigned long long k1,
-                                   long long* indices, long long* n_selected, void* temp, size_t temp_bytes, cudaStream_t s);
+                                   long long* indices, long long* n_selected, void* temp, cudaStream_t s);
 cudaError_t pn_launch_check_gather(const long long* indices, long long m, const double* init, const double* masses,
                                    double* sub_init, double* sub_masses, cudaStream_t s);
 cudaError_t pn_launch_check_compare(const long long* indices, long long m, const double* fin, const double* times,

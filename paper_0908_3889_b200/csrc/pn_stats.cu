@@ -15,6 +15,7 @@
 // This file shares nothing with oracle/ (which evaluates the two-pass definitions in numpy).
 #include <cstdint>
 #include "pn_internal.h"
+#include "pn_dots.cuh"
 
 #define ST_TILE 256
 #define ST_STAGES 2      /* one ring slot per consumer group (see pn_stats_kernel) */
@@ -104,28 +105,13 @@ struct StAcc {
     }
 };
 
-// unit dot products of one AoS row; ok[k] false where a norm is zero or the quotient is not finite (R14)
+// unit dot products of one AoS row (the shared routine of pn_dots.cuh); ok[k] false where undefined (R14)
 __device__ __forceinline__ void st_unit_dots(const double* __restrict__ row, double (&d)[3], bool (&ok)[3])
 {
-    const double s1x = row[1], s1y = row[2], s1z = row[3], s2x = row[4], s2y = row[5], s2z = row[6];
-    const double lx = row[7], ly = row[8], lz = row[9];
-    const double a = fma(s1x, s1x, fma(s1y, s1y, s1z * s1z));
-    const double b = fma(s2x, s2x, fma(s2y, s2y, s2z * s2z));
-    const double c = fma(lx, lx, fma(ly, ly, lz * lz));
-    const double ra = rsqrt(a), rb = rsqrt(b), rc = rsqrt(c);
-    d[0] = fma(s1x, s2x, fma(s1y, s2y, s1z * s2z)) * ra * rb;
-    d[1] = fma(s1x, lx, fma(s1y, ly, s1z * lz)) * ra * rc;
-    d[2] = fma(s2x, lx, fma(s2y, ly, s2z * lz)) * rb * rc;
-    // a unit dot product cannot leave [-1, 1]; the three roundings above can overshoot by an ulp or two
-    ok[0] = a > 0.0 && b > 0.0 && isfinite(d[0]);
-    ok[1] = a > 0.0 && c > 0.0 && isfinite(d[1]);
-    ok[2] = b > 0.0 && c > 0.0 && isfinite(d[2]);
+    const double v[9] = {row[1], row[2], row[3], row[4], row[5], row[6], row[7], row[8], row[9]};
+    pn_unit_dots(v, d, ok);
 }
-__device__ __forceinline__ int st_bin(double d, int bins)
-{
-    const int b = (int)floor((d + 1.0) * (double)bins * 0.5);
-    return max(0, min(bins - 1, b));
-}
+__device__ __forceinline__ int st_bin(double d, int bins) { return pn_bin_of(d, bins); }
 
 struct StParams {
     const double* init;     // [N][10] or null (final-only mode: 1-D histograms and skipped counts only)

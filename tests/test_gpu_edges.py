@@ -180,16 +180,10 @@ def test_uniform_mass_fast_path_is_bit_identical(pn):
     """FP64 batches whose systems all have the masses of system 0 run a kernel that takes the 15 mass-dependent
     constants as kernel parameters.  Same constants, same arithmetic: the results are bit-identical to
     the generic kernel's; one deviating system anywhere in the batch switches the whole launch to the generic kernel."""
-    import os
-
     cfg = W.with_size(W.CONFIGS["C4"], 3000 + 17)
     y0, m = W.generate(cfg)
     a = gpu_integrate(pn, y0, m, cfg)
-    os.environ["PN_NO_UNIFORM"] = "1"
-    try:
-        b = gpu_integrate(pn, y0, m, cfg)
-    finally:
-        del os.environ["PN_NO_UNIFORM"]
+    b = gpu_integrate(pn, y0, m, cfg, variant=1)          # pn_options.variant bit 0: always the generic kernel
     for k in ("final", "steps", "time", "rejected"):
         assert np.array_equal(a[k], b[k]), k
     # a batch that is uniform except for its last system, and one whose system 0 is invalid
@@ -275,3 +269,63 @@ def test_fp64_at_loose_tolerances_full_batch(pn, oracle):
         assert err_g <= 3 * err_o + 1e-6, (tol, err_g, err_o)
         assert abs(g["steps"][idx].mean() / o["steps"].mean() - 1) < 0.1
         assert np.abs(g["time"][idx] / o["time"] - 1).max() < 50 * tol
+
+
+def test_async_calls_keep_their_status_and_scratch(pn):
+    """The async contract of include/pn.h: pn_stream_status returns the worst status of ALL async calls enqueued on the
+    stream since the last collection (a later call does not erase an earlier call's status), calls in flight on
+    different streams do not share scratch, and async calls keep the uniform-mass fast path (decided on the device)."""
+    dev = "cuda:0"
+    cfg3 = W.with_size(W.CONFIGS["C3"], 3000 + 5)
+    y3, m3 = W.generate(cfg3)
+    cfg4 = W.with_size(W.CONFIGS["C4"], 4000 + 3)
+    y4, m4 = W.generate(cfg4)
+    ref3 = gpu_integrate(pn, y3, m3, cfg3)
+    ref4 = gpu_integrate(pn, y4, m4, cfg4)
+    ref4g = gpu_integrate(pn, y4, m4, cfg4, variant=1)
+    assert np.array_equal(ref4["final"], ref4g["final"])
+
+    def bufs(n):
+        return (torch.full((n, 10), float("nan"), dtype=torch.float64, device=dev), torch.zeros(n, dtype=torch.int32, device=dev))
+
+    m3_bad = m3.copy(); m3_bad[3, 1] = -0.5
+    d_y3, d_m3, d_m3b = (torch.from_numpy(a).to(dev) for a in (y3, m3, m3_bad))
+    d_y4, d_m4 = torch.from_numpy(y4).to(dev), torch.from_numpy(m4).to(dev)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    # (a) two calls back to back on ONE stream, the first with a bad-mass system
+    f1, st1 = bufs(cfg3.n); f2, st2 = bufs(cfg3.n)
+    assert pn.pn_integrate(d_y3, d_m3b, 0.0, cfg3.omegaf, cfg3.rtol, cfg3.atol, 0, f1, st1, stream=s1, async_=True) == 0
+    assert pn.pn_integrate(d_y3, d_m3, 0.0, cfg3.omegaf, cfg3.rtol, cfg3.atol, 0, f2, st2, stream=s1, async_=True) == 0
+    assert pn.pn_stream_status(s1) == 1                     # PN_EINVAL of the FIRST call survives the second
+    assert pn.pn_stream_status(s1) == 0                     # collected: cleared
+    good = np.ones(cfg3.n, bool); good[3] = False
+    assert st1.cpu().numpy()[3] == -5
+    assert np.array_equal(f1.cpu().numpy()[good], ref3["final"][good]) and np.array_equal(st1.cpu().numpy()[good], ref3["steps"][good])
+    assert np.array_equal(f2.cpu().numpy(), ref3["final"]) and np.array_equal(st2.cpu().numpy(), ref3["steps"])
+    # (b) two calls in flight on DIFFERENT streams (mixed-mass batch on one, uniform-mass batch on the other), twice
+    for _ in range(2):
+        fa, sa = bufs(cfg3.n); fb, sb = bufs(cfg4.n)
+        pn.pn_integrate(d_y3, d_m3, 0.0, cfg3.omegaf, cfg3.rtol, cfg3.atol, 0, fa, sa, stream=s1, async_=True)
+        pn.pn_integrate(d_y4, d_m4, 0.0, cfg4.omegaf, cfg4.rtol, cfg4.atol, 0, fb, sb, stream=s2, async_=True)
+        assert pn.pn_stream_status(s2) == 0 and pn.pn_stream_status(s1) == 0
+        assert np.array_equal(fa.cpu().numpy(), ref3["final"]) and np.array_equal(sa.cpu().numpy(), ref3["steps"])
+        assert np.array_equal(fb.cpu().numpy(), ref4["final"]) and np.array_equal(sb.cpu().numpy(), ref4["steps"])
+    # a sync call on the default stream is untouched by all that
+    again = gpu_integrate(pn, y3, m3, cfg3)
+    assert again["status"] == 0 and np.array_equal(again["final"], ref3["final"])
+
+
+def test_fma_microbenchmark_is_self_consistent(pn):
+    """The FP64 peak and operand-port micro-benchmarks behind the roofline denominator: the SM clock
+    estimated from the longest per-block clock64() span agrees with nvidia-smi, the throughput with 64 FMA lanes per SM
+    at that clock, and a DFMA issues every 2 cycles with <= 2 distinct register sources, every 3 with 3."""
+    import subprocess
+
+    tf, mhz = pn.pn_measure_fma_peak(pn.PN_FP64, 0.2)
+    mx = float(subprocess.check_output(["nvidia-smi", "--query-gpu=clocks.max.sm", "--format=csv,noheader,nounits", "-i", "0"]).decode().split()[0])
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    assert 0.9 * mx <= mhz <= 1.02 * mx, (mhz, mx)
+    assert abs(tf / (sms * 64 * 2 * mhz * 1e6 / 1e12) - 1) < 0.03, (tf, mhz)
+    cyc = [pn.pn_measure_fma_operands(pn.PN_FP64, k) for k in (1, 2, 3)]
+    assert abs(cyc[0] - 2.0) < 0.25 and abs(cyc[1] - 2.0) < 0.1 and abs(cyc[2] - 3.0) < 0.15, cyc

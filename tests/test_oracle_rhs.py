@@ -196,3 +196,24 @@ def test_precession_leading_behaviour(oracle):
     assert np.allclose(f[1:4], Om * np.cross(L, S1), rtol=1e-13, atol=0)
     assert np.allclose(f[4:7], 0.0)
     assert np.allclose(f[7:10], -om ** (1 / 3) / eta * f[1:4], rtol=1e-13, atol=0)
+
+
+def test_two_spin_precession_by_hand(oracle):
+    """Eq. (4) with BOTH spins present, reduced by hand for a configuration whose numbers are exact
+    (Omega_1 = (M omega)^2/(2M) [eta (M omega)^{-1/3} (4 + 3 m2/m1) L^ + 1/M^2 (S2 - 3 (S2.L^) L^)]).
+
+    m = (1.2, 0.8): M = 2, eta = 0.24.  omega = 1/16: M omega = 1/8, (M omega)^{1/3} = 1/2, (M omega)^2/(2M) = 1/256.
+    L^ = z, S1 = (0.5, 0, 0), S2 = (0, 0.25, 0.4).
+      Omega_1: eta/v (4 + 3*0.8/1.2) = 0.48 * 6 = 2.88;  S2 - 3 (S2.L^) L^ = (0, 0.25, 0.4 - 1.2) = (0, 0.25, -0.8);
+               Omega_1 = (0, 0.25/4, 2.88 - 0.8/4)/256 = (0, 0.0625, 2.68)/256
+      S1_dot = Omega_1 x S1 = (0, 2.68*0.5, -0.0625*0.5)/256 = (0, 1.34, -0.03125)/256
+      Omega_2: eta/v (4 + 3*1.2/0.8) = 0.48 * 8.5 = 4.08;  S1 - 3 (S1.L^) L^ = S1;  Omega_2 = (0.125, 0, 4.08)/256
+      S2_dot = Omega_2 x S2 = (-4.08*0.25, -0.125*0.4, 0.125*0.25)/256 = (-1.02, -0.05, 0.03125)/256
+      L^_dot = -(1/2)/(0.24*4) (S1_dot + S2_dot) = -(1/1.92) (-1.02, 1.29, 0)/256 = (0.53125, -0.671875, 0)/256
+    The z-component of S1_dot is pure spin-spin (pins 1/M^2); the -0.8 = 0.4 - 3*0.4 pins the "3"."""
+    y = np.array([[1 / 16, 0.5, 0, 0, 0, 0.25, 0.4, 0, 0, 1.0]])
+    f = oracle.rhs(y, np.array([[1.2, 0.8]]))[0]
+    expect = np.array([0, 1.34, -0.03125, -1.02, -0.05, 0.03125, 0.53125, -0.671875, 0]) / 256
+    assert np.abs(f[1:] - expect).max() < 2e-17 + 1e-14 * np.abs(expect).max()
+    # a wrong "3" (say 2) would move S1_dot_y by 0.5*0.4/4/256 = 1.95e-4; a missing 1/M^2 would quadruple S1_dot_z
+    assert abs(f[2] * 256 - 1.34) < 1e-13 and abs(f[3] * 256 + 0.03125) < 1e-15

@@ -76,3 +76,37 @@ def test_single_process_is_a_noop():
     assert sharding.allreduce_counts(c, dist).sum().item() == 15
     assert sharding.max_over_ranks(3.5, torch.device("cpu"), dist) == 3.5
     assert sharding.allgather_moments(torch.ones(4, 3, 6, dtype=torch.float64), dist).shape == (1, 4, 3, 6)
+
+
+def _bench(*flags, env=None):
+    import json
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    e = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    e.update(env or {})
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), *flags], capture_output=True, text=True, env=e, timeout=300)
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    return r, (json.loads(lines[-1]) if lines else None)
+
+
+def test_bench_spawns_its_own_ranks():
+    """`python bench.py --gpus 2` (no torchrun environment) must run TWO ranks: bench.py re-executes itself under
+    torch.distributed.run.  --dry keeps CUDA out of it: launch, sharding and the exchange step only (gloo)."""
+    r, line = _bench("--gpus", "2", "--dry", "--workload", "C1")
+    assert r.returncode == 0, r.stderr[-2000:]
+    assert line["n_gpus"] == 2 and line["scaling"] == "weak"
+    assert line["systems_all_ranks"] == line["systems_expected"] == 2 * 1024      # both ranks reached the all-reduce
+    assert line["max_over_ranks"] == 2.0
+    # strong scaling: one batch split over the ranks
+    r, line = _bench("--gpus", "2", "--dry", "--workload", "C1", "--scaling", "strong")
+    assert r.returncode == 0 and line["n_gpus"] == 2 and line["systems_rank0"] == 512 and line["systems_all_ranks"] == 1024
+    # one rank: no spawn, same code path
+    r, line = _bench("--dry", "--workload", "C1")
+    assert r.returncode == 0 and line["n_gpus"] == 1 and line["systems_all_ranks"] == 1024
+
+
+def test_bench_refuses_a_mislabelled_world():
+    r, line = _bench("--gpus", "8", "--dry", env={"WORLD_SIZE": "2", "RANK": "0"})
+    assert r.returncode != 0 and line is None and "WORLD_SIZE=2" in r.stderr
