@@ -234,7 +234,7 @@ def run_ours(args, cfg):
 
     def step():
         pn.pn_integrate(d_y0, d_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, d_yf, d_steps,
-                        input_order=bool(args.input_order))
+                        input_order=bool(args.input_order), variant=args.variant)
         pn.pn_histogram(d_yf, cfg.bins, d_counts)
         sharding.allreduce_counts(d_counts, dist if world > 1 else None)   # the one exchange step
 
@@ -278,7 +278,7 @@ def run_ours(args, cfg):
 
     def e2e_step():
         pn.pn_integrate(h_y0, h_m, cfg.omega0, cfg.omegaf, cfg.rtol, cfg.atol, prec, h_yf, h_steps,
-                        input_order=bool(args.input_order))
+                        input_order=bool(args.input_order), variant=args.variant)
         pn.pn_histogram(h_yf, cfg.bins, h_counts)
 
     e2e_step()
@@ -352,7 +352,7 @@ def run_ours(args, cfg):
         "dtype": {pn.PN_FP32: "f32", pn.PN_MIXED: "f32 slopes + f64 state"}.get(prec, "f64"), "data": "synthetic",
         "comm": {"backend": "nccl" if world > 1 else None, "nranks": world, "exchange": "all-reduce of 3 x bins int64 counters per step"},
         "config": {"workload": cfg.name, "n_inspirals": cfg.n, "n_inspirals_per_gpu": n, "omega0": cfg.omega0, "omegaf": cfg.omegaf,
-                   "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "queue": "input order" if args.input_order else "longest-expected-first", "parallelism": f"batch-sharded x{world}",
+                   "rtol": cfg.rtol, "atol": cfg.atol, "bins": cfg.bins, "queue": "input order" if args.input_order else "longest-expected-first", "variant": args.variant, "parallelism": f"batch-sharded x{world}",
                    "l2": "256 MiB memset between steps, inside the timed region (<0.1 % of a step)"},
         "rhs_evals_per_sec": rhs_all_ranks / (ms_step * 1e-3),
         "trial_steps_per_inspiral": float(np.mean(trial_steps)) / n,
@@ -399,6 +399,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--input-order", type=int, default=0, help="1: issue the work queue in input order instead of longest-expected-first")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--variant", type=int, default=0, help="pn_options.variant (kernel selection bits; not a bench line unless 0)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="weak: every rank its own full-size batch; strong: one batch split over the ranks")
     ap.add_argument("--dry", action="store_true", help="launch / sharding / exchange logic only, on the CPU with gloo (tests)")

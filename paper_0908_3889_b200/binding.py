@@ -257,8 +257,8 @@ def pn_generate(ensembles, n_total, init_states, masses, *, first=0, count=None,
     arr = (PnEnsemble * len(ens))(*ens)
     count = int(n_total) - int(first) if count is None else int(count)
     host = _is_host(init_states)
-    _require("init_states", init_states, "f64", (len(ens) * max(count, 0), 10), host)
-    _require("masses", masses, "f64", (len(ens) * max(count, 0), 2), host)
+    _require("init_states", init_states, "f64", (len(ens) * max(count, 0), 10), host, at_least=True)
+    _require("masses", masses, "f64", (len(ens) * max(count, 0), 2), host, at_least=True)
     if host:
         opts["host_buffers"] = True
     o = make_options(**opts)

@@ -42,55 +42,59 @@
 // error estimate err = sum_s e_s K_s.  6 RHS evaluations, 200 + 60 FMAs.
 // WANT_DY (mixed precision): the increment dy = sum_s b_s K_s is formed on its own and
 // y_new = y + dy, so that the caller can add dy to a higher-precision copy of the state.
-template <bool SLOW, typename real, bool WANT_DY = false>
-__device__ __forceinline__ void pn_dp5_trial(const real (&y)[10], const real (&K1)[10], real h,
+// vec / NV: the element type and length of the state and slope arrays.  Default: NV = 10 values of `real`.  The
+// pair-packed FP32 kernel (pn_integrate_packed.cu) passes vec = f2, NV = 5: the ten components of ONE system in five
+// register pairs, so that every stage sum below is a packed FFMA2 (two components per issue slot); pn_rhs has an
+// overload for that layout.
+template <bool SLOW, typename real, bool WANT_DY = false, typename vec = real, int NV = 10>
+__device__ __forceinline__ void pn_dp5_trial(const vec (&y)[NV], const vec (&K1)[NV], real h,
                                              const PnConsts<real>& c, const PnUni<real>& u, const PnBase<real>& base,
-                                             real (&ynew)[10], real (&K7)[10], real (&err)[10], PnBase<real>& base_new, bool& bad,
-                                             real* dy = nullptr)
+                                             vec (&ynew)[NV], vec (&K7)[NV], vec (&err)[NV], PnBase<real>& base_new, bool& bad,
+                                             vec* dy = nullptr)
 {
-    real K2[10], K3[10], K4[10], K5[10], K6[10], ys[10];
+    vec K2[NV], K3[NV], K4[NV], K5[NV], K6[NV], ys[NV];
     real r_tmp, l_tmp;
     PnScaled<real> sc;
     pn_make_scaled(c, h, sc);
 #pragma unroll
-    for (int i = 0; i < 10; ++i) ys[i] = pn_fma((real)DP_A21, K1[i], y[i]);
+    for (int i = 0; i < NV; ++i) ys[i] = pn_fma((vec)DP_A21, K1[i], y[i]);
     pn_rhs<SLOW>(ys, c, u, sc, base, K2, r_tmp, l_tmp, bad);
 #pragma unroll
-    for (int i = 0; i < 10; ++i) ys[i] = pn_fma((real)DP_A32, K2[i], pn_fma((real)DP_A31, K1[i], y[i]));
+    for (int i = 0; i < NV; ++i) ys[i] = pn_fma((vec)DP_A32, K2[i], pn_fma((vec)DP_A31, K1[i], y[i]));
     pn_rhs<SLOW>(ys, c, u, sc, base, K3, r_tmp, l_tmp, bad);
 #pragma unroll
-    for (int i = 0; i < 10; ++i)
-        ys[i] = pn_fma((real)DP_A43, K3[i], pn_fma((real)DP_A42, K2[i], pn_fma((real)DP_A41, K1[i], y[i])));
+    for (int i = 0; i < NV; ++i)
+        ys[i] = pn_fma((vec)DP_A43, K3[i], pn_fma((vec)DP_A42, K2[i], pn_fma((vec)DP_A41, K1[i], y[i])));
     pn_rhs<SLOW>(ys, c, u, sc, base, K4, r_tmp, l_tmp, bad);
 #pragma unroll
-    for (int i = 0; i < 10; ++i)
-        ys[i] = pn_fma((real)DP_A54, K4[i],
-                       pn_fma((real)DP_A53, K3[i], pn_fma((real)DP_A52, K2[i], pn_fma((real)DP_A51, K1[i], y[i]))));
+    for (int i = 0; i < NV; ++i)
+        ys[i] = pn_fma((vec)DP_A54, K4[i],
+                       pn_fma((vec)DP_A53, K3[i], pn_fma((vec)DP_A52, K2[i], pn_fma((vec)DP_A51, K1[i], y[i]))));
     pn_rhs<SLOW>(ys, c, u, sc, base, K5, r_tmp, l_tmp, bad);
 #pragma unroll
-    for (int i = 0; i < 10; ++i)
-        ys[i] = pn_fma((real)DP_A65, K5[i],
-                       pn_fma((real)DP_A64, K4[i],
-                              pn_fma((real)DP_A63, K3[i], pn_fma((real)DP_A62, K2[i], pn_fma((real)DP_A61, K1[i], y[i])))));
+    for (int i = 0; i < NV; ++i)
+        ys[i] = pn_fma((vec)DP_A65, K5[i],
+                       pn_fma((vec)DP_A64, K4[i],
+                              pn_fma((vec)DP_A63, K3[i], pn_fma((vec)DP_A62, K2[i], pn_fma((vec)DP_A61, K1[i], y[i])))));
     pn_rhs<SLOW>(ys, c, u, sc, base, K6, r_tmp, l_tmp, bad);
 #pragma unroll
-    for (int i = 0; i < 10; ++i) {
+    for (int i = 0; i < NV; ++i) {
         if (WANT_DY) {
-            dy[i] = pn_fma((real)DP_B6, K6[i],
-                           pn_fma((real)DP_B5, K5[i],
-                                  pn_fma((real)DP_B4, K4[i], pn_fma((real)DP_B3, K3[i], (real)DP_B1 * K1[i]))));
+            dy[i] = pn_fma((vec)DP_B6, K6[i],
+                           pn_fma((vec)DP_B5, K5[i],
+                                  pn_fma((vec)DP_B4, K4[i], pn_fma((vec)DP_B3, K3[i], (vec)DP_B1 * K1[i]))));
             ynew[i] = y[i] + dy[i];
         } else {
-            ynew[i] = pn_fma((real)DP_B6, K6[i],
-                             pn_fma((real)DP_B5, K5[i],
-                                    pn_fma((real)DP_B4, K4[i], pn_fma((real)DP_B3, K3[i], pn_fma((real)DP_B1, K1[i], y[i])))));
+            ynew[i] = pn_fma((vec)DP_B6, K6[i],
+                             pn_fma((vec)DP_B5, K5[i],
+                                    pn_fma((vec)DP_B4, K4[i], pn_fma((vec)DP_B3, K3[i], pn_fma((vec)DP_B1, K1[i], y[i])))));
         }
-        err[i] = pn_fma((real)DP_E6, K6[i],
-                        pn_fma((real)DP_E5, K5[i],
-                               pn_fma((real)DP_E4, K4[i], pn_fma((real)DP_E3, K3[i], (real)DP_E1 * K1[i]))));
+        err[i] = pn_fma((vec)DP_E6, K6[i],
+                        pn_fma((vec)DP_E5, K5[i],
+                               pn_fma((vec)DP_E4, K4[i], pn_fma((vec)DP_E3, K3[i], (vec)DP_E1 * K1[i]))));
     }
     pn_rhs<SLOW>(ynew, c, u, sc, base, K7, r_tmp, l_tmp, bad);
     base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
 #pragma unroll
-    for (int i = 0; i < 10; ++i) err[i] = pn_fma((real)DP_E7, K7[i], err[i]);
+    for (int i = 0; i < NV; ++i) err[i] = pn_fma((vec)DP_E7, K7[i], err[i]);
 }

@@ -6,67 +6,7 @@
 // global atomic work queue (warp-aggregated atomicAdd), so adaptive-step and termination divergence
 // cost only the short refill section.  All state (y, k1..k7, per-system constants) lives in
 // registers; global memory is touched only at refill and at finish.  (DESIGN.md 2, 7.)
-#include <cfloat>
-#include "pn_dp5.cuh"
-#include "pn_internal.h"
-
-#define PN_ST_EINVAL 1
-#define PN_ST_ENOTCONVERGED 3
-#define PN_ST_ENONFINITE 4
-#define PN_F_MAXSTEPS (-1)
-#define PN_F_HUNDERFLOW (-2)
-#define PN_F_NONFINITE (-3)
-#define PN_F_LANDING (-4)
-#define PN_F_BADINPUT (-5)
-
-template <typename real> struct PnLimits;
-template <> struct PnLimits<double> { static __device__ double tiny() { return 1e-300; } static __device__ double huge() { return DBL_MAX; } };
-template <> struct PnLimits<float> { static __device__ float tiny() { return 1e-30f; } static __device__ float huge() { return FLT_MAX; } };
-
-template <typename real> struct PnVec;
-template <> struct PnVec<double> {
-    typedef double2 type;
-    static __device__ __forceinline__ double2 make(const double* a) { return make_double2(a[0], a[1]); }
-    static __device__ __forceinline__ void unpack(double2 v, double* a) { a[0] = v.x; a[1] = v.y; }
-};
-template <> struct PnVec<float> {
-    typedef float4 type;
-    static __device__ __forceinline__ float4 make(const float* a) { return make_float4(a[0], a[1], a[2], a[3]); }
-    static __device__ __forceinline__ void unpack(float4 v, float* a) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
-};
-
-// 0.9 * E^{-1/5} (controller, DESIGN.md 3 R8).  Evaluated with the FP32 special-function unit in both
-// precisions: the factor only sets the next trial's step size, 1e-6 relative accuracy is ample and
-// it keeps ~100 instructions per trial step off the FP64 pipe.
-// argument: E^2 = mean_j (err_j/sc_j)^2, so the factor is 0.9 (E^2)^{-1/10}; no square root needed.
-__device__ __forceinline__ float pn_ctrl_factor(float E2) { return 0.9f * exp2f(-0.1f * __log2f(E2)); }
-
-// err/sc for the error norm: MUFU reciprocal seed (rcp.approx.ftz.f64, ~2^-23) + one Newton step gives
-// ~1.4e-14 relative accuracy with 3 FP64-pipe instructions and no slow-path branch (an IEEE divide is ~10).
-__device__ __forceinline__ double pn_ratio(double a, double b)
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
-    r = fma(fma(-b, r, 1.0), r, r);
-    return a * r;
-}
-__device__ __forceinline__ float pn_ratio(float a, float b) { return __fdividef(a, b); }
-
-template <typename real>
-__device__ __forceinline__ void pn_store_result(const PnKernelParams& p, int idx, const real (&y)[10], int code,
-                                                double t, int nrej)
-{
-#pragma unroll
-    for (int i = 0; i < 10; ++i) p.yf[(size_t)i * p.n + idx] = (double)y[i];
-    p.steps[idx] = code;
-    if (p.time) p.time[idx] = t;
-    if (p.rejected) p.rejected[idx] = nrej;
-}
-
-// FP32 helpers without the denormal-range fix-up code the CUDA intrinsics carry (inputs are clamped).
-__device__ __forceinline__ float pn_rcp_f(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
-__device__ __forceinline__ float pn_lg2_f(float a) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
-__device__ __forceinline__ float pn_ex2_f(float a) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+#include "pn_step_common.cuh"
 
 // E^2 of the scaled RMS error norm, returned in FP32 (see the call site).
 __device__ __forceinline__ float pn_err_norm2(const double (&y)[10], const double (&ynew)[10], const double (&err)[10],
@@ -109,7 +49,6 @@ __device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float 
 // PN_REC reals per system (FP64 320 B, FP32 160 B), so a lane's refill is 20 (10) 16-byte loads.
 //   [0..9] y0   [10..19] K1 = h0 f(y0)   [20..34] PnConsts   [35..37] PnBase   [38] atol |S1|   [39] atol |S2|
 // A record with [38] < 0 marks a system the seed kernel has already failed (bad input).
-#define PN_REC 40
 template <typename real>
 __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
 {
@@ -173,7 +112,11 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     const double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
     real out[PN_REC];
 #pragma unroll
-    for (int j = 0; j < 10; ++j) { out[j] = y[j]; out[10 + j] = k1[j]; }
+    for (int j = 0; j < 10; ++j) {
+        // rec_pairs: the pair-packed FP32 kernel wants each register pair as two adjacent, 8-byte aligned words
+        const int pos = p.rec_pairs ? 2 * PN_PAIR_OF[j] + PN_PAIR_HALF[j] : j;
+        out[pos] = y[j]; out[10 + pos] = k1[j];
+    }
     out[20] = c.M; out[21] = c.c2; out[22] = c.c4; out[23] = c.c5; out[24] = c.c6; out[25] = c.c7;
     out[26] = c.p1; out[27] = c.p2; out[28] = c.q1; out[29] = c.q2; out[30] = c.K0; out[31] = c.A1;
     out[32] = c.A2; out[33] = c.Bc; out[34] = c.G;
@@ -185,16 +128,6 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     constexpr int W = 16 / (int)sizeof(real);
 #pragma unroll
     for (int j = 0; j < PN_REC / W; ++j) dst[j] = PnVec<real>::make(&out[j * W]);
-}
-
-template <typename real>
-__device__ __forceinline__ void pn_load_record(const void* seed, int i, real (&out)[PN_REC])
-{
-    using vec = typename PnVec<real>::type;
-    constexpr int W = 16 / (int)sizeof(real);
-    const vec* src = (const vec*)((const real*)seed + (size_t)i * PN_REC);
-#pragma unroll
-    for (int j = 0; j < PN_REC / W; ++j) PnVec<real>::unpack(__ldg(src + j), &out[j * W]);
 }
 
 // SLOW = true: the redo pass.  Systems whose step left the range of the cbrt/log series in the fast kernel
@@ -523,6 +456,7 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
         // stage-in: per-system seed records (constants, base powers, K1 = h0 f(y0)), expected-cost keys; bad inputs fail here
         const int grid = (p.n + 127) / 128;
         if (p.keys && (e = pn_launch_order_init(p.order_scratch, s)) != cudaSuccess) return e;
+        p.rec_pairs = (precision == 1 && block_threads == 0 && !(variant & 2)) ? 1 : 0;      // consumer: the pair-packed kernel
         if (precision == 0) pn_seed_kernel<double><<<grid, 128, 0, s>>>(p);
         else pn_seed_kernel<float><<<grid, 128, 0, s>>>(p);
         ++g_pn_launches;
@@ -556,6 +490,9 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
         return launch_adaptive<double, 128, 2, true>(p, grid_blocks, s);
     }
     if (precision == 2) return launch_adaptive<float, 128, 3, false, true>(p, grid_blocks, s);   // PN_MIXED
+    // PN_FP32: two systems per lane with packed f32x2 arithmetic (pn_integrate_packed.cu) unless the scalar kernel is
+    // asked for (pn_options.variant bit 1, or an explicit block shape); the results are bit-identical
     if (block_threads == 128) return launch_adaptive<float, 128, 4, false>(p, grid_blocks, s);
-    return launch_adaptive<float, 256, 2, false>(p, grid_blocks, s);
+    if (block_threads == 256 || (variant & 2)) return launch_adaptive<float, 256, 2, false>(p, grid_blocks, s);
+    return pn_launch_integrate_packed(p, grid_blocks, s);         // its seed records were written with rec_pairs = 1 above
 }

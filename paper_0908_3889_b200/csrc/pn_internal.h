@@ -34,12 +34,15 @@ struct PnKernelParams {
     float* keys;                    // [n] or null: expected-cost keys written by the seed kernel (queue ordering)
     unsigned int* order_scratch;    // [PN_ORDER_BUCKETS + 2]: bucket cursors, then the bit patterns of the smallest / largest key
     int* order_out;                 // [n]: the queue order the bucket sort writes (= order when keys != null)
+    int rec_pairs;                  // FP32 seed records with y0 and K1 in the pair order of the pair-packed kernel (pn_rhs.cuh)
 };
 
 // launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults
 // variant bits (pn_options.variant): 1 = always the generic FP64 kernel (per-lane constants), 2 = always the scalar FP32 kernel
 cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
                                 cudaStream_t s, int variant);
+// pair-packed FP32 integrator (pn_integrate_packed.cu); the seed records must be float ones written with rec_pairs = 1
+cudaError_t pn_launch_integrate_packed(const PnKernelParams& p, int grid_blocks, cudaStream_t s);
 // staging + histogram + peak (pn_aux.cu)
 cudaError_t pn_launch_aos_to_soa(const double* aos, double* soa, int n, int width, cudaStream_t s);
 cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int width, cudaStream_t s);

@@ -10,6 +10,7 @@
 // This file shares nothing with oracle/ (which evaluates the equations as printed).
 #pragma once
 #include <cuda_runtime.h>
+#include "pn_f2.cuh"
 
 #define PN_MASK_ALL 0x100FFu
 #define PN_MASK_SPIN (1u << 16)
@@ -109,6 +110,7 @@ __device__ __forceinline__ void pn_base_init(double x, PnBase<double>& b)
     b.l0 = log(x);
 }
 __device__ __forceinline__ void pn_base_init(float, PnBase<float>& b) { b.r0 = b.r03 = b.l0 = 0.0f; }
+__device__ __forceinline__ void pn_base_init(f2, PnBase<f2>& b) { b.r0 = b.r03 = b.l0 = f2(0.0f); }
 
 // r = x^{-1/3}, lnx = ln x  ->  returned so that an accepted step can adopt them as the next base.
 // SLOW = false: series only, branch-free; `bad` is raised when |e| is outside the series' range, and the
@@ -193,6 +195,25 @@ __device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float, 
     r = 0.0f;
 }
 
+// packed FP32 (two systems per lane): the special-function unit is per component, the polish and the powers are packed
+template <bool SLOW>
+__device__ __forceinline__ void pn_powers(f2 x, const PnBase<f2>&, f2, f2& v, f2& lnx, f2& r, bool&)
+{
+    float la, lb, ra, rb;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(la) : "f"(x.v.x));
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lb) : "f"(x.v.y));
+    const f2 l2(la, lb);
+    lnx = l2 * f2(0.693147180559945f);
+    const f2 t = l2 * f2(-1.0f / 3.0f);
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ra) : "f"(t.v.x));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(rb) : "f"(t.v.y));
+    f2 r0(ra, rb);
+    const f2 e = pn_fma(-(x * r0), r0 * r0, f2(1.0f));
+    r0 = pn_fma(r0 * e, f2(1.0f / 3.0f), r0);
+    v = x * (r0 * r0);
+    r = f2(0.0f);
+}
+
 // The slopes are produced already multiplied by the step size h ("scaled slopes" K = h f): the four
 // prefactors that enter every output linearly are pre-multiplied by h once per trial step, which costs
 // nothing per evaluation and lets every stage sum of the stepper use compile-time tableau coefficients
@@ -267,4 +288,69 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     f[7] = g * (f[1] + f[4]);
     f[8] = g * (f[2] + f[5]);
     f[9] = g * (f[3] + f[6]);
+}
+
+// ---- pair-packed FP32 layout (pn_integrate_packed.cu) -------------------------------------------------------------
+// The ten components of ONE system in five register pairs, so that everything that treats the components alike (the
+// Dormand-Prince stage sums, the error vector, the state update: 270 of the ~780 FP32 operations of a trial step) is
+// a packed FFMA2 / FMUL2 (two components per issue slot), and the vector operations of the RHS whose x and y
+// components share their scalar factors are packed too:
+//     pair 0 = (S1x, S1y)   pair 1 = (S2x, S2y)   pair 2 = (Lx, Ly)   pair 3 = (omega, S1z)   pair 4 = (S2z, Lz)
+// Component i of y = (omega, S1, S2, L^) lives in half PN_PAIR_HALF[i] of pair PN_PAIR_OF[i].  Per component the
+// operations and their order are exactly those of the scalar pn_rhs above, so the results are bit-identical.
+__device__ constexpr int PN_PAIR_OF[10] = {3, 0, 0, 3, 1, 1, 4, 2, 2, 4};
+__device__ constexpr int PN_PAIR_HALF[10] = {0, 0, 1, 1, 0, 1, 0, 0, 1, 1};
+template <int I> __device__ __forceinline__ float pn_pair_get(const f2 (&a)[5]) { return f2_get<PN_PAIR_HALF[I]>(a[PN_PAIR_OF[I]]); }
+template <int I> __device__ __forceinline__ void pn_pair_set(f2 (&a)[5], float x) { f2_set<PN_PAIR_HALF[I]>(a[PN_PAIR_OF[I]], x); }
+
+template <bool SLOW>
+__device__ __forceinline__ void pn_rhs(const f2 (&y)[5], const PnConsts<float>& c, const PnUni<float>& u,
+                                       const PnScaled<float>& sc, const PnBase<float>& base,
+                                       f2 (&f)[5], float& r_out, float& lnx_out, bool& bad)
+{
+    const float x = c.M * y[3].v.x;
+    float v, lnx, r;
+    pn_powers<SLOW>(x, base, u.emax, v, lnx, r, bad);
+    r_out = r; lnx_out = lnx;
+    const float v2 = v * v, v4 = v2 * v2, v5 = v4 * v, x2 = x * x;
+
+    const float S1x = y[0].v.x, S1y = y[0].v.y, S1z = y[3].v.y;
+    const float S2x = y[1].v.x, S2y = y[1].v.y, S2z = y[4].v.x;
+    const float Lx = y[2].v.x, Ly = y[2].v.y, Lz = y[4].v.y;
+
+    const float LS1 = fmaf(Lx, S1x, fmaf(Ly, S1y, Lz * S1z));
+    const float LS2 = fmaf(Lx, S2x, fmaf(Ly, S2y, Lz * S2z));
+    const float S12 = fmaf(S1x, S2x, fmaf(S1y, S2y, S1z * S2z));
+
+    const float k3 = fmaf(c.p1, LS1, fmaf(c.p2, LS2, u.c3));
+    const float k4 = fmaf(c.q1, S12, fmaf(c.q2 * LS1, LS2, c.c4));
+    const float k6 = fmaf(u.cl, lnx, c.c6);
+    const float e67 = fmaf(c.c7, v, k6), e45 = fmaf(c.c5, v, k4), e23 = fmaf(k3, v, c.c2);
+    const float hi = fmaf(e67, v2, e45);
+    float B = fmaf(e23, v2, u.c0);
+    B = fmaf(hi, v4, B);
+    const float f0 = (sc.hK0 * (v5 * x2)) * B;
+
+    // Eq. (4): h Omega_1 = al1 L + beta S2,  h Omega_2 = al2 L + beta S1; x and y components packed
+    const float beta = sc.hBc * x2;
+    const float b3 = 3.0f * beta;
+    const float al1 = fmaf(-b3, LS2, sc.hA1 * v5);
+    const float al2 = fmaf(-b3, LS1, sc.hA2 * v5);
+    const f2 O1 = pn_fma(f2(beta), y[1], f2(al1) * y[2]);
+    const f2 O2 = pn_fma(f2(beta), y[0], f2(al2) * y[2]);
+    const float O1z = fmaf(beta, S2z, al1 * Lz), O2z = fmaf(beta, S1z, al2 * Lz);
+    // Eq. (2): S_i_dot = Omega_i x S_i
+    const float f1 = fmaf(O1.v.y, S1z, -(O1z * S1y));
+    const float f2v = fmaf(O1z, S1x, -(O1.v.x * S1z));
+    const float f3 = fmaf(O1.v.x, S1y, -(O1.v.y * S1x));
+    const float f4 = fmaf(O2.v.y, S2z, -(O2z * S2y));
+    const float f5 = fmaf(O2z, S2x, -(O2.v.x * S2z));
+    const float f6 = fmaf(O2.v.x, S2y, -(O2.v.y * S2x));
+    // Eq. (3)
+    const float g = c.G * v;
+    f[0] = f2(f1, f2v);
+    f[1] = f2(f4, f5);
+    f[2] = f2(g) * (f[0] + f[1]);
+    f[3] = f2(f0, f3);
+    f[4] = f2(f6, g * (f3 + f6));
 }

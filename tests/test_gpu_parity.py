@@ -170,3 +170,41 @@ def test_leading_order_closed_form_on_gpu(pn):
     tf = (0.005 ** (-8 / 3) - 0.05 ** (-8 / 3)) / (256 / 5 * m1 * (1 - m1))
     assert np.abs(g["time"] / tf - 1).max() < 5e-12
     assert np.array_equal(g["final"][:, 1:], y0[:, 1:])      # nothing precesses
+
+
+def test_packed_fp32_kernel_is_bit_identical_to_the_scalar_one(pn):
+    """PN_FP32 keeps the ten components of a system in five register pairs and uses packed f32x2 arithmetic (FFMA2 /
+    FMUL2 / FADD2) for the stage sums, the error vector and the x / y halves of the RHS's vector operations, and it
+    prefetches seed records through shared memory.  Per component it performs the same IEEE operations
+    in the same order as the plain scalar kernel (pn_options.variant bit 1 selects that one), so every output must agree
+    bit for bit: ragged batch sizes, mixed masses, bad inputs, max_steps failures, tight and loose tolerances."""
+    for name, n, tol in (("C4f", 5003, None), ("C3", 4097, (1e-5, 1e-7)), ("C3", 1, (1e-6, 1e-8)), ("C2", 2, (1e-4, 1e-6)),
+                         ("C5", 63, (1e-5, 1e-7)), ("C1", 257, (1e-7, 1e-9))):
+        cfg = W.with_size(W.CONFIGS[name], n)
+        y0, m = W.generate(cfg)
+        rtol, atol = tol if tol else (cfg.rtol, cfg.atol)
+        a = gpu_integrate(pn, y0, m, cfg, rtol=rtol, atol=atol, precision=1)
+        b = gpu_integrate(pn, y0, m, cfg, rtol=rtol, atol=atol, precision=1, variant=2)
+        assert a["status"] == 0 and np.all(a["steps"] > 0)
+        for k in ("final", "steps", "time", "rejected"):
+            assert np.array_equal(a[k], b[k]), (name, n, k)
+    # batches large enough for every lane to run through the prefetch pipeline many times, in both queue orders
+    cfg = W.with_size(W.CONFIGS["C4f"], 300000 + 11)
+    y0, m = W.generate(cfg)
+    for io in (False, True):
+        a = gpu_integrate(pn, y0, m, cfg, precision=1, input_order=io)
+        b = gpu_integrate(pn, y0, m, cfg, precision=1, variant=2, input_order=io)
+        for k in ("final", "steps", "time", "rejected"):
+            assert np.array_equal(a[k], b[k]), (io, k)
+    # failures and bad inputs land in the same slots with the same codes
+    cfg = W.with_size(W.CONFIGS["C3"], 777)
+    y0, m = W.generate(cfg)
+    m[5, 0] = -1.0; y0[6, 0] = 0.07; y0[9, 2] = np.nan
+    for extra in ({}, {"max_steps": 15}):
+        a = gpu_integrate(pn, y0, m, cfg, rtol=1e-5, atol=1e-7, precision=1, allow_failures=True, **extra)
+        b = gpu_integrate(pn, y0, m, cfg, rtol=1e-5, atol=1e-7, precision=1, variant=2, allow_failures=True, **extra)
+        assert a["status"] == b["status"] != 0
+        assert a["steps"][5] == a["steps"][6] == -5 and a["steps"][9] == -3
+        for k in ("steps", "time", "rejected"):
+            assert np.array_equal(a[k], b[k]), k
+        assert np.array_equal(a["final"], b["final"], equal_nan=True)
