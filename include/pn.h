@@ -207,6 +207,30 @@ int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long
                 double* init_states, double* masses, const struct pn_options* opt);
 
 /*
+ * pn_run_ensembles -- seed in, statistics out: ONE fused launch sequence that draws the initial data (as pn_generate),
+ * integrates every system to omegaf (as pn_integrate, PN_FP64) and reduces the ensemble statistics (as pn_statistics with
+ * group_size = count), without any state array in device memory: the persistent integrator draws a system from the
+ * counter-based Philox stream when a lane pulls work, and folds a finished system into the statistics instead of storing
+ * it ("generated on the GPU", 104, 112-138).  The device memory a
+ * run needs is independent of its size (the paper's 3.6e8-system run of PAPER.md:120 is one call).
+ *   ens, n_ensembles, n_total, first, count   as in pn_generate: ensemble e contributes the systems
+ *               [first, first+count) of its variate stream; every ens[e].omega0 must be below omegaf.
+ *   omegaf, rtol, atol                        as in pn_integrate; precision must be PN_FP64.
+ *   bins1, bins2, out                         as in pn_statistics with G = n_ensembles groups: pearson_r [G][3],
+ *               moments [G][3][6], n_skipped [G][3] (undefined dot product, or the system failed), hist1 [G][3][bins1],
+ *               hist2 [G][3][bins2][bins2], hist2_max, hist2_norm; any member may be NULL.  DEVICE pointers (host with
+ *               opt->host_buffers).  bins1 <= 2^24, bins2 <= 4096.
+ *   opt         h0, max_steps, term_mask, tau_land, host_buffers, async, stream, grid_blocks are honoured.
+ * Results equal the chain pn_generate -> pn_integrate -> pn_statistics on the same arguments: n, n_skipped and every
+ * histogram count exactly (and reproducibly); means, M2x, M2y, Cxy and r to rounding (the order in which partial moments
+ * are merged depends on timing: r agrees to ~1e-13, not bit for bit).  Queue order is index order (no cost ordering).
+ * Returns the worst per-system status like pn_integrate; pn_last_counters / pn_last_kernel_ms()[1] refer to the run.
+ */
+int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,
+                     double omegaf, double rtol, double atol, int precision, int bins1, int bins2,
+                     const pn_stats_out* out, const struct pn_options* opt);
+
+/*
  * pn_selfcheck -- the paper's cross-check ("a random ~1 % subset" evolved in double precision next to
  * the single-precision GPU run and compared afterwards), on the device.
  *   selection   system i is checked iff u_i < fraction, u_i = element i of the uniform stream of `key`

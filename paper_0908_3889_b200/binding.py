@@ -18,7 +18,7 @@ PN_FP64, PN_FP32, PN_MIXED = 0, 1, 2
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_merge_statistics", "pn_generate", "pn_selfcheck", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_merge_statistics", "pn_generate", "pn_run_ensembles", "pn_selfcheck", "pn_stream_status",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -82,6 +82,7 @@ def load():
         lib.pn_statistics.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
         lib.pn_merge_statistics.argtypes = [vp, i, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_generate.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, vp, vp, C.POINTER(PnOptions)]
+        lib.pn_run_ensembles.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, d, d, d, i, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
         lib.pn_selfcheck.argtypes = [vp, vp, vp, vp, ll, d, d, C.POINTER(C.c_ulonglong), d, d, C.POINTER(PnCheckOut), vp, ll,
                                      C.POINTER(PnOptions)]
         lib.pn_stream_status.argtypes = [vp]
@@ -263,6 +264,37 @@ def pn_generate(ensembles, n_total, init_states, masses, *, first=0, count=None,
         opts["host_buffers"] = True
     o = make_options(**opts)
     return _check(lib.pn_generate(arr, len(ens), int(n_total), int(first), count, _ptr(init_states), _ptr(masses), C.byref(o)))
+
+
+def pn_run_ensembles(ensembles, n_total, omegaf, rtol, atol, *, first=0, count=None, precision=PN_FP64, bins1=0, bins2=0,
+                     pearson_r=None, moments=None, n_skipped=None, hist1=None, hist2=None, hist2_max=None, hist2_norm=None,
+                     allow_failures=False, **opts):
+    """pn_run_ensembles of include/pn.h: seed in, statistics out (no state arrays).  `ensembles`: one PnEnsemble or a list;
+    outputs as in pn_statistics with one group per ensemble (torch CUDA tensors, or numpy for host buffers)."""
+    lib = load()
+    ens = ensembles if isinstance(ensembles, (list, tuple)) else [ensembles]
+    arr = (PnEnsemble * len(ens))(*ens)
+    count = int(n_total) - int(first) if count is None else int(count)
+    G = len(ens)
+    outs = [a for a in (pearson_r, moments, n_skipped, hist1, hist2, hist2_max, hist2_norm) if a is not None]
+    host = _is_host(outs[0]) if outs else False
+    _require("pearson_r", pearson_r, "f64", (G, 3), host, at_least=True)
+    _require("moments", moments, "f64", (G, 3, 6), host, at_least=True)
+    _require("n_skipped", n_skipped, "i64", (G, 3), host, at_least=True)
+    _require("hist1", hist1, "i64", (G, 3, max(int(bins1), 0)), host, at_least=True)
+    _require("hist2", hist2, "i64", (G, 3, max(int(bins2), 0), max(int(bins2), 0)), host, at_least=True)
+    _require("hist2_max", hist2_max, "i64", (G, 3), host, at_least=True)
+    _require("hist2_norm", hist2_norm, "f64", (G, 3, max(int(bins2), 0), max(int(bins2), 0)), host, at_least=True)
+    if host:
+        opts["host_buffers"] = True
+    o = make_options(**opts)
+    out = PnStatsOut()
+    out.size = C.sizeof(PnStatsOut)
+    out.pearson_r, out.moments, out.n_skipped = _ptr(pearson_r), _ptr(moments), _ptr(n_skipped)
+    out.hist1, out.hist2, out.hist2_max, out.hist2_norm = _ptr(hist1), _ptr(hist2), _ptr(hist2_max), _ptr(hist2_norm)
+    st = lib.pn_run_ensembles(arr, len(ens), int(n_total), int(first), count, float(omegaf), float(rtol), float(atol), int(precision),
+                              int(bins1), int(bins2), C.byref(out), C.byref(o))
+    return _check(st, allow=(PN_ENOTCONVERGED, PN_ENONFINITE) if allow_failures else ())
 
 
 def pn_selfcheck(init_states, masses, final_states, omegaf, *, fraction=0.01, key=(0, 0), times=None, rtol_ref=0.0,

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpn_b200.so")
 SOURCES = ["pn_integrate.cu", "pn_integrate_packed.cu", "pn_aux.cu", "pn_stats.cu", "pn_gen.cu", "pn_check.cu", "pn_api.cu"]
-HEADERS = ["pn_rhs.cuh", "pn_dp5.cuh", "pn_f2.cuh", "pn_step_common.cuh", "pn_dots.cuh", "pn_philox.cuh", "pn_internal.h", os.path.join("..", "..", "include", "pn.h")]
+HEADERS = ["pn_rhs.cuh", "pn_dp5.cuh", "pn_f2.cuh", "pn_step_common.cuh", "pn_dots.cuh", "pn_gen.cuh", "pn_moments.cuh", "pn_philox.cuh", "pn_internal.h", os.path.join("..", "..", "include", "pn.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

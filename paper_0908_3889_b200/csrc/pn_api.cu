@@ -49,14 +49,14 @@ struct Buf {
 // with a one-thread kernel at the end, which only pn_stream_status reads and clears.
 struct Ctx {
     Buf soa_in, soa_m, soa_out, small, sticky, redo, seed, keys, order, ord_scr, h_init, h_m, h_final, h_steps, h_time, h_rej,
-        h_counts, st_scratch, st_in, st_out, gen_specs, gen_y, gen_m, ck_idx, ck_tmp, ck_sub, ck_out, ck_in;
+        h_counts, st_scratch, st_in, st_out, gen_specs, gen_y, gen_m, ck_idx, ck_tmp, ck_sub, ck_out, ck_in, fu_scr;
     cudaEvent_t ev[5];
     bool ev_ok = false;
     bool async_pending = false;
     int slot = -1;              // row of the __constant__ table of the uniform-mass kernel; -1: none left (generic kernel only)
-    Buf* all[28] = {&soa_in, &soa_m, &soa_out, &small, &sticky, &redo, &seed, &keys, &order, &ord_scr, &h_init, &h_m, &h_final,
+    Buf* all[29] = {&soa_in, &soa_m, &soa_out, &small, &sticky, &redo, &seed, &keys, &order, &ord_scr, &h_init, &h_m, &h_final,
                     &h_steps, &h_time, &h_rej, &h_counts, &st_scratch, &st_in, &st_out, &gen_specs, &gen_y, &gen_m, &ck_idx,
-                    &ck_tmp, &ck_sub, &ck_out, &ck_in};
+                    &ck_tmp, &ck_sub, &ck_out, &ck_in, &fu_scr};
 };
 static std::map<void*, Ctx*> g_ctx;
 static int g_next_slot = 0;
@@ -434,6 +434,140 @@ extern "C" int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_
     CK(cudaGetLastError());
     CK(cudaEventElapsedTime(&g_ms[0], c.ev[0], c.ev[1]));
     return PN_OK;
+}
+
+// Systems per launch of a fused ensemble run: bounds the redo list (4 B per system) so that the device memory a run
+// needs does not grow with its size; 2^22 systems keep the persistent grid busy for > 100 resident-lane refills.
+#define PN_FUSED_CHUNK (1LL << 22)
+
+extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,
+                                double omegaf, double rtol, double atol, int precision, int bins1, int bins2,
+                                const pn_stats_out* out_in, const pn_options* opt_in)
+{
+    pn_options o;
+    default_options(&o);
+    if (opt_in) {
+        if (opt_in->size != (int)sizeof(pn_options)) return PN_EINVAL;
+        o = *opt_in;
+    }
+    if (!out_in || out_in->size != (int)sizeof(pn_stats_out)) return PN_EINVAL;
+    pn_stats_out out = *out_in;
+    if (!ens || n_ensembles < 1 || n_ensembles > 65536 || n_total < 0 || first < 0 || count < 0 || first + count > n_total ||
+        o.layout != 0 || (o.async && o.host_buffers) || o.fixed_steps > 0)
+        return PN_EINVAL;
+    if (n_total > (1LL << 59) || (long long)n_ensembles * count > (1LL << 40)) return PN_EINVAL;
+    if (precision != PN_FP64) return PN_EINVAL;                          // the fused kernel is the FP64 integrator
+    if (!(rtol > 0.0) || !(atol >= 0.0) || !(omegaf > 0.0)) return PN_EINVAL;
+    if (bins1 > (1 << 24) || bins2 > 4096) return PN_EINVAL;
+    if (bins1 < 1) { bins1 = 0; out.hist1 = nullptr; }
+    if (bins2 < 1) { bins2 = 0; out.hist2 = nullptr; }
+    if (!out.hist2 && (out.hist2_max || out.hist2_norm)) return PN_EINVAL;
+    struct Spec { unsigned long long k0, k1; double v[9]; };
+    std::vector<Spec> h(n_ensembles);
+    for (int e = 0; e < n_ensembles; ++e) {
+        const pn_ensemble& x = ens[e];
+        if (x.size != (int)sizeof(pn_ensemble) || !(x.omega0 > 0.0) || !(x.omega0 < omegaf) || !(x.q_lo > 0.0) || !(x.chi1_lo >= 0.0) ||
+            !(x.chi2_lo >= 0.0) || !(x.m1_fixed < 1.0))
+            return PN_EINVAL;
+        h[e].k0 = x.key[0]; h[e].k1 = x.key[1];
+        const double v[9] = {x.omega0, x.q_lo, x.q_hi, x.m1_fixed, x.chi1_lo, x.chi1_hi, x.chi2_lo, x.chi2_hi, x.s1_tilt_deg};
+        memcpy(h[e].v, v, sizeof v);
+    }
+    if (count == 0) return PN_OK;
+    cudaStream_t s = (cudaStream_t)o.stream;
+    Ctx& c = *ctx_for(o.stream);
+    int rc;
+    if ((rc = ensure_events(c)) != PN_OK) return rc;
+    const long long G = n_ensembles, N = G * count;
+    if ((rc = c.gen_specs.ensure(sizeof(Spec) * (size_t)n_ensembles)) != PN_OK) return rc;
+    CK(cudaMemcpyAsync(c.gen_specs.p, h.data(), sizeof(Spec) * (size_t)n_ensembles, cudaMemcpyHostToDevice, s));
+    CK(cudaStreamSynchronize(s));      // h is a local: the copy must have left it before we return
+
+    // outputs (device, or staged for host buffers) and scratch: running moments, locks, skipped counts, redo list
+    const size_t b_r = sizeof(double) * 3 * (size_t)G, b_m = 6 * b_r, b_sk = sizeof(unsigned long long) * 3 * (size_t)G;
+    const size_t b_h1 = sizeof(unsigned long long) * 3 * (size_t)bins1 * G, b_h2 = sizeof(unsigned long long) * 3 * (size_t)bins2 * bins2 * G;
+    pn_stats_out d = out;
+    if (o.host_buffers) {
+        if ((rc = c.st_out.ensure(b_r + b_m + 2 * b_sk + b_h1 + 2 * b_h2 + 128)) != PN_OK) return rc;
+        char* w = (char*)c.st_out.p;
+        auto take = [&](size_t bytes) { char* r = w; w += (bytes + 15) & ~(size_t)15; return r; };
+        if (out.pearson_r) d.pearson_r = (double*)take(b_r);
+        if (out.moments) d.moments = (double*)take(b_m);
+        if (out.n_skipped) d.n_skipped = (unsigned long long*)take(b_sk);
+        if (out.hist1) d.hist1 = (unsigned long long*)take(b_h1);
+        if (out.hist2) d.hist2 = (unsigned long long*)take(b_h2);
+        if (out.hist2_max) d.hist2_max = (unsigned long long*)take(b_sk);
+        if (out.hist2_norm) d.hist2_norm = (double*)take(b_h2);
+    }
+    const long long chunk = N < PN_FUSED_CHUNK ? N : PN_FUSED_CHUNK;
+    const size_t scr_bytes = b_m + b_sk + sizeof(int) * (size_t)G + sizeof(int) * (size_t)chunk + 64;
+    if ((rc = c.fu_scr.ensure(scr_bytes)) != PN_OK) return rc;
+    if ((rc = c.small.ensure(sizeof(Small))) != PN_OK) return rc;
+    Small* small = (Small*)c.small.p;
+    char* q = (char*)c.fu_scr.p;
+    double* f_mom = (double*)q; q += b_m;
+    unsigned long long* f_skip = (unsigned long long*)q; q += b_sk;
+    int* f_lock = (int*)q; q += sizeof(int) * (size_t)G;
+    q = (char*)(((uintptr_t)q + 15) & ~(uintptr_t)15);
+    int* redo_list = (int*)q;
+    CK(cudaMemsetAsync(c.fu_scr.p, 0, b_m + b_sk + sizeof(int) * (size_t)G, s));
+    CK(cudaMemsetAsync(small, 0, sizeof(Small), s));
+    if (d.hist1) CK(cudaMemsetAsync(d.hist1, 0, b_h1, s));
+    if (d.hist2) CK(cudaMemsetAsync(d.hist2, 0, b_h2, s));
+
+    PnKernelParams p;
+    memset(&p, 0, sizeof p);
+    p.omega0 = 0.0; p.omegaf = omegaf; p.rtol = rtol; p.atol = atol; p.h0 = o.h0;
+    p.tau = o.tau_land > 0.0 ? o.tau_land : 1e-13;
+    p.emax = 0.03;
+    if (rtol > 1e-10) { p.emax = pow(1e-3 * rtol / 0.0852, 1.0 / 9.0); if (p.emax > 0.2) p.emax = 0.2; }
+    p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
+    p.mask = o.term_mask;
+    p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
+    p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = redo_list;
+    p.nonuniform = &small->nonuniform;
+    p.uni_slot = -1;
+    p.f_specs = c.gen_specs.p; p.f_n_total = n_total; p.f_first = first; p.f_count = count;
+    p.f_mom = f_mom; p.f_lock = f_lock; p.f_skipped = f_skip; p.f_hist1 = d.hist1; p.f_hist2 = d.hist2;
+    p.f_bins1 = bins1; p.f_bins2 = bins2;
+    CK(cudaEventRecord(c.ev[1], s));
+    for (long long lo = 0; lo < N; lo += chunk) {
+        if (lo > 0) {                    // fresh work counters for every chunk; step counters and status accumulate
+            CK(cudaMemsetAsync(&small->queue, 0, sizeof(unsigned), s));
+            CK(cudaMemsetAsync(&small->queue2, 0, 2 * sizeof(unsigned), s));
+        }
+        p.n = (int)(N - lo < chunk ? N - lo : chunk);
+        p.f_base = lo;
+        CK(pn_launch_fused(p, o.grid_blocks, s));
+    }
+    CK(cudaEventRecord(c.ev[2], s));
+    if (d.pearson_r || d.moments) CK(pn_launch_stats_merge(f_mom, 1, (int)G, d.moments, d.pearson_r, s));
+    if (d.n_skipped) CK(cudaMemcpyAsync(d.n_skipped, f_skip, b_sk, cudaMemcpyDeviceToDevice, s));
+    if (d.hist2 && (d.hist2_max || d.hist2_norm)) CK(pn_launch_stats_norm(d.hist2, G * 3, bins2 * bins2, d.hist2_max, d.hist2_norm, s));
+    if (o.async) {
+        if ((rc = c.sticky.ensure(sizeof(int))) != PN_OK) return rc;
+        if (!c.async_pending) CK(cudaMemsetAsync(c.sticky.p, 0, sizeof(int), s));
+        CK(pn_launch_fold_status(&small->status, (int*)c.sticky.p, s));
+        c.async_pending = true;
+        return PN_OK;
+    }
+    if (o.host_buffers) {
+        if (out.pearson_r) CK(cudaMemcpyAsync(out.pearson_r, d.pearson_r, b_r, cudaMemcpyDeviceToHost, s));
+        if (out.moments) CK(cudaMemcpyAsync(out.moments, d.moments, b_m, cudaMemcpyDeviceToHost, s));
+        if (out.n_skipped) CK(cudaMemcpyAsync(out.n_skipped, d.n_skipped, b_sk, cudaMemcpyDeviceToHost, s));
+        if (out.hist1) CK(cudaMemcpyAsync(out.hist1, d.hist1, b_h1, cudaMemcpyDeviceToHost, s));
+        if (out.hist2) CK(cudaMemcpyAsync(out.hist2, d.hist2, b_h2, cudaMemcpyDeviceToHost, s));
+        if (out.hist2_max) CK(cudaMemcpyAsync(out.hist2_max, d.hist2_max, b_sk, cudaMemcpyDeviceToHost, s));
+        if (out.hist2_norm) CK(cudaMemcpyAsync(out.hist2_norm, d.hist2_norm, b_h2, cudaMemcpyDeviceToHost, s));
+    }
+    Small hs;
+    CK(cudaMemcpyAsync(&hs, small, sizeof hs, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    CK(cudaGetLastError());
+    CK(cudaEventElapsedTime(&g_ms[1], c.ev[1], c.ev[2]));
+    memcpy(g_counters, hs.counters, sizeof g_counters);
+    g_redo_count = hs.redo_count;          // of the last chunk
+    return hs.status;
 }
 
 extern "C" int pn_selfcheck(const double* init_states, const double* masses, const double* final_states, const double* times,

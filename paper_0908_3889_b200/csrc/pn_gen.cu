@@ -17,27 +17,7 @@
 
 #define GEN_TILE 256
 
-#include "pn_philox.cuh"
-
-// lo + (hi - lo) u without contraction (the reference recipe rounds the product, then the sum)
-__device__ __forceinline__ double gen_lerp(double lo, double hi, double u)
-{
-    return hi > lo ? __dadd_rn(lo, __dmul_rn(__dsub_rn(hi, lo), u)) : lo;
-}
-__device__ __forceinline__ void gen_unit(double uz, double uphi, double (&v)[3])
-{
-    const double z = __dsub_rn(__dmul_rn(2.0, uz), 1.0);
-    const double phi = __dmul_rn(2.0 * 3.14159265358979323846, uphi);
-    const double r = sqrt(fmax(0.0, __dsub_rn(1.0, __dmul_rn(z, z))));
-    double s, c;
-    sincos(phi, &s, &c);
-    v[0] = __dmul_rn(r, c); v[1] = __dmul_rn(r, s); v[2] = z;
-}
-
-struct GenSpec {           // device copy of pn_ensemble
-    unsigned long long key0, key1;
-    double omega0, q_lo, q_hi, m1_fixed, chi1_lo, chi1_hi, chi2_lo, chi2_hi, s1_tilt_deg;
-};
+#include "pn_gen.cuh"
 
 template <bool SHARE>
 __global__ void __launch_bounds__(GEN_TILE) pn_generate_kernel(const GenSpec* __restrict__ specs, long long n_total,
@@ -79,26 +59,11 @@ __global__ void __launch_bounds__(GEN_TILE) pn_generate_kernel(const GenSpec* __
             if (SHARE) u[k] = (double)(words[((t >> 2) * 7 + k) * 4 + (t & 3)] >> 11) * (1.0 / 9007199254740992.0);
             else u[k] = gen_uniform(sp.key0, sp.key1, (unsigned long long)k * N + i);
         }
-        const double q = gen_lerp(sp.q_lo, sp.q_hi, u[0]);
-        const double chi1 = gen_lerp(sp.chi1_lo, sp.chi1_hi, u[1]);
-        const double chi2 = gen_lerp(sp.chi2_lo, sp.chi2_hi, u[2]);
-        double s1[3], s2[3];
-        gen_unit(u[3], u[4], s1);
-        gen_unit(u[5], u[6], s2);
-        double m1, m2;
-        if (sp.m1_fixed > 0.0) { m1 = sp.m1_fixed; m2 = __dsub_rn(1.0, m1); }
-        else { const double d = __dadd_rn(1.0, q); m1 = __ddiv_rn(1.0, d); m2 = __ddiv_rn(q, d); }
-        if (sp.s1_tilt_deg >= 0.0) {
-            const double th = __dmul_rn(sp.s1_tilt_deg, 3.14159265358979323846 / 180.0);
-            sincos(th, &s1[0], &s1[2]);
-            s1[1] = 0.0;
-        }
-        const double a1 = __dmul_rn(__dmul_rn(chi1, m1), m1), a2 = __dmul_rn(__dmul_rn(chi2, m2), m2);
+        double yy[10], m1, m2;
+        gen_system(sp, u, yy, m1, m2);
         double* y = tile_y + t * 10;
-        y[0] = sp.omega0;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) { y[1 + c] = __dmul_rn(a1, s1[c]); y[4 + c] = __dmul_rn(a2, s2[c]); }
-        y[7] = 0.0; y[8] = 0.0; y[9] = 1.0;
+        for (int c = 0; c < 10; ++c) y[c] = yy[c];
         tile_m[2 * t] = m1; tile_m[2 * t + 1] = m2;
     }
     // generic-proxy writes -> visible to the async proxy, then one bulk store per array by one thread

@@ -7,13 +7,16 @@
 // cost only the short refill section.  All state (y, k1..k7, per-system constants) lives in
 // registers; global memory is touched only at refill and at finish.  (DESIGN.md 2, 7.)
 #include "pn_step_common.cuh"
+#include "pn_dots.cuh"
+#include "pn_gen.cuh"
+#include "pn_moments.cuh"
 
 // E^2 of the scaled RMS error norm, returned in FP32 (see the call site).
 __device__ __forceinline__ float pn_err_norm2(const double (&y)[10], const double (&ynew)[10], const double (&err)[10],
                                               float rtol, float atol1, float atS1, float atS2)
 {
     const double rt = (double)rtol;
-    double sum = 0.0;
+    double sum = 0.0, sum1 = 0.0;          // two accumulators: the ten dependent FMAs were a 10-deep chain at the end of a step
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         const double at = (double)((i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1));
@@ -23,9 +26,9 @@ __device__ __forceinline__ float pn_err_norm2(const double (&y)[10], const doubl
         double r;
         asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(sc));
         const double q = err[i] * r;
-        sum = fma(q, q, sum);
+        if (i & 1) sum1 = fma(q, q, sum1); else sum = fma(q, q, sum);
     }
-    return (float)(sum * 0.1);
+    return (float)((sum + sum1) * 0.1);
 }
 __device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float (&ynew)[10], const float (&err)[10],
                                               float rtol, float atol1, float atS1, float atS2)
@@ -49,6 +52,43 @@ __device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float 
 // PN_REC reals per system (FP64 320 B, FP32 160 B), so a lane's refill is 20 (10) 16-byte loads.
 //   [0..9] y0   [10..19] K1 = h0 f(y0)   [20..34] PnConsts   [35..37] PnBase   [38] atol |S1|   [39] atol |S2|
 // A record with [38] < 0 marks a system the seed kernel has already failed (bad input).
+// The seed record of one valid system: constants, base powers, K1 = h0 f(y0), norm-scaled atol (layout above).
+template <typename real>
+__device__ __forceinline__ void pn_make_record(const double (&y0)[10], double m1, double m2, const PnKernelParams& p, real (&out)[PN_REC])
+{
+    real y[10], k1[10];
+#pragma unroll
+    for (int j = 0; j < 10; ++j) y[j] = (real)y0[j];
+    PnConsts<real> c;
+    PnBase<real> base;
+    PnUni<real> u;
+    pn_make_uni<real>(p.mask, u);
+    u.emax = (real)p.emax;
+    pn_make_consts<real>(m1, m2, p.mask, c);
+    pn_base_init(c.M * y[0], base);
+    const real h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;      // first step (DESIGN.md 3, R13); same expression at refill
+    real r_tmp, l_tmp;
+    bool bad_tmp = false;
+    PnScaled<real> sc;
+    pn_make_scaled(c, h, sc);
+    pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad_tmp);      // K1 = h0 f(y0)
+    // atol scaled by the conserved spin norms (DESIGN.md 3, R7)
+    const double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
+    const double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
+#pragma unroll
+    for (int j = 0; j < 10; ++j) {
+        // rec_pairs: the pair-packed FP32 kernel wants each register pair as two adjacent, 8-byte aligned words
+        const int pos = p.rec_pairs ? 2 * PN_PAIR_OF[j] + PN_PAIR_HALF[j] : j;
+        out[pos] = y[j]; out[10 + pos] = k1[j];
+    }
+    out[20] = c.M; out[21] = c.c2; out[22] = c.c4; out[23] = c.c5; out[24] = c.c6; out[25] = c.c7;
+    out[26] = c.p1; out[27] = c.p2; out[28] = c.q1; out[29] = c.q2; out[30] = c.K0; out[31] = c.A1;
+    out[32] = c.A2; out[33] = c.Bc; out[34] = c.G;
+    out[35] = base.r0; out[36] = base.r03; out[37] = base.l0;
+    out[38] = (real)(p.atol * (s1 > 0.0 ? s1 : 1.0));
+    out[39] = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
+}
+
 template <typename real>
 __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
 {
@@ -94,35 +134,8 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
         return;
     }
     if (m1 != p.masses[0] || m2 != p.masses[p.n]) *p.nonuniform = 1;      // benign race: every writer stores 1
-    PnConsts<real> c;
-    PnBase<real> base;
-    PnUni<real> u;
-    pn_make_uni<real>(p.mask, u);
-    u.emax = (real)p.emax;
-    pn_make_consts<real>(m1, m2, p.mask, c);
-    pn_base_init(c.M * y[0], base);
-    const real h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;      // first step (DESIGN.md 3, R13); same expression at refill
-    real r_tmp, l_tmp;
-    bool bad_tmp = false;
-    PnScaled<real> sc;
-    pn_make_scaled(c, h, sc);
-    pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad_tmp);      // K1 = h0 f(y0)
-    // atol scaled by the conserved spin norms (DESIGN.md 3, R7)
-    const double s1 = sqrt(y0[1] * y0[1] + y0[2] * y0[2] + y0[3] * y0[3]);
-    const double s2 = sqrt(y0[4] * y0[4] + y0[5] * y0[5] + y0[6] * y0[6]);
     real out[PN_REC];
-#pragma unroll
-    for (int j = 0; j < 10; ++j) {
-        // rec_pairs: the pair-packed FP32 kernel wants each register pair as two adjacent, 8-byte aligned words
-        const int pos = p.rec_pairs ? 2 * PN_PAIR_OF[j] + PN_PAIR_HALF[j] : j;
-        out[pos] = y[j]; out[10 + pos] = k1[j];
-    }
-    out[20] = c.M; out[21] = c.c2; out[22] = c.c4; out[23] = c.c5; out[24] = c.c6; out[25] = c.c7;
-    out[26] = c.p1; out[27] = c.p2; out[28] = c.q1; out[29] = c.q2; out[30] = c.K0; out[31] = c.A1;
-    out[32] = c.A2; out[33] = c.Bc; out[34] = c.G;
-    out[35] = base.r0; out[36] = base.r03; out[37] = base.l0;
-    out[38] = (real)(p.atol * (s1 > 0.0 ? s1 : 1.0));
-    out[39] = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
+    pn_make_record<real>(y0, m1, m2, p, out);
     using vec = typename PnVec<real>::type;           // 16-byte stores
     vec* dst = (vec*)rec;
     constexpr int W = 16 / (int)sizeof(real);
@@ -144,7 +157,103 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
 // kernel (p.uni_slot >= 0 marks such a pair); each looks at the seed kernel's verdict and the one that does not apply
 // returns at once, so no host synchronisation is needed and async calls keep the fast path.
 __constant__ double pn_uni_table[PN_UNI_SLOTS][16];
-template <typename real, int BLOCK, int MINB, bool SLOW, bool MIXED = false, int UNI = -1>
+
+// ---- fused ensemble mode (FUSED = true; pn_run_ensembles): seed in, statistics out ----------------
+// The work pull DRAWS the system (counter-based Philox + sphere sampling, pn_gen.cuh: the same bits as pn_generate)
+// instead of loading it, and a finished system is folded into the ensemble statistics instead of being stored, so the
+// launch reads and writes no state arrays at all.  To keep the draw off the divergent path (one lane working, 31
+// waiting: ~2000 instructions for the Philox blocks, the two sincos, the per-system constants and the seed slope),
+// a warp draws 32 systems AT ONCE, one per lane, into a shared-memory ring ([word][slot], conflict-free), and lanes
+// whose inspiral has finished pop records off the ring; the global queue counter is advanced by 32 per draw.
+// Statistics: every thread keeps Welford moments (n, xbar, ybar, M2x, M2y, Cxy) of its own finished systems per dot
+// product in shared memory, for ONE ensemble at a time (queue order is index order, so a thread's ensembles never
+// decrease); when its ensemble changes and at kernel exit they are merged into the ensemble's global record with the
+// pairwise update under a per-ensemble spin lock (try-lock loop, safe under intra-warp contention).  Histogram counts
+// go straight to global memory with integer atomics (one per finished system and dot product).  Counts are exact and
+// reproducible; moments are reproducible to rounding (the merge order depends on timing).
+#define PN_FREC (PN_REC + 4)      /* ring record: seed record + the three initial unit dot products (+ pad) */
+template <int BLOCK> struct PnFusedSmem {
+    static constexpr int NW = BLOCK / 32;
+    double* ring;     // [NW][PN_FREC][32]
+    double* xin;      // [3][BLOCK]      initial unit dot products of the lane's current system (NaN: undefined)
+    double* acc;      // [3][6][BLOCK]   per-thread moments
+    int* ring_idx;    // [NW][32]
+    int* acc_g;       // [BLOCK]         ensemble the thread's moments belong to, -1: none
+    static constexpr size_t bytes() { return sizeof(double) * ((size_t)NW * PN_FREC * 32 + 3 * BLOCK + 18 * BLOCK) + sizeof(int) * (NW * 32 + BLOCK); }
+    __device__ explicit PnFusedSmem(unsigned char* base)
+    {
+        ring = reinterpret_cast<double*>(base);
+        xin = ring + (size_t)NW * PN_FREC * 32;
+        acc = xin + 3 * BLOCK;
+        ring_idx = reinterpret_cast<int*>(acc + 18 * BLOCK);
+        acc_g = ring_idx + NW * 32;
+    }
+};
+
+// merge this thread's moments (acc[(k*6 + c)*BLOCK], already offset by the thread index) into ensemble g's record
+template <int BLOCK>
+__device__ __noinline__ void pn_fused_flush(const PnKernelParams& p, double* acc, int g)
+{
+    bool done = false;
+    while (!done) {                                   // try-lock loop: a lane that fails simply tries again next round
+        if (atomicCAS(p.f_lock + g, 0, 1) == 0) {
+            __threadfence();
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                StMom a = {acc[(k * 6 + 0) * BLOCK], acc[(k * 6 + 1) * BLOCK], acc[(k * 6 + 2) * BLOCK],
+                           acc[(k * 6 + 3) * BLOCK], acc[(k * 6 + 4) * BLOCK], acc[(k * 6 + 5) * BLOCK]};
+                if (a.n > 0.0) {
+                    volatile double* q = p.f_mom + ((size_t)g * 3 + k) * 6;
+                    StMom m = {q[0], q[1], q[2], q[3], q[4], q[5]};
+                    st_merge(m, a);
+                    q[0] = m.n; q[1] = m.mx; q[2] = m.my; q[3] = m.m2x; q[4] = m.m2y; q[5] = m.cxy;
+                }
+            }
+            __threadfence();
+            atomicExch(p.f_lock + g, 0);
+            done = true;
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 18; ++j) acc[j * BLOCK] = 0.0;
+}
+
+// a finished system of the fused mode: final unit dot products -> the thread's moments and the global histograms
+template <int BLOCK>
+__device__ __noinline__ void pn_fused_finish(const PnKernelParams& p, const PnFusedSmem<BLOCK>& fs, int idx, int code, const double (&v9)[9])
+{
+    const long long gsys = p.f_base + idx;
+    const int g = (int)(gsys / p.f_count);
+    const int tid = threadIdx.x;
+    if (code <= 0) {                                  // failed: left out of all three statistics
+#pragma unroll
+        for (int k = 0; k < 3; ++k) atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull);
+        return;
+    }
+    double df[3];
+    bool okf[3];
+    pn_unit_dots(v9, df, okf);
+    double* acc = fs.acc + tid;
+    if (fs.acc_g[tid] != g) {
+        if (fs.acc_g[tid] >= 0) pn_fused_flush<BLOCK>(p, acc, fs.acc_g[tid]);
+        fs.acc_g[tid] = g;
+    }
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {
+        const double x = fs.xin[k * BLOCK + tid];
+        if (!(okf[k] && x == x)) { atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull); continue; }
+        StMom a = {acc[(k * 6 + 0) * BLOCK], acc[(k * 6 + 1) * BLOCK], acc[(k * 6 + 2) * BLOCK],
+                   acc[(k * 6 + 3) * BLOCK], acc[(k * 6 + 4) * BLOCK], acc[(k * 6 + 5) * BLOCK]};
+        st_add(a, x, df[k]);
+        acc[(k * 6 + 0) * BLOCK] = a.n; acc[(k * 6 + 1) * BLOCK] = a.mx; acc[(k * 6 + 2) * BLOCK] = a.my;
+        acc[(k * 6 + 3) * BLOCK] = a.m2x; acc[(k * 6 + 4) * BLOCK] = a.m2y; acc[(k * 6 + 5) * BLOCK] = a.cxy;
+        if (p.f_hist1) atomicAdd(p.f_hist1 + ((size_t)g * 3 + k) * p.f_bins1 + pn_bin_of(df[k], p.f_bins1), 1ull);
+        if (p.f_hist2)
+            atomicAdd(p.f_hist2 + (((size_t)g * 3 + k) * p.f_bins2 + pn_bin_of(x, p.f_bins2)) * p.f_bins2 + pn_bin_of(df[k], p.f_bins2), 1ull);
+    }
+}
+
+template <typename real, int BLOCK, int MINB, bool SLOW, bool MIXED = false, int UNI = -1, bool FUSED = false>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(const PnKernelParams p)
 {
     if (UNI >= 0) { if (*p.nonuniform != 0) return; }
@@ -154,6 +263,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     if (SLOW && n_queue == 0u) return;
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+    extern __shared__ __align__(16) unsigned char pn_fused_smem[];
+    PnFusedSmem<BLOCK> fs(pn_fused_smem);                 // FUSED only (no dynamic shared memory otherwise)
+    unsigned ring_used = 0, ring_count = 0;               // warp-uniform: records popped / drawn in the current batch
+    if constexpr (FUSED) {
+#pragma unroll
+        for (int j = 0; j < 18; ++j) fs.acc[j * BLOCK + threadIdx.x] = 0.0;
+        fs.acc_g[threadIdx.x] = -1;
+    }
 
     // lane state.  k1 holds the SCALED slope h*f(y).  Idle lanes are frozen (h = 0, k1 = 0) on a benign
     // dummy state, so the lock-step arithmetic stays finite and never leaves the series' range.
@@ -188,7 +305,72 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     const real om_tol = (real)(p.tau * p.omegaf);
     const float rtol = (float)p.rtol, atol1 = fmaxf((float)p.atol, 1e-30f);
 
+    // a lane starts the system whose seed record is rec
+    auto start_system = [&](const real (&rec)[PN_REC], int i) {
+#pragma unroll
+        for (int j = 0; j < 10; ++j) { y[j] = rec[j]; k1[j] = rec[10 + j]; }
+        if constexpr (UNI < 0) {
+            c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
+            c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
+            c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
+        }
+        base.r0 = rec[35]; base.r03 = rec[36]; base.l0 = rec[37];
+        atS1 = fmaxf((float)rec[38], 1e-30f); atS2 = fmaxf((float)rec[39], 1e-30f);   // keeps every scale > 0 (atol = 0 is allowed)
+        t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
+        idx = i;
+        h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;
+    };
+
     for (;;) {
+        if constexpr (FUSED) {
+            // ---------------- fused refill: draw 32 systems per warp into the ring, idle lanes pop ----------------
+            if (__any_sync(FULL, idx < 0) && !(queue_empty && ring_used >= ring_count)) {
+                double* ring_w = fs.ring + (size_t)(threadIdx.x >> 5) * PN_FREC * 32;
+                int* ring_idx_w = fs.ring_idx + (threadIdx.x >> 5) * 32;
+                if (ring_used >= ring_count) {
+                    unsigned qb = 0;
+                    if (lane == 0) qb = atomicAdd(SLOW ? p.queue2 : p.queue, 32u);
+                    qb = __shfl_sync(FULL, qb, 0);
+                    ring_used = 0u;
+                    ring_count = qb < n_queue ? min(32u, n_queue - qb) : 0u;
+                    if (qb + 32u >= n_queue) queue_empty = true;
+                    if ((unsigned)lane < ring_count) {
+                        const int i = order ? order[qb + lane] : (int)(qb + lane);
+                        const long long gsys = p.f_base + i;
+                        const long long e = gsys / p.f_count;
+                        const GenSpec sp = ((const GenSpec*)p.f_specs)[e];
+                        double y0[10], m1, m2;
+                        gen_system_at(sp, (unsigned long long)p.f_n_total, (unsigned long long)(p.f_first + (gsys - e * p.f_count)), y0, m1, m2);
+                        real rec[PN_REC];
+                        pn_make_record<real>(y0, m1, m2, p, rec);
+#pragma unroll
+                        for (int j = 0; j < PN_REC; ++j) ring_w[j * 32 + lane] = (double)rec[j];
+                        const double v9[9] = {y0[1], y0[2], y0[3], y0[4], y0[5], y0[6], y0[7], y0[8], y0[9]};
+                        double d0[3];
+                        bool ok0[3];
+                        pn_unit_dots(v9, d0, ok0);
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) ring_w[(PN_REC + k) * 32 + lane] = ok0[k] ? d0[k] : nan("");
+                        ring_idx_w[lane] = i;
+                    }
+                    __syncwarp();
+                }
+                const unsigned need = __ballot_sync(FULL, idx < 0);
+                const unsigned avail = ring_count - ring_used;
+                const unsigned rank = (unsigned)__popc(need & ((1u << lane) - 1u));
+                if (idx < 0 && rank < avail) {
+                    const unsigned slot = ring_used + rank;
+                    real rec[PN_REC];
+#pragma unroll
+                    for (int j = 0; j < PN_REC; ++j) rec[j] = (real)ring_w[j * 32 + slot];
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) fs.xin[k * BLOCK + threadIdx.x] = ring_w[(PN_REC + k) * 32 + slot];
+                    start_system(rec, ring_idx_w[slot]);
+                }
+                ring_used += min((unsigned)__popc(need), avail);
+                __syncwarp();
+            }
+        } else
         // ---------------- refill: lanes without a system pull the next queue entries ----------------
         if (!queue_empty && __any_sync(FULL, idx < 0)) {
             const unsigned wm = __ballot_sync(FULL, idx < 0);
@@ -207,27 +389,16 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                         // bad input: already failed and stored by the seed kernel; the lane stays frozen and
                         // asks again next iteration
                     } else {
-#pragma unroll
-                        for (int j = 0; j < 10; ++j) { y[j] = rec[j]; k1[j] = rec[10 + j]; }
                         if constexpr (MIXED)
 #pragma unroll
                             for (int j = 0; j < 10; ++j) yd[j] = __ldg(p.y0 + (size_t)j * p.n + i);
-                        if constexpr (UNI < 0) {
-                            c.M = rec[20]; c.c2 = rec[21]; c.c4 = rec[22]; c.c5 = rec[23]; c.c6 = rec[24]; c.c7 = rec[25];
-                            c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
-                            c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
-                        }
-                        base.r0 = rec[35]; base.r03 = rec[36]; base.l0 = rec[37];
-                        atS1 = fmaxf((float)rec[38], 1e-30f); atS2 = fmaxf((float)rec[39], 1e-30f);   // keeps every scale > 0 (atol = 0 is allowed)
-                        t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
-                        idx = i;
-                        h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;
+                        start_system(rec, i);
                     }
                 }
             }
         }
         if (__all_sync(FULL, idx < 0)) {
-            if (queue_empty) break;
+            if (queue_empty && (!FUSED || ring_used >= ring_count)) break;
             continue;                        // only bad-input lanes were drawn: ask again
         }
 
@@ -306,7 +477,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         code = !finite ? PN_F_NONFINITE : code;
         code = active ? code : 0;
         if (code != 0) {
-            if constexpr (MIXED) {
+            if constexpr (FUSED) {
+                double v9[9];
+#pragma unroll
+                for (int i = 0; i < 9; ++i) v9[i] = (double)(accept ? ynew[i + 1] : y[i + 1]);
+                pn_fused_finish<BLOCK>(p, fs, idx, code, v9);
+            } else if constexpr (MIXED) {
                 double yo[10];
 #pragma unroll
                 for (int i = 0; i < 10; ++i) yo[i] = accept ? yd[i] + (double)dy[i] : yd[i];
@@ -339,6 +515,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         h *= ratio;
     }
 
+    if constexpr (FUSED) {
+        // the thread's moments go to its last ensemble's record
+        if (fs.acc_g[threadIdx.x] >= 0) pn_fused_flush<BLOCK>(p, fs.acc + threadIdx.x, fs.acc_g[threadIdx.x]);
+    }
     // ---------------- per-launch counters: warp reduce, one atomic per warp ----------------
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -431,6 +611,42 @@ static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cud
     if (grid < 1) grid = 1;
     kern<<<grid, BLOCK, 0, s>>>(p);
     ++g_pn_launches;
+    return cudaGetLastError();
+}
+
+// One chunk of a fused ensemble run: the fast kernel draws and integrates systems [p.f_base, p.f_base + p.n); the redo
+// pass re-draws and re-integrates those that left the range of the cbrt/log series (their chunk-local indices are in
+// p.redo_list).  p.queue, p.queue2, p.redo_count must be zero on entry.
+cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s)
+{
+    if (p.n <= 0) return cudaSuccess;
+    constexpr int BLOCK = 128, MINB = 2;
+    auto fast = pn_integrate_adaptive_kernel<double, BLOCK, MINB, false, false, -1, true>;
+    auto redo = pn_integrate_adaptive_kernel<double, BLOCK, MINB, true, false, -1, true>;
+    const int shm = (int)PnFusedSmem<BLOCK>::bytes();
+    static int grid_full[64] = {0};
+    int dev = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    int& gf = grid_full[dev & 63];
+    if (gf == 0) {
+        int sms = 0, per_sm = 0;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fast, cudaFuncAttributeMaxDynamicSharedMemorySize, shm)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(redo, cudaFuncAttributeMaxDynamicSharedMemorySize, shm)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fast, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(redo, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fast, BLOCK, shm)) != cudaSuccess) return e;
+        gf = sms * (per_sm < 1 ? 1 : per_sm);
+    }
+    int grid = grid_blocks > 0 ? grid_blocks : gf;
+    const long long need = ((long long)p.n + BLOCK - 1) / BLOCK;
+    if (need < grid) grid = (int)need;
+    if (grid < 1) grid = 1;
+    p.uni_slot = -1; p.order = nullptr;
+    fast<<<grid, BLOCK, shm, s>>>(p);
+    redo<<<grid, BLOCK, shm, s>>>(p);
+    g_pn_launches += 2;
     return cudaGetLastError();
 }
 

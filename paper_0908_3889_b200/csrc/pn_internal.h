@@ -35,12 +35,25 @@ struct PnKernelParams {
     unsigned int* order_scratch;    // [PN_ORDER_BUCKETS + 2]: bucket cursors, then the bit patterns of the smallest / largest key
     int* order_out;                 // [n]: the queue order the bucket sort writes (= order when keys != null)
     int rec_pairs;                  // FP32 seed records with y0 and K1 in the pair order of the pair-packed kernel (pn_rhs.cuh)
+    // ---- fused ensemble mode (pn_run_ensembles): seed in, statistics out, no state arrays ----
+    // queue position q of this launch <-> system g = f_base + q of the run; ensemble e = g / f_count, index inside the
+    // ensemble's variate stream j = f_first + g % f_count.  y0, masses, yf, steps, time, rejected, seed are unused.
+    const void* f_specs;            // device array of GenSpec (pn_gen.cuh), one per ensemble; null: not a fused launch
+    long long f_n_total, f_first, f_count, f_base;
+    double* f_mom;                  // [G][3][6] running moments n, xbar, ybar, M2x, M2y, Cxy (merged under f_lock[g])
+    int* f_lock;                    // [G] spin locks, zero-initialised
+    unsigned long long* f_skipped;  // [G][3]
+    unsigned long long* f_hist1;    // [G][3][bins1] or null
+    unsigned long long* f_hist2;    // [G][3][bins2][bins2] or null
+    int f_bins1, f_bins2;
 };
 
 // launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults
 // variant bits (pn_options.variant): 1 = always the generic FP64 kernel (per-lane constants), 2 = always the scalar FP32 kernel
 cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
                                 cudaStream_t s, int variant);
+// fused ensemble run (pn_integrate.cu): one chunk of systems [p.f_base, p.f_base + p.n); fast kernel + redo pass
+cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s);
 // pair-packed FP32 integrator (pn_integrate_packed.cu); the seed records must be float ones written with rec_pairs = 1
 cudaError_t pn_launch_integrate_packed(const PnKernelParams& p, int grid_blocks, cudaStream_t s);
 // staging + histogram + peak (pn_aux.cu)
@@ -58,6 +71,8 @@ cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch
 // ensemble statistics (pn_stats.cu)
 size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out);
 cudaError_t pn_launch_stats_merge(const double* parts, int n_parts, int n_groups, double* mom_out, double* r_out, cudaStream_t s);
+cudaError_t pn_launch_stats_norm(const unsigned long long* hist2, long long n_hists, int cells, unsigned long long* max_out,
+                                 double* norm_out, cudaStream_t s);
 cudaError_t pn_launch_stats(const double* init, const double* fin, const int* steps, long long n, long long group_size,
                             int bins1, int bins2, void* scratch, double* r_out, double* mom_out,
                             unsigned long long* skipped_out, unsigned long long* hist1, unsigned long long* hist2,

@@ -4,9 +4,10 @@
 //   x = M omega, v = x^{1/3};  everything that depends only on (m1, m2) is folded once per system into
 //   PnConsts, the brace of Eq. (1) becomes a Horner polynomial in v whose v^3, v^4 and v^6 coefficients
 //   carry the spin-orbit, spin-spin and log terms, and Eq. (4) collapses to
-//     Omega_1 = alpha1 L + beta S2,   alpha_i = A_i v^5 - 3 beta (L.S_j),  beta = x^2/(2 M^3)
-//     Omega_2 = alpha2 L + beta S1
-//   followed by the two cross products of Eq. (2) and L_dot = -v/(eta M^2) (S1_dot + S2_dot) of Eq. (3).
+//     Omega_1 = beta (gamma1 L + S2),   gamma_i = A_i x^{-1/3} - 3 (L.S_j),  beta = x^2/(2 M^3),
+//     Omega_2 = beta (gamma2 L + S1)    A_i = eta M^2 (4 + 3 m_j/m_i)
+//   followed by the two cross products of Eq. (2), c_i = (gamma_i L + S_j) x S_i, S_i_dot = beta c_i, and
+//   L_dot = -v/(eta M^2) beta (c_1 + c_2) of Eq. (3).
 // This file shares nothing with oracle/ (which evaluates the equations as printed).
 #pragma once
 #include <cuda_runtime.h>
@@ -33,7 +34,7 @@ struct PnConsts {
     real p1, p2;   // spin-orbit: v^3 coefficient += p1 (L.S1) + p2 (L.S2)
     real q1, q2;   // spin-spin:  v^4 coefficient += q1 (S1.S2) + q2 (L.S1)(L.S2)
     real K0;       // omega_dot = K0 v^11 brace,  K0 = 96 eta / (5 M^2)
-    real A1, A2;   // A_i = eta (4 + 3 m_j/m_i) / (2M)
+    real A1, A2;   // A_i = eta M^2 (4 + 3 m_j/m_i): Omega_i = beta (gamma_i L + S_j), gamma_i = A_i x^{-1/3} - 3 L.S_j
     real Bc;       // beta = Bc x^2,  Bc = 1/(2 M^3)
     real G;        // L_dot prefactor: -1/(eta M^2), times v
 };
@@ -84,8 +85,8 @@ __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned ma
     c.q1 = (real)(-on(4) * spin * 247.0 * eta / (48.0 * mm));
     c.q2 = (real)(on(4) * spin * 721.0 * eta / (48.0 * mm));
     c.K0 = (real)(96.0 * eta / (5.0 * M2));
-    c.A1 = (real)(eta * (4.0 + 3.0 * m2 / m1) / (2.0 * M));
-    c.A2 = (real)(eta * (4.0 + 3.0 * m1 / m2) / (2.0 * M));
+    c.A1 = (real)(eta * M2 * (4.0 + 3.0 * m2 / m1));
+    c.A2 = (real)(eta * M2 * (4.0 + 3.0 * m1 / m2));
     c.Bc = (real)(1.0 / (2.0 * M2 * M));
     c.G = (real)(-1.0 / (eta * M2));
 }
@@ -192,7 +193,7 @@ __device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float, 
     const float e = fmaf(-x * r0, r0 * r0, 1.0f);
     r0 = fmaf(r0 * e, 1.0f / 3.0f, r0);
     v = x * (r0 * r0);
-    r = 0.0f;
+    r = r0;
 }
 
 // packed FP32 (two systems per lane): the special-function unit is per component, the polish and the powers are packed
@@ -211,7 +212,7 @@ __device__ __forceinline__ void pn_powers(f2 x, const PnBase<f2>&, f2, f2& v, f2
     const f2 e = pn_fma(-(x * r0), r0 * r0, f2(1.0f));
     r0 = pn_fma(r0 * e, f2(1.0f / 3.0f), r0);
     v = x * (r0 * r0);
-    r = f2(0.0f);
+    r = r0;
 }
 
 // The slopes are produced already multiplied by the step size h ("scaled slopes" K = h f): the four
@@ -220,11 +221,11 @@ __device__ __forceinline__ void pn_powers(f2 x, const PnBase<f2>&, f2, f2& v, f2
 // (constant-bank operands) instead of per-lane h*a_sj registers.  This matters on sm_100a because a DFMA
 // with three distinct register sources issues every 3 cycles, one with two every 2 (measured,
 // DESIGN.md 7.2).
-template <typename real> struct PnScaled { real hK0, hA1, hA2, hBc; };
+template <typename real> struct PnScaled { real hK0, hBc; };
 template <typename real>
 __device__ __forceinline__ void pn_make_scaled(const PnConsts<real>& c, real h, PnScaled<real>& s)
 {
-    s.hK0 = h * c.K0; s.hA1 = h * c.A1; s.hA2 = h * c.A2; s.hBc = h * c.Bc;
+    s.hK0 = h * c.K0; s.hBc = h * c.Bc;
 }
 
 // K = h f(y).  ~70 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and
@@ -238,7 +239,8 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     real v, lnx, r;
     pn_powers<SLOW>(x, base, u.emax, v, lnx, r, bad);
     r_out = r; lnx_out = lnx;
-    const real v2 = v * v, v4 = v2 * v2, v5 = v4 * v, x2 = x * x;
+    // x^{2/3} straight from r = x^{-1/3} (one multiply after r, not two): the powers are ready earlier in the chain
+    const real x2 = x * x, v2 = x * r, v4 = v2 * v2, v5 = v4 * v;
 
     const real S1x = y[1], S1y = y[2], S1z = y[3];
     const real S2x = y[4], S2y = y[5], S2z = y[6];
@@ -248,46 +250,40 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     const real LS2 = pn_fma(Lx, S2x, pn_fma(Ly, S2y, Lz * S2z));
     const real S12 = pn_fma(S1x, S2x, pn_fma(S1y, S2y, S1z * S2z));
 
-    // Eq. (1): Horner in v; coefficients of v^3, v^4, v^6 carry the spin-orbit, spin-spin, log pieces
+    // Eq. (1): coefficients of v^3, v^4, v^6 carry the spin-orbit, spin-spin, log pieces
     const real k3 = pn_fma(c.p1, LS1, pn_fma(c.p2, LS2, u.c3));
     const real k4 = pn_fma(c.q1, S12, pn_fma(c.q2 * LS1, LS2, c.c4));
     const real k6 = pn_fma(u.cl, lnx, c.c6);
-#ifndef PN_HORNER
     // Estrin form, brace = c0 + v2 (c2 + k3 v) + v4 ((k4 + c5 v) + v2 (k6 + c7 v)): the same six FMAs as Horner's
     // rule in a dependency chain of three instead of six
     const real e67 = pn_fma(c.c7, v, k6), e45 = pn_fma(c.c5, v, k4), e23 = pn_fma(k3, v, c.c2);
     const real hi = pn_fma(e67, v2, e45);
     real B = pn_fma(e23, v2, u.c0);
     B = pn_fma(hi, v4, B);
-#else
-    real B = pn_fma(c.c7, v, k6);
-    B = pn_fma(B, v, c.c5);
-    B = pn_fma(B, v, k4);
-    B = pn_fma(B, v, k3);
-    B = pn_fma(B, v, c.c2);
-    B = pn_fma(B, v2, u.c0);
-#endif
     f[0] = (sc.hK0 * (v5 * x2)) * B;
 
-    // Eq. (4): h Omega_1 = al1 L + beta S2,  h Omega_2 = al2 L + beta S1
+    // Eq. (4) over beta = h x^2/(2M^3): Omega_1/beta = gamma1 L + S2, Omega_2/beta = gamma2 L + S1.  gamma_i needs only
+    // r and a dot product, so the cross products below do not wait for the powers of v; -3 is an immediate operand, so
+    // the two FMAs read two registers (a DFMA with three register sources issues every 3 cycles).
+    const real g1 = pn_fma((real)-3.0, LS2, c.A1 * r);
+    const real g2 = pn_fma((real)-3.0, LS1, c.A2 * r);
+    const real O1x = pn_fma(g1, Lx, S2x), O1y = pn_fma(g1, Ly, S2y), O1z = pn_fma(g1, Lz, S2z);
+    const real O2x = pn_fma(g2, Lx, S1x), O2y = pn_fma(g2, Ly, S1y), O2z = pn_fma(g2, Lz, S1z);
+    // Eq. (2): S_i_dot = beta (Omega_i/beta) x S_i
+    const real c1x = pn_fma(O1y, S1z, -(O1z * S1y));
+    const real c1y = pn_fma(O1z, S1x, -(O1x * S1z));
+    const real c1z = pn_fma(O1x, S1y, -(O1y * S1x));
+    const real c2x = pn_fma(O2y, S2z, -(O2z * S2y));
+    const real c2y = pn_fma(O2z, S2x, -(O2x * S2z));
+    const real c2z = pn_fma(O2x, S2y, -(O2y * S2x));
     const real beta = sc.hBc * x2;
-    const real b3 = (real)3.0 * beta;
-    const real al1 = pn_fma(-b3, LS2, sc.hA1 * v5);
-    const real al2 = pn_fma(-b3, LS1, sc.hA2 * v5);
-    const real O1x = pn_fma(beta, S2x, al1 * Lx), O1y = pn_fma(beta, S2y, al1 * Ly), O1z = pn_fma(beta, S2z, al1 * Lz);
-    const real O2x = pn_fma(beta, S1x, al2 * Lx), O2y = pn_fma(beta, S1y, al2 * Ly), O2z = pn_fma(beta, S1z, al2 * Lz);
-    // Eq. (2): S_i_dot = Omega_i x S_i
-    f[1] = pn_fma(O1y, S1z, -(O1z * S1y));
-    f[2] = pn_fma(O1z, S1x, -(O1x * S1z));
-    f[3] = pn_fma(O1x, S1y, -(O1y * S1x));
-    f[4] = pn_fma(O2y, S2z, -(O2z * S2y));
-    f[5] = pn_fma(O2z, S2x, -(O2x * S2z));
-    f[6] = pn_fma(O2x, S2y, -(O2y * S2x));
-    // Eq. (3)
-    const real g = c.G * v;
-    f[7] = g * (f[1] + f[4]);
-    f[8] = g * (f[2] + f[5]);
-    f[9] = g * (f[3] + f[6]);
+    f[1] = beta * c1x; f[2] = beta * c1y; f[3] = beta * c1z;
+    f[4] = beta * c2x; f[5] = beta * c2y; f[6] = beta * c2z;
+    // Eq. (3): L_dot = -v/(eta M^2) (S1_dot + S2_dot) = (G v beta) (c_1 + c_2)
+    const real gb = (c.G * v) * beta;
+    f[7] = gb * (c1x + c2x);
+    f[8] = gb * (c1y + c2y);
+    f[9] = gb * (c1z + c2z);
 }
 
 // ---- pair-packed FP32 layout (pn_integrate_packed.cu) -------------------------------------------------------------
@@ -312,7 +308,7 @@ __device__ __forceinline__ void pn_rhs(const f2 (&y)[5], const PnConsts<float>& 
     float v, lnx, r;
     pn_powers<SLOW>(x, base, u.emax, v, lnx, r, bad);
     r_out = r; lnx_out = lnx;
-    const float v2 = v * v, v4 = v2 * v2, v5 = v4 * v, x2 = x * x;
+    const float x2 = x * x, v2 = x * r, v4 = v2 * v2, v5 = v4 * v;
 
     const float S1x = y[0].v.x, S1y = y[0].v.y, S1z = y[3].v.y;
     const float S2x = y[1].v.x, S2y = y[1].v.y, S2z = y[4].v.x;
@@ -331,26 +327,26 @@ __device__ __forceinline__ void pn_rhs(const f2 (&y)[5], const PnConsts<float>& 
     B = fmaf(hi, v4, B);
     const float f0 = (sc.hK0 * (v5 * x2)) * B;
 
-    // Eq. (4): h Omega_1 = al1 L + beta S2,  h Omega_2 = al2 L + beta S1; x and y components packed
+    // Eq. (4) over beta: Omega_i/beta = gamma_i L + S_j; x and y components packed
+    const float g1 = fmaf(-3.0f, LS2, c.A1 * r);
+    const float g2 = fmaf(-3.0f, LS1, c.A2 * r);
+    const f2 O1 = pn_fma(f2(g1), y[2], y[1]);
+    const f2 O2 = pn_fma(f2(g2), y[2], y[0]);
+    const float O1z = fmaf(g1, Lz, S2z), O2z = fmaf(g2, Lz, S1z);
+    // Eq. (2): S_i_dot = beta (Omega_i/beta) x S_i
+    const float c1x = fmaf(O1.v.y, S1z, -(O1z * S1y));
+    const float c1y = fmaf(O1z, S1x, -(O1.v.x * S1z));
+    const float c1z = fmaf(O1.v.x, S1y, -(O1.v.y * S1x));
+    const float c2x = fmaf(O2.v.y, S2z, -(O2z * S2y));
+    const float c2y = fmaf(O2z, S2x, -(O2.v.x * S2z));
+    const float c2z = fmaf(O2.v.x, S2y, -(O2.v.y * S2x));
     const float beta = sc.hBc * x2;
-    const float b3 = 3.0f * beta;
-    const float al1 = fmaf(-b3, LS2, sc.hA1 * v5);
-    const float al2 = fmaf(-b3, LS1, sc.hA2 * v5);
-    const f2 O1 = pn_fma(f2(beta), y[1], f2(al1) * y[2]);
-    const f2 O2 = pn_fma(f2(beta), y[0], f2(al2) * y[2]);
-    const float O1z = fmaf(beta, S2z, al1 * Lz), O2z = fmaf(beta, S1z, al2 * Lz);
-    // Eq. (2): S_i_dot = Omega_i x S_i
-    const float f1 = fmaf(O1.v.y, S1z, -(O1z * S1y));
-    const float f2v = fmaf(O1z, S1x, -(O1.v.x * S1z));
-    const float f3 = fmaf(O1.v.x, S1y, -(O1.v.y * S1x));
-    const float f4 = fmaf(O2.v.y, S2z, -(O2z * S2y));
-    const float f5 = fmaf(O2z, S2x, -(O2.v.x * S2z));
-    const float f6 = fmaf(O2.v.x, S2y, -(O2.v.y * S2x));
+    const f2 c1(c1x, c1y), c2(c2x, c2y);
     // Eq. (3)
-    const float g = c.G * v;
-    f[0] = f2(f1, f2v);
-    f[1] = f2(f4, f5);
-    f[2] = f2(g) * (f[0] + f[1]);
-    f[3] = f2(f0, f3);
-    f[4] = f2(f6, g * (f3 + f6));
+    const float gb = (c.G * v) * beta;
+    f[0] = f2(beta) * c1;
+    f[1] = f2(beta) * c2;
+    f[2] = f2(gb) * (c1 + c2);
+    f[3] = f2(f0, beta * c1z);
+    f[4] = f2(beta * c2z, gb * (c1z + c2z));
 }

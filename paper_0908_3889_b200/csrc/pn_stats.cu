@@ -16,6 +16,7 @@
 #include <cstdint>
 #include "pn_internal.h"
 #include "pn_dots.cuh"
+#include "pn_moments.cuh"
 
 #define ST_TILE 256
 #define ST_STAGES 2      /* one ring slot per consumer group (see pn_stats_kernel) */
@@ -47,35 +48,6 @@ __device__ __forceinline__ void st_mbar_wait(uint32_t bar, uint32_t parity)
                      : "r"(bar), "r"(parity)
                      : "memory");
     } while (!ok);
-}
-
-// ---- moments ----------------------------------------------------------------------------------------------
-struct StMom { double n, mx, my, m2x, m2y, cxy; };
-
-// Chan et al. pairwise update: merge b into a
-__device__ __forceinline__ void st_merge(StMom& a, const StMom& b)
-{
-    const double n = a.n + b.n;
-    if (n == 0.0) return;
-    const double dx = b.mx - a.mx, dy = b.my - a.my;
-    const double w = a.n * b.n / n, f = b.n / n;
-    a.m2x += b.m2x + dx * dx * w;
-    a.m2y += b.m2y + dy * dy * w;
-    a.cxy += b.cxy + dx * dy * w;
-    a.mx = (b.n == 0.0) ? a.mx : ((a.n == 0.0) ? b.mx : a.mx + dx * f);
-    a.my = (b.n == 0.0) ? a.my : ((a.n == 0.0) ? b.my : a.my + dy * f);
-    a.n = n;
-}
-__device__ __forceinline__ StMom st_shfl_xor(const StMom& a, int o)
-{
-    StMom r;
-    r.n = __shfl_xor_sync(0xffffffffu, a.n, o);
-    r.mx = __shfl_xor_sync(0xffffffffu, a.mx, o);
-    r.my = __shfl_xor_sync(0xffffffffu, a.my, o);
-    r.m2x = __shfl_xor_sync(0xffffffffu, a.m2x, o);
-    r.m2y = __shfl_xor_sync(0xffffffffu, a.m2y, o);
-    r.cxy = __shfl_xor_sync(0xffffffffu, a.cxy, o);
-    return r;
 }
 
 // per-thread running sums of (x - x0), (y - y0) about the thread's first sample of the group
@@ -331,6 +303,15 @@ __global__ void __launch_bounds__(256) pn_stats_norm_kernel(const unsigned long 
         for (int c = threadIdx.x; c < cells; c += 256)
             norm_out[(size_t)blockIdx.x * cells + c] = mx ? (double)h[c] / (double)mx : 0.0;    // correctly rounded quotient
     }
+}
+
+cudaError_t pn_launch_stats_norm(const unsigned long long* hist2, long long n_hists, int cells, unsigned long long* max_out,
+                                 double* norm_out, cudaStream_t s)
+{
+    if (n_hists <= 0) return cudaSuccess;
+    pn_stats_norm_kernel<<<(unsigned)n_hists, 256, 0, s>>>(hist2, cells, max_out, norm_out);
+    ++g_pn_launches;
+    return cudaGetLastError();
 }
 
 // Multi-GPU exchange step of the statistics: the moment records of R parts of the same ensembles
