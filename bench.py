@@ -324,6 +324,23 @@ def run_ours(args, cfg):
                                 "frac_of_hbm": 96 * n / ge / 1e6 / hbm,
                                 "max_abs_diff_vs_host_recipe": float((g_y0 - d_y0).abs().max().item())},
                    "hbm_peak_gbs": hbm, "hbm_peak_source": hbm_src}
+        # the same workload as ONE fused call (pn_run_ensembles: seed in, statistics out, no state arrays; FP64 only),
+        # next to the unfused chain generate -> integrate -> statistics on the same ensemble
+        if prec == pn.PN_FP64:
+            fo = dict(pearson_r=torch.zeros(1, 3, dtype=torch.float64, device=dev), hist1=torch.zeros(1, 3, cfg.bins, dtype=torch.int64, device=dev),
+                      hist2=torch.zeros(1, 3, 79, 79, dtype=torch.int64, device=dev))
+            fu_ms, fu_wall = [], []
+            for i in range(3):
+                flush.zero_(); torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                pn.pn_run_ensembles(ens, n, cfg.omegaf, cfg.rtol, cfg.atol, bins1=cfg.bins, bins2=79, **fo)
+                fu_wall.append((time.perf_counter() - t0) * 1e3); fu_ms.append(pn.pn_last_kernel_ms()["integrate"])
+            chain_ms = ge + float(np.mean(kern_ms)) + st
+            widened["fused"] = {"ms_kernels": float(np.median(fu_ms[1:])), "ms_call": float(np.median(fu_wall[1:])),
+                                "inspirals_per_sec": n / (float(np.median(fu_wall[1:])) * 1e-3),
+                                "unfused_chain_ms_kernels": chain_ms, "pearson_r": fo["pearson_r"].cpu().numpy()[0].tolist(),
+                                "hist1_equals_unfused": bool(torch.equal(fo["hist1"], out["hist1"])),
+                                "hist2_equals_unfused": bool(torch.equal(fo["hist2"], out["hist2"]))}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

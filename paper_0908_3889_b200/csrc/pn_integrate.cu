@@ -165,43 +165,48 @@ __constant__ double pn_uni_table[PN_UNI_SLOTS][16];
 // waiting: ~2000 instructions for the Philox blocks, the two sincos, the per-system constants and the seed slope),
 // a warp draws 32 systems AT ONCE, one per lane, into a shared-memory ring ([word][slot], conflict-free), and lanes
 // whose inspiral has finished pop records off the ring; the global queue counter is advanced by 32 per draw.
-// Statistics: every thread keeps Welford moments (n, xbar, ybar, M2x, M2y, Cxy) of its own finished systems per dot
-// product in shared memory, for ONE ensemble at a time (queue order is index order, so a thread's ensembles never
-// decrease); when its ensemble changes and at kernel exit they are merged into the ensemble's global record with the
-// pairwise update under a per-ensemble spin lock (try-lock loop, safe under intra-warp contention).  Histogram counts
-// go straight to global memory with integer atomics (one per finished system and dot product).  Counts are exact and
-// reproducible; moments are reproducible to rounding (the merge order depends on timing).
+// Statistics: every BLOCK keeps Welford moments (n, xbar, ybar, M2x, M2y, Cxy) per dot product in shared memory for the
+// few ensembles it is currently working on (a table of PN_FW entries tagged with the ensemble; queue order is index
+// order, so the ensembles a block sees only grow); a finished system is added under a shared-memory spin lock (finishes
+// are rare: one per block every ~20 us).  An entry that has to make room, and every entry at kernel exit, is merged
+// into the ensemble's global record with the pairwise update under a per-ensemble global spin lock: a few hundred
+// uncontended merges per ensemble.  (r2 first kept per-thread moments and merged every thread into the global record:
+// 38 K threads taking one lock at kernel exit took 8.7 s.)  Both locks are try-lock loops, safe under intra-warp
+// contention.  Histogram counts go straight to global memory with integer atomics (one per finished system and dot
+// product).  Counts are exact and reproducible; moments are reproducible to rounding (merge order depends on timing).
 #define PN_FREC (PN_REC + 4)      /* ring record: seed record + the three initial unit dot products (+ pad) */
+#define PN_FW 4                   /* ensembles a block accumulates at a time */
 template <int BLOCK> struct PnFusedSmem {
     static constexpr int NW = BLOCK / 32;
     double* ring;     // [NW][PN_FREC][32]
     double* xin;      // [3][BLOCK]      initial unit dot products of the lane's current system (NaN: undefined)
-    double* acc;      // [3][6][BLOCK]   per-thread moments
+    double* mom;      // [PN_FW][3][6]   the block's moments
     int* ring_idx;    // [NW][32]
-    int* acc_g;       // [BLOCK]         ensemble the thread's moments belong to, -1: none
-    static constexpr size_t bytes() { return sizeof(double) * ((size_t)NW * PN_FREC * 32 + 3 * BLOCK + 18 * BLOCK) + sizeof(int) * (NW * 32 + BLOCK); }
+    int* tag;         // [PN_FW]         ensemble of each table entry, -1: free
+    int* lock;        // [1]             shared-memory lock of the table;  [1]: threads that have left the main loop
+    static constexpr size_t bytes() { return sizeof(double) * ((size_t)NW * PN_FREC * 32 + 3 * BLOCK + PN_FW * 18) + sizeof(int) * (NW * 32 + PN_FW + 4); }
     __device__ explicit PnFusedSmem(unsigned char* base)
     {
         ring = reinterpret_cast<double*>(base);
         xin = ring + (size_t)NW * PN_FREC * 32;
-        acc = xin + 3 * BLOCK;
-        ring_idx = reinterpret_cast<int*>(acc + 18 * BLOCK);
-        acc_g = ring_idx + NW * 32;
+        mom = xin + 3 * BLOCK;
+        ring_idx = reinterpret_cast<int*>(mom + PN_FW * 18);
+        tag = ring_idx + NW * 32;
+        lock = tag + PN_FW;
     }
 };
 
-// merge this thread's moments (acc[(k*6 + c)*BLOCK], already offset by the thread index) into ensemble g's record
-template <int BLOCK>
-__device__ __noinline__ void pn_fused_flush(const PnKernelParams& p, double* acc, int g)
+// merge one table entry (18 doubles in shared memory) into ensemble g's global record, then clear it.  Caller holds the
+// block's table lock.
+__device__ __noinline__ void pn_fused_flush(const PnKernelParams& p, volatile double* mom, int g)
 {
     bool done = false;
-    while (!done) {                                   // try-lock loop: a lane that fails simply tries again next round
+    while (!done) {                                   // try-lock loop: a thread that fails simply tries again
         if (atomicCAS(p.f_lock + g, 0, 1) == 0) {
             __threadfence();
 #pragma unroll 1
             for (int k = 0; k < 3; ++k) {
-                StMom a = {acc[(k * 6 + 0) * BLOCK], acc[(k * 6 + 1) * BLOCK], acc[(k * 6 + 2) * BLOCK],
-                           acc[(k * 6 + 3) * BLOCK], acc[(k * 6 + 4) * BLOCK], acc[(k * 6 + 5) * BLOCK]};
+                StMom a = {mom[k * 6 + 0], mom[k * 6 + 1], mom[k * 6 + 2], mom[k * 6 + 3], mom[k * 6 + 4], mom[k * 6 + 5]};
                 if (a.n > 0.0) {
                     volatile double* q = p.f_mom + ((size_t)g * 3 + k) * 6;
                     StMom m = {q[0], q[1], q[2], q[3], q[4], q[5]};
@@ -212,13 +217,15 @@ __device__ __noinline__ void pn_fused_flush(const PnKernelParams& p, double* acc
             __threadfence();
             atomicExch(p.f_lock + g, 0);
             done = true;
+        } else {
+            __nanosleep(200);
         }
     }
-#pragma unroll
-    for (int j = 0; j < 18; ++j) acc[j * BLOCK] = 0.0;
+#pragma unroll 1
+    for (int j = 0; j < 18; ++j) mom[j] = 0.0;
 }
 
-// a finished system of the fused mode: final unit dot products -> the thread's moments and the global histograms
+// a finished system of the fused mode: final unit dot products -> the block's moments and the global histograms
 template <int BLOCK>
 __device__ __noinline__ void pn_fused_finish(const PnKernelParams& p, const PnFusedSmem<BLOCK>& fs, int idx, int code, const double (&v9)[9])
 {
@@ -230,26 +237,47 @@ __device__ __noinline__ void pn_fused_finish(const PnKernelParams& p, const PnFu
         for (int k = 0; k < 3; ++k) atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull);
         return;
     }
-    double df[3];
-    bool okf[3];
+    double df[3], x[3];
+    bool okf[3], ok[3];
     pn_unit_dots(v9, df, okf);
-    double* acc = fs.acc + tid;
-    if (fs.acc_g[tid] != g) {
-        if (fs.acc_g[tid] >= 0) pn_fused_flush<BLOCK>(p, acc, fs.acc_g[tid]);
-        fs.acc_g[tid] = g;
-    }
-#pragma unroll 1
+#pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const double x = fs.xin[k * BLOCK + tid];
-        if (!(okf[k] && x == x)) { atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull); continue; }
-        StMom a = {acc[(k * 6 + 0) * BLOCK], acc[(k * 6 + 1) * BLOCK], acc[(k * 6 + 2) * BLOCK],
-                   acc[(k * 6 + 3) * BLOCK], acc[(k * 6 + 4) * BLOCK], acc[(k * 6 + 5) * BLOCK]};
-        st_add(a, x, df[k]);
-        acc[(k * 6 + 0) * BLOCK] = a.n; acc[(k * 6 + 1) * BLOCK] = a.mx; acc[(k * 6 + 2) * BLOCK] = a.my;
-        acc[(k * 6 + 3) * BLOCK] = a.m2x; acc[(k * 6 + 4) * BLOCK] = a.m2y; acc[(k * 6 + 5) * BLOCK] = a.cxy;
+        x[k] = fs.xin[k * BLOCK + tid];
+        ok[k] = okf[k] && x[k] == x[k];
+        if (!ok[k]) { atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull); continue; }
         if (p.f_hist1) atomicAdd(p.f_hist1 + ((size_t)g * 3 + k) * p.f_bins1 + pn_bin_of(df[k], p.f_bins1), 1ull);
         if (p.f_hist2)
-            atomicAdd(p.f_hist2 + (((size_t)g * 3 + k) * p.f_bins2 + pn_bin_of(x, p.f_bins2)) * p.f_bins2 + pn_bin_of(df[k], p.f_bins2), 1ull);
+            atomicAdd(p.f_hist2 + (((size_t)g * 3 + k) * p.f_bins2 + pn_bin_of(x[k], p.f_bins2)) * p.f_bins2 + pn_bin_of(df[k], p.f_bins2), 1ull);
+    }
+    if (!(ok[0] || ok[1] || ok[2])) return;
+    volatile int* tag = fs.tag;
+    bool done = false;
+    while (!done) {
+        if (atomicCAS(fs.lock, 0, 1) == 0) {
+            __threadfence_block();
+            int slot = -1, lowest = 0;
+#pragma unroll
+            for (int w = 0; w < PN_FW; ++w) {
+                if (tag[w] == g) slot = w;
+                if (tag[w] < tag[lowest]) lowest = w;              // a free entry (-1) or the oldest ensemble
+            }
+            if (slot < 0) {
+                slot = lowest;
+                if (tag[slot] >= 0) pn_fused_flush(p, fs.mom + slot * 18, tag[slot]);
+                tag[slot] = g;
+            }
+            volatile double* m = fs.mom + slot * 18;
+#pragma unroll 1
+            for (int k = 0; k < 3; ++k) {
+                if (!ok[k]) continue;
+                StMom a = {m[k * 6 + 0], m[k * 6 + 1], m[k * 6 + 2], m[k * 6 + 3], m[k * 6 + 4], m[k * 6 + 5]};
+                st_add(a, x[k], df[k]);
+                m[k * 6 + 0] = a.n; m[k * 6 + 1] = a.mx; m[k * 6 + 2] = a.my; m[k * 6 + 3] = a.m2x; m[k * 6 + 4] = a.m2y; m[k * 6 + 5] = a.cxy;
+            }
+            __threadfence_block();
+            atomicExch(fs.lock, 0);
+            done = true;
+        }
     }
 }
 
@@ -267,9 +295,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     PnFusedSmem<BLOCK> fs(pn_fused_smem);                 // FUSED only (no dynamic shared memory otherwise)
     unsigned ring_used = 0, ring_count = 0;               // warp-uniform: records popped / drawn in the current batch
     if constexpr (FUSED) {
-#pragma unroll
-        for (int j = 0; j < 18; ++j) fs.acc[j * BLOCK + threadIdx.x] = 0.0;
-        fs.acc_g[threadIdx.x] = -1;
+        if (threadIdx.x < PN_FW * 18) fs.mom[threadIdx.x] = 0.0;
+        if (threadIdx.x < PN_FW) fs.tag[threadIdx.x] = -1;
+        if (threadIdx.x < 2) fs.lock[threadIdx.x] = 0;
+        __syncthreads();
     }
 
     // lane state.  k1 holds the SCALED slope h*f(y).  Idle lanes are frozen (h = 0, k1 = 0) on a benign
@@ -328,12 +357,22 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                 double* ring_w = fs.ring + (size_t)(threadIdx.x >> 5) * PN_FREC * 32;
                 int* ring_idx_w = fs.ring_idx + (threadIdx.x >> 5) * 32;
                 if (ring_used >= ring_count) {
-                    unsigned qb = 0;
-                    if (lane == 0) qb = atomicAdd(SLOW ? p.queue2 : p.queue, 32u);
+                    // 32 systems per draw, except in the last wave of the queue (fewer systems left than resident lanes):
+                    // there a warp draws only what its idle lanes start right now, so that no warp sits on drawn but
+                    // unstarted systems while lanes elsewhere have run dry (the drain tail stays one inspiral long)
+                    unsigned* qptr = SLOW ? p.queue2 : p.queue;
+                    const unsigned idle_now = (unsigned)__popc(__ballot_sync(FULL, idx < 0));
+                    unsigned qb = 0, take = 32u;
+                    if (lane == 0) {
+                        const unsigned seen = *(volatile unsigned*)qptr;
+                        if (seen + gridDim.x * BLOCK >= n_queue) take = idle_now;
+                        qb = atomicAdd(qptr, take);
+                    }
                     qb = __shfl_sync(FULL, qb, 0);
+                    take = __shfl_sync(FULL, take, 0);
                     ring_used = 0u;
-                    ring_count = qb < n_queue ? min(32u, n_queue - qb) : 0u;
-                    if (qb + 32u >= n_queue) queue_empty = true;
+                    ring_count = qb < n_queue ? min(take, n_queue - qb) : 0u;
+                    if (qb + take >= n_queue) queue_empty = true;
                     if ((unsigned)lane < ring_count) {
                         const int i = order ? order[qb + lane] : (int)(qb + lane);
                         const long long gsys = p.f_base + i;
@@ -516,8 +555,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     }
 
     if constexpr (FUSED) {
-        // the thread's moments go to its last ensemble's record
-        if (fs.acc_g[threadIdx.x] >= 0) pn_fused_flush<BLOCK>(p, fs.acc + threadIdx.x, fs.acc_g[threadIdx.x]);
+        // the last thread of the block to leave the loop merges the block's table into the global records
+        __threadfence_block();
+        if (atomicAdd(fs.lock + 1, 1) == BLOCK - 1) {
+            __threadfence_block();
+            for (int w = 0; w < PN_FW; ++w)
+                if (((volatile int*)fs.tag)[w] >= 0) pn_fused_flush(p, fs.mom + w * 18, ((volatile int*)fs.tag)[w]);
+        }
     }
     // ---------------- per-launch counters: warp reduce, one atomic per warp ----------------
 #pragma unroll
