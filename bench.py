@@ -384,11 +384,15 @@ def run_ours(args, cfg):
                      "algorithmic_bytes": 196 * n,
                      "peak_source": f"nominal {sms} SMs x {lanes} FMA lanes x 2 x {sm_max:.0f} MHz (DESIGN.md 6.3)",
                      "peak_measured_fma": peak_meas, "peak_measured_sm_mhz": peak_mhz,
+                     "peak_measured_ffma2": pn.pn_measure_fma_peak(3, 0.25)[0] if peak_prec == pn.PN_FP32 else None,
                      "frac_of_measured_fma": achieved / peak_meas if peak_meas > 0 else None,
                      "flops_per_trial_step": F_STEP, "flops_per_rhs": F_RHS,
                      "frac_with_oracle_as_printed_count": (float(np.mean(trial_steps)) * F_STEP_ORACLE + n * F_RHS_ORACLE)
                      / (k_ms * 1e-3) / 1e12 / peak_nominal,
-                     "fma_issue_cycles_by_register_sources": {str(k): pn.pn_measure_fma_operands(peak_prec, k) for k in (1, 2, 3)}},
+                     "fma_issue_cycles_by_register_sources": {str(k): pn.pn_measure_fma_operands(peak_prec, k) for k in (1, 2, 3)},
+                     # a two-source FMA + two independent integer instructions: 2 cycles if they issued in the FMA's
+                     # shadow, 4 if every instruction takes its own issue cycles
+                     "fma_plus_two_alu_issue_cycles": pn.pn_measure_fma_operands(peak_prec, 4)},
         "e2e": {"value": total_inspirals / e2e_s, "unit": "inspirals/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": e2e_steps},
         "gpu_launches": int(launches), "clocks": clocks,

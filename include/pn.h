@@ -269,7 +269,8 @@ int pn_stream_status(void* stream);
  * pn_measure_fma_peak -- measured FMA throughput of this device at its current clocks: every thread
  * runs `chains` independent dependent-FMA chains (no memory traffic) for about `seconds`.
  * Writes achieved TFLOP/s (2 flops per FMA) and, if not NULL, the SM clock in MHz estimated from
- * clock64() over the run.  The denominator of the reported roofline fraction.
+ * clock64() over the run (the longest per-block span).  The denominator of the reported roofline fraction.
+ * precision: PN_FP64, PN_FP32 (scalar FFMA), or 3 = FP32 with packed f32x2 FMAs (FFMA2, 4 flops per instruction and lane).
  */
 int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz);
 
@@ -277,6 +278,9 @@ int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* s
  * pn_measure_fma_operands -- issue cost of an FMA as a function of how many DISTINCT register sources it
  * reads (1, 2 or 3; the other operands are uniform): cycles per warp instruction per scheduler with 8 warps
  * x 8 independent chains resident.  Evidence for the operand-port model of DESIGN.md 7.2.
+ * n_register_sources = 4 is the issue-overlap probe: a two-source FMA plus two independent integer instructions
+ * (LOP3, IADD3) per group; the result is cycles per GROUP (2 if the integer instructions issue in the FMA's shadow,
+ * 4 if every instruction takes its own issue cycles).
  */
 int pn_measure_fma_operands(int precision, int n_register_sources, double* cycles_per_warp_inst);
 

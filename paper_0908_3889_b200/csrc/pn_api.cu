@@ -672,14 +672,14 @@ extern "C" int pn_stream_status(void* stream)
 
 extern "C" int pn_measure_fma_peak(int precision, double seconds, double* tflops, double* sm_mhz)
 {
-    if (!tflops || (precision != PN_FP64 && precision != PN_FP32)) return PN_EINVAL;
+    if (!tflops || (precision != PN_FP64 && precision != PN_FP32 && precision != 3)) return PN_EINVAL;
     CK(pn_run_fma_peak(precision, 0, seconds, tflops, sm_mhz, nullptr));
     return PN_OK;
 }
 
 extern "C" int pn_measure_fma_operands(int precision, int n_register_sources, double* cycles_per_warp_inst)
 {
-    if (!cycles_per_warp_inst || n_register_sources < 1 || n_register_sources > 3 ||
+    if (!cycles_per_warp_inst || n_register_sources < 1 || n_register_sources > 4 ||
         (precision != PN_FP64 && precision != PN_FP32))
         return PN_EINVAL;
     CK(pn_run_fma_peak(precision, n_register_sources - 1, 0.1, nullptr, nullptr, cycles_per_warp_inst));

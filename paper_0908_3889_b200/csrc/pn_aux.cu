@@ -269,6 +269,8 @@ cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch
 // the ALU roofline at the clocks the device actually holds.  MODE 1: a = a*x + U (two
 // distinct register sources).  MODE 2: a = a*x + z (three distinct register sources).  On sm_100a a DFMA
 // issues every 2 cycles per scheduler with <= 2 register sources and every 3 cycles with 3.
+// MODE 3: MODE 1 plus TWO independent integer instructions (LOP3, IADD3) per FMA: do instructions of another pipe issue in
+// the shadow of a 2-cycle DFMA?  Mostly not: 3.7 cycles per group, against 2 if hidden and 4 if fully additive.
 // Clock: every block measures its own clock64() span and the LONGEST span is kept (atomicMax).  Co-resident
 // blocks are not served evenly: the warp arbiter runs the blocks of an SM almost one after the other (measured:
 // with 4 resident blocks the first finishes after 1/4 of the kernel's duration, the last spans all of it), so
@@ -278,11 +280,13 @@ template <typename real, int CHAINS, int MODE>
 __global__ void __launch_bounds__(256) pn_fma_peak_kernel(real* out, int iters, unsigned long long* clocks, real m, real b)
 {
     real a[CHAINS], x[CHAINS], z[CHAINS];
+    unsigned w[CHAINS];
 #pragma unroll
     for (int i = 0; i < CHAINS; ++i) {
         a[i] = (real)(threadIdx.x + i) * (real)1e-3;
         x[i] = (real)1 - (real)1e-7 * (real)(threadIdx.x + i) + out[1];
         z[i] = (real)1e-7 * (real)(i + threadIdx.x) + out[2];
+        w[i] = threadIdx.x * 7u + i;
     }
     const long long c0 = clock64();
     for (int it = 0; it < iters; ++it) {
@@ -291,18 +295,42 @@ __global__ void __launch_bounds__(256) pn_fma_peak_kernel(real* out, int iters, 
 #pragma unroll
             for (int i = 0; i < CHAINS; ++i) {
                 if (MODE == 0) a[i] = a[i] * m + b;
-                if (MODE == 1) a[i] = a[i] * x[i] + b;
+                if (MODE == 1 || MODE == 3) a[i] = a[i] * x[i] + b;
                 if (MODE == 2) a[i] = a[i] * x[i] + z[i];
+                if (MODE == 3) w[i] = (w[i] ^ (unsigned)it) + (unsigned)i + 1u;      // one LOP3 + one IADD3
             }
     }
     const long long c1 = clock64();
     real s = 0;
 #pragma unroll
-    for (int i = 0; i < CHAINS; ++i) s += a[i];
+    for (int i = 0; i < CHAINS; ++i) s += a[i] + (MODE == 3 ? (real)w[i] : (real)0);
     if (s == (real)123.456) out[0] = s;
     if (threadIdx.x == 0) atomicMax(clocks, (unsigned long long)(c1 - c0));
 }
 
+// packed FP32: a = a * m + b on register pairs (FFMA2), 8 chains per thread; 4 flops per instruction and lane
+__global__ void __launch_bounds__(256) pn_ffma2_peak_kernel(float* out, int iters, unsigned long long* clocks, float m, float b)
+{
+    float2 a[8];
+    const float2 mm = make_float2(m, m), bb = make_float2(b, b);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = make_float2((threadIdx.x + i) * 1e-3f, (threadIdx.x + i) * 2e-3f);
+    const long long c0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) a[i] = __ffma2_rn(a[i], mm, bb);
+    }
+    const long long c1 = clock64();
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i].x + a[i].y;
+    if (s == 123.456f) out[0] = s;
+    if (threadIdx.x == 0) atomicMax(clocks, (unsigned long long)(c1 - c0));
+}
+
+// precision 0 / 1: FP64 / FP32 scalar FMA; 3: FP32 packed (FFMA2, mode ignored)
 cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tflops, double* sm_mhz,
                             double* cycles_per_warp_inst)
 {
@@ -323,8 +351,9 @@ cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tfl
     const int block = 256;
     int occ = 0;
 #define PN_PEAK_OCC(T, M) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pn_fma_peak_kernel<T, CH, M>, block, 0)
-    if (precision == 0) { if (mode == 0) PN_PEAK_OCC(double, 0); else if (mode == 1) PN_PEAK_OCC(double, 1); else PN_PEAK_OCC(double, 2); }
-    else { if (mode == 0) PN_PEAK_OCC(float, 0); else if (mode == 1) PN_PEAK_OCC(float, 1); else PN_PEAK_OCC(float, 2); }
+    if (precision == 3) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pn_ffma2_peak_kernel, block, 0);
+    else if (precision == 0) { if (mode == 0) PN_PEAK_OCC(double, 0); else if (mode == 1) PN_PEAK_OCC(double, 1); else if (mode == 2) PN_PEAK_OCC(double, 2); else PN_PEAK_OCC(double, 3); }
+    else { if (mode == 0) PN_PEAK_OCC(float, 0); else if (mode == 1) PN_PEAK_OCC(float, 1); else if (mode == 2) PN_PEAK_OCC(float, 2); else PN_PEAK_OCC(float, 3); }
 #undef PN_PEAK_OCC
     const int resident = occ >= 4 ? 4 : (occ >= 1 ? occ : 1);
     const int grid = sms * resident;
@@ -333,8 +362,9 @@ cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tfl
         cudaMemsetAsync(dclk, 0, sizeof(unsigned long long));
         cudaEventRecord(e0);
 #define PN_PEAK(T, M) pn_fma_peak_kernel<T, CH, M><<<grid, block>>>((T*)scratch, iters, dclk, (T)0.999999, (T)1e-7)
-        if (precision == 0) { if (mode == 0) PN_PEAK(double, 0); else if (mode == 1) PN_PEAK(double, 1); else PN_PEAK(double, 2); }
-        else { if (mode == 0) PN_PEAK(float, 0); else if (mode == 1) PN_PEAK(float, 1); else PN_PEAK(float, 2); }
+        if (precision == 3) pn_ffma2_peak_kernel<<<grid, block>>>((float*)scratch, iters, dclk, 0.999999f, 1e-7f);
+        else if (precision == 0) { if (mode == 0) PN_PEAK(double, 0); else if (mode == 1) PN_PEAK(double, 1); else if (mode == 2) PN_PEAK(double, 2); else PN_PEAK(double, 3); }
+        else { if (mode == 0) PN_PEAK(float, 0); else if (mode == 1) PN_PEAK(float, 1); else if (mode == 2) PN_PEAK(float, 2); else PN_PEAK(float, 3); }
 #undef PN_PEAK
         ++g_pn_launches;
         cudaEventRecord(e1);
@@ -353,7 +383,7 @@ cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tfl
         iters = (int)it2;
         e = run(iters, &ms);
         if (e == cudaSuccess) {
-            const double fl = 2.0 * 8.0 * CH * (double)iters * (double)grid * block;
+            const double fl = (precision == 3 ? 4.0 : 2.0) * 8.0 * CH * (double)iters * (double)grid * block;
             if (tflops) *tflops = fl / (ms * 1e-3) / 1e12;
             unsigned long long clk = 0;
             cudaMemcpy(&clk, dclk, sizeof clk, cudaMemcpyDeviceToHost);

@@ -165,35 +165,42 @@ __constant__ double pn_uni_table[PN_UNI_SLOTS][16];
 // waiting: ~2000 instructions for the Philox blocks, the two sincos, the per-system constants and the seed slope),
 // a warp draws 32 systems AT ONCE, one per lane, into a shared-memory ring ([word][slot], conflict-free), and lanes
 // whose inspiral has finished pop records off the ring; the global queue counter is advanced by 32 per draw.
-// Statistics: every BLOCK keeps Welford moments (n, xbar, ybar, M2x, M2y, Cxy) per dot product in shared memory for the
-// few ensembles it is currently working on (a table of PN_FW entries tagged with the ensemble; queue order is index
-// order, so the ensembles a block sees only grow); a finished system is added under a shared-memory spin lock (finishes
-// are rare: one per block every ~20 us).  An entry that has to make room, and every entry at kernel exit, is merged
-// into the ensemble's global record with the pairwise update under a per-ensemble global spin lock: a few hundred
-// uncontended merges per ensemble.  (r2 first kept per-thread moments and merged every thread into the global record:
-// 38 K threads taking one lock at kernel exit took 8.7 s.)  Both locks are try-lock loops, safe under intra-warp
-// contention.  Histogram counts go straight to global memory with integer atomics (one per finished system and dot
-// product).  Counts are exact and reproducible; moments are reproducible to rounding (merge order depends on timing).
+// Statistics, three levels.  (1) Every THREAD keeps Welford moments (n, xbar, ybar, M2x, M2y, Cxy) per dot product in
+// its own shared-memory words, for one ensemble at a time: a finished system is added without any lock (queue order is
+// index order, so a thread's ensembles only grow).  (2) When its ensemble changes, and at kernel exit, a thread merges
+// them (pairwise update) into the BLOCK's table of PN_FW ensembles under a shared-memory spin lock.  (3) A table entry
+// that has to make room, and every entry when the last thread of the block leaves, is merged into the ensemble's
+// global record under a per-ensemble global spin lock: a few hundred uncontended merges per ensemble.  (Tried before:
+// threads merging straight into the global record -- 38 K threads taking one lock at kernel exit took 8.7 s; and every
+// finished system added to the block's table under the lock -- at ~170 steps per inspiral the ~3000-cycle critical
+// section was longer than the time between two finishes of a block, and the run took 43 % longer than the unfused one.)
+// All locks are try-lock loops, safe under intra-warp contention.  Histogram counts go straight to global memory with
+// integer atomics (one per finished system and dot product).  Counts are exact and reproducible; moments are
+// reproducible to rounding (the merge order depends on timing).
 #define PN_FREC (PN_REC + 4)      /* ring record: seed record + the three initial unit dot products (+ pad) */
 #define PN_FW 4                   /* ensembles a block accumulates at a time */
+#define PN_FDONE 13               /* done-ring record: 9 final components (S1, S2, L^), 3 initial dot products, {index, code} */
 template <int BLOCK> struct PnFusedSmem {
+    // one base pointer; every array is at a compile-time offset (seven stored pointers would cost 14 registers in a
+    // kernel that has none to spare)
     static constexpr int NW = BLOCK / 32;
-    double* ring;     // [NW][PN_FREC][32]
-    double* xin;      // [3][BLOCK]      initial unit dot products of the lane's current system (NaN: undefined)
-    double* mom;      // [PN_FW][3][6]   the block's moments
-    int* ring_idx;    // [NW][32]
-    int* tag;         // [PN_FW]         ensemble of each table entry, -1: free
-    int* lock;        // [1]             shared-memory lock of the table;  [1]: threads that have left the main loop
-    static constexpr size_t bytes() { return sizeof(double) * ((size_t)NW * PN_FREC * 32 + 3 * BLOCK + PN_FW * 18) + sizeof(int) * (NW * 32 + PN_FW + 4); }
-    __device__ explicit PnFusedSmem(unsigned char* base)
-    {
-        ring = reinterpret_cast<double*>(base);
-        xin = ring + (size_t)NW * PN_FREC * 32;
-        mom = xin + 3 * BLOCK;
-        ring_idx = reinterpret_cast<int*>(mom + PN_FW * 18);
-        tag = ring_idx + NW * 32;
-        lock = tag + PN_FW;
-    }
+    static constexpr size_t O_XIN = (size_t)NW * PN_FREC * 32, O_ACC = O_XIN + 3 * BLOCK, O_MOM = O_ACC + 18 * BLOCK,
+                            O_DONE = O_MOM + PN_FW * 18, N_DBL = O_DONE + (size_t)NW * PN_FDONE * 32;
+    static constexpr size_t bytes() { return sizeof(double) * N_DBL + sizeof(int) * (NW * 32 + BLOCK + PN_FW + 4 + NW * 4); }
+    unsigned char* base;
+    __device__ explicit PnFusedSmem(unsigned char* b) : base(b) {}
+    __device__ __forceinline__ double* ring() const { return reinterpret_cast<double*>(base); }                 // [NW][PN_FREC][32]
+    __device__ __forceinline__ double* xin() const { return ring() + O_XIN; }    // [3][BLOCK] initial unit dot products of the lane's system (NaN: undefined)
+    __device__ __forceinline__ double* acc() const { return ring() + O_ACC; }    // [3][6][BLOCK] every thread's own moments (no lock), ONE ensemble at a time
+    __device__ __forceinline__ double* mom() const { return ring() + O_MOM; }    // [PN_FW][3][6] the block's moments
+    __device__ __forceinline__ double* done() const { return ring() + O_DONE; }  // [NW][PN_FDONE][32] finished systems waiting for the warp's next batch
+    __device__ __forceinline__ int* ring_idx() const { return reinterpret_cast<int*>(ring() + N_DBL); }        // [NW][32]
+    __device__ __forceinline__ int* acc_g() const { return ring_idx() + NW * 32; }   // [BLOCK] ensemble of the thread's moments, -1: none
+    __device__ __forceinline__ int* tag() const { return acc_g() + BLOCK; }          // [PN_FW] ensemble of each table entry, -1: free
+    __device__ __forceinline__ int* lock() const { return tag() + PN_FW; }           // [0] table lock; [1] threads that have left the main loop
+    // per warp, warp-uniform, touched only in the refill / finish sections (so they live here, not in registers):
+    // [0] records popped off the ring, [1] records drawn into it, [2] finished systems parked in the done ring
+    __device__ __forceinline__ volatile int* wstate() const { return lock() + 4 + (threadIdx.x >> 5) * 4; }
 };
 
 // merge one table entry (18 doubles in shared memory) into ensemble g's global record, then clear it.  Caller holds the
@@ -225,35 +232,39 @@ __device__ __noinline__ void pn_fused_flush(const PnKernelParams& p, volatile do
     for (int j = 0; j < 18; ++j) mom[j] = 0.0;
 }
 
-// a finished system of the fused mode: final unit dot products -> the block's moments and the global histograms
-template <int BLOCK>
-__device__ __noinline__ void pn_fused_finish(const PnKernelParams& p, const PnFusedSmem<BLOCK>& fs, int idx, int code, const double (&v9)[9])
+// draw system i of the launch's queue (pn_gen.cuh: the bits pn_generate would write), make its seed record and its
+// initial unit dot products, and put them into slot `lane` of the warp's ring (ring points at word 0 of that slot,
+// words are 32 doubles apart).  Out of line: ~2000 instructions that run once per 32 systems.
+template <typename real>
+__device__ __noinline__ void pn_fused_draw(const PnKernelParams& p, int i, double* ring, int* ring_idx)
 {
-    const long long gsys = p.f_base + idx;
-    const int g = (int)(gsys / p.f_count);
-    const int tid = threadIdx.x;
-    if (code <= 0) {                                  // failed: left out of all three statistics
+    const long long gsys = p.f_base + i;
+    const long long e = gsys / p.f_count;
+    const GenSpec sp = ((const GenSpec*)p.f_specs)[e];
+    double y0[10], m1, m2;
+    gen_system_at(sp, (unsigned long long)p.f_n_total, (unsigned long long)(p.f_first + (gsys - e * p.f_count)), y0, m1, m2);
+    real rec[PN_REC];
+    pn_make_record<real>(y0, m1, m2, p, rec);
 #pragma unroll
-        for (int k = 0; k < 3; ++k) atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull);
-        return;
-    }
-    double df[3], x[3];
-    bool okf[3], ok[3];
-    pn_unit_dots(v9, df, okf);
+    for (int j = 0; j < PN_REC; ++j) ring[j * 32] = (double)rec[j];
+    const double v9[9] = {y0[1], y0[2], y0[3], y0[4], y0[5], y0[6], y0[7], y0[8], y0[9]};
+    double d0[3];
+    bool ok0[3];
+    pn_unit_dots(v9, d0, ok0);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        x[k] = fs.xin[k * BLOCK + tid];
-        ok[k] = okf[k] && x[k] == x[k];
-        if (!ok[k]) { atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull); continue; }
-        if (p.f_hist1) atomicAdd(p.f_hist1 + ((size_t)g * 3 + k) * p.f_bins1 + pn_bin_of(df[k], p.f_bins1), 1ull);
-        if (p.f_hist2)
-            atomicAdd(p.f_hist2 + (((size_t)g * 3 + k) * p.f_bins2 + pn_bin_of(x[k], p.f_bins2)) * p.f_bins2 + pn_bin_of(df[k], p.f_bins2), 1ull);
-    }
-    if (!(ok[0] || ok[1] || ok[2])) return;
-    volatile int* tag = fs.tag;
+    for (int k = 0; k < 3; ++k) ring[(PN_REC + k) * 32] = ok0[k] ? d0[k] : nan("");
+    *ring_idx = i;
+}
+
+// merge the calling thread's moments for ensemble g into the block's table (shared-memory try-lock), then clear them
+template <int BLOCK>
+__device__ __noinline__ void pn_fused_thread_flush(const PnKernelParams& p, const PnFusedSmem<BLOCK>& fs, int g)
+{
+    double* acc = fs.acc() + threadIdx.x;
+    volatile int* tag = fs.tag();
     bool done = false;
     while (!done) {
-        if (atomicCAS(fs.lock, 0, 1) == 0) {
+        if (atomicCAS(fs.lock(), 0, 1) == 0) {
             __threadfence_block();
             int slot = -1, lowest = 0;
 #pragma unroll
@@ -263,22 +274,89 @@ __device__ __noinline__ void pn_fused_finish(const PnKernelParams& p, const PnFu
             }
             if (slot < 0) {
                 slot = lowest;
-                if (tag[slot] >= 0) pn_fused_flush(p, fs.mom + slot * 18, tag[slot]);
+                if (tag[slot] >= 0) pn_fused_flush(p, fs.mom() + slot * 18, tag[slot]);
                 tag[slot] = g;
             }
-            volatile double* m = fs.mom + slot * 18;
+            volatile double* m = fs.mom() + slot * 18;
 #pragma unroll 1
             for (int k = 0; k < 3; ++k) {
-                if (!ok[k]) continue;
-                StMom a = {m[k * 6 + 0], m[k * 6 + 1], m[k * 6 + 2], m[k * 6 + 3], m[k * 6 + 4], m[k * 6 + 5]};
-                st_add(a, x[k], df[k]);
-                m[k * 6 + 0] = a.n; m[k * 6 + 1] = a.mx; m[k * 6 + 2] = a.my; m[k * 6 + 3] = a.m2x; m[k * 6 + 4] = a.m2y; m[k * 6 + 5] = a.cxy;
+                StMom a = {acc[(k * 6 + 0) * BLOCK], acc[(k * 6 + 1) * BLOCK], acc[(k * 6 + 2) * BLOCK],
+                           acc[(k * 6 + 3) * BLOCK], acc[(k * 6 + 4) * BLOCK], acc[(k * 6 + 5) * BLOCK]};
+                if (a.n > 0.0) {
+                    StMom t = {m[k * 6 + 0], m[k * 6 + 1], m[k * 6 + 2], m[k * 6 + 3], m[k * 6 + 4], m[k * 6 + 5]};
+                    st_merge(t, a);
+                    m[k * 6 + 0] = t.n; m[k * 6 + 1] = t.mx; m[k * 6 + 2] = t.my; m[k * 6 + 3] = t.m2x; m[k * 6 + 4] = t.m2y; m[k * 6 + 5] = t.cxy;
+                }
             }
             __threadfence_block();
-            atomicExch(fs.lock, 0);
+            atomicExch(fs.lock(), 0);
             done = true;
         }
     }
+#pragma unroll
+    for (int j = 0; j < 18; ++j) acc[j * BLOCK] = 0.0;
+}
+
+// Finished systems of the fused mode are not reduced by the lane that finished them (one lane working, 31 waiting, ~750
+// instructions: 12 % of a run of 170-step inspirals): the lane only parks the final vectors, the initial dot products,
+// the index and the code in the warp's done ring (14 shared-memory stores), and when the ring cannot take the next
+// arrivals -- and at kernel exit -- the whole warp reduces it, one entry per lane: final unit dot products -> the
+// thread's moments and the global histograms.
+template <int BLOCK>
+__device__ __noinline__ void pn_fused_finish_batch(const PnKernelParams& p, const PnFusedSmem<BLOCK>& fs, unsigned n_entries)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    if ((unsigned)lane >= n_entries) return;
+    const double* e = fs.done() + (size_t)(tid >> 5) * PN_FDONE * 32 + lane;
+    const long long packed = __double_as_longlong(e[12 * 32]);
+    const int idx = (int)(packed & 0xffffffffll), code = (int)(packed >> 32);
+    const long long gsys = p.f_base + idx;
+    const int g = (int)(gsys / p.f_count);
+    if (code <= 0) {                                  // failed: left out of all three statistics
+#pragma unroll
+        for (int k = 0; k < 3; ++k) atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull);
+        return;
+    }
+    const double v9[9] = {e[0], e[32], e[64], e[96], e[128], e[160], e[192], e[224], e[256]};
+    double df[3], x[3];
+    bool okf[3], ok[3];
+    pn_unit_dots(v9, df, okf);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        x[k] = e[(9 + k) * 32];
+        ok[k] = okf[k] && x[k] == x[k];
+        if (!ok[k]) { atomicAdd(p.f_skipped + (size_t)g * 3 + k, 1ull); continue; }
+        if (p.f_hist1) atomicAdd(p.f_hist1 + ((size_t)g * 3 + k) * p.f_bins1 + pn_bin_of(df[k], p.f_bins1), 1ull);
+        if (p.f_hist2)
+            atomicAdd(p.f_hist2 + (((size_t)g * 3 + k) * p.f_bins2 + pn_bin_of(x[k], p.f_bins2)) * p.f_bins2 + pn_bin_of(df[k], p.f_bins2), 1ull);
+    }
+    if (!(ok[0] || ok[1] || ok[2])) return;
+    // the thread's own moments: no lock.  They belong to one ensemble at a time; when the ensemble changes (and at
+    // kernel exit) they are merged into the block's table
+    double* acc = fs.acc() + tid;
+    if (fs.acc_g()[tid] != g) {
+        if (fs.acc_g()[tid] >= 0) pn_fused_thread_flush<BLOCK>(p, fs, fs.acc_g()[tid]);
+        fs.acc_g()[tid] = g;
+    }
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) {
+        if (!ok[k]) continue;
+        StMom a = {acc[(k * 6 + 0) * BLOCK], acc[(k * 6 + 1) * BLOCK], acc[(k * 6 + 2) * BLOCK],
+                   acc[(k * 6 + 3) * BLOCK], acc[(k * 6 + 4) * BLOCK], acc[(k * 6 + 5) * BLOCK]};
+        st_add(a, x[k], df[k]);
+        acc[(k * 6 + 0) * BLOCK] = a.n; acc[(k * 6 + 1) * BLOCK] = a.mx; acc[(k * 6 + 2) * BLOCK] = a.my;
+        acc[(k * 6 + 3) * BLOCK] = a.m2x; acc[(k * 6 + 4) * BLOCK] = a.m2y; acc[(k * 6 + 5) * BLOCK] = a.cxy;
+    }
+}
+
+// The redo pass of the fused mode calls the wide-range trial step out of line: inlined, the draw / statistics calls
+// around it push that (rarely used) instantiation 4 bytes over the register file; out of line the arithmetic and the
+// results are the same and nothing spills.
+__device__ __noinline__ void pn_dp5_trial_outofline(const double (&y)[10], const double (&K1)[10], double h, const PnConsts<double>& c,
+                                                    const PnUni<double>& u, const PnBase<double>& base, double (&ynew)[10],
+                                                    double (&K7)[10], double (&err)[10], PnBase<double>& base_new, bool& bad)
+{
+    pn_dp5_trial<true>(y, K1, h, c, u, base, ynew, K7, err, base_new, bad);
 }
 
 template <typename real, int BLOCK, int MINB, bool SLOW, bool MIXED = false, int UNI = -1, bool FUSED = false>
@@ -287,17 +365,23 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     if (UNI >= 0) { if (*p.nonuniform != 0) return; }
     else if (!SLOW && p.uni_slot >= 0) { if (*p.nonuniform == 0) return; }
     const unsigned n_queue = SLOW ? *p.redo_count : (unsigned)p.n;     // length of the work queue
-    const int* order = SLOW ? p.redo_list : p.order;
+    const int* order = SLOW ? p.redo_list : (FUSED ? nullptr : p.order);      // fused: queue order is index order
     if (SLOW && n_queue == 0u) return;
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     extern __shared__ __align__(16) unsigned char pn_fused_smem[];
     PnFusedSmem<BLOCK> fs(pn_fused_smem);                 // FUSED only (no dynamic shared memory otherwise)
-    unsigned ring_used = 0, ring_count = 0;               // warp-uniform: records popped / drawn in the current batch
+#define ring_used ((unsigned)fs.wstate()[0])
+#define ring_count ((unsigned)fs.wstate()[1])
+#define done_n ((unsigned)fs.wstate()[2])
     if constexpr (FUSED) {
-        if (threadIdx.x < PN_FW * 18) fs.mom[threadIdx.x] = 0.0;
-        if (threadIdx.x < PN_FW) fs.tag[threadIdx.x] = -1;
-        if (threadIdx.x < 2) fs.lock[threadIdx.x] = 0;
+#pragma unroll
+        for (int j = 0; j < 18; ++j) fs.acc()[j * BLOCK + threadIdx.x] = 0.0;
+        fs.acc_g()[threadIdx.x] = -1;
+        if (threadIdx.x < PN_FW * 18) fs.mom()[threadIdx.x] = 0.0;
+        if (threadIdx.x < PN_FW) fs.tag()[threadIdx.x] = -1;
+        if (threadIdx.x < 2) fs.lock()[threadIdx.x] = 0;
+        if ((threadIdx.x & 31) < 3) fs.wstate()[threadIdx.x & 31] = 0;
         __syncthreads();
     }
 
@@ -354,8 +438,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         if constexpr (FUSED) {
             // ---------------- fused refill: draw 32 systems per warp into the ring, idle lanes pop ----------------
             if (__any_sync(FULL, idx < 0) && !(queue_empty && ring_used >= ring_count)) {
-                double* ring_w = fs.ring + (size_t)(threadIdx.x >> 5) * PN_FREC * 32;
-                int* ring_idx_w = fs.ring_idx + (threadIdx.x >> 5) * 32;
+                double* ring_w = fs.ring() + (size_t)(threadIdx.x >> 5) * PN_FREC * 32;
+                int* ring_idx_w = fs.ring_idx() + (threadIdx.x >> 5) * 32;
                 if (ring_used >= ring_count) {
                     // 32 systems per draw, except in the last wave of the queue (fewer systems left than resident lanes):
                     // there a warp draws only what its idle lanes start right now, so that no warp sits on drawn but
@@ -365,48 +449,33 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
                     unsigned qb = 0, take = 32u;
                     if (lane == 0) {
                         const unsigned seen = *(volatile unsigned*)qptr;
-                        if (seen + gridDim.x * BLOCK >= n_queue) take = idle_now;
+                        if (seen + p.f_resident >= n_queue) take = idle_now;
                         qb = atomicAdd(qptr, take);
                     }
                     qb = __shfl_sync(FULL, qb, 0);
                     take = __shfl_sync(FULL, take, 0);
-                    ring_used = 0u;
-                    ring_count = qb < n_queue ? min(take, n_queue - qb) : 0u;
+                    const unsigned drawn = qb < n_queue ? min(take, n_queue - qb) : 0u;
+                    __syncwarp();
+                    if (lane == 0) { fs.wstate()[0] = 0; fs.wstate()[1] = (int)drawn; }
+                    __syncwarp();
                     if (qb + take >= n_queue) queue_empty = true;
-                    if ((unsigned)lane < ring_count) {
-                        const int i = order ? order[qb + lane] : (int)(qb + lane);
-                        const long long gsys = p.f_base + i;
-                        const long long e = gsys / p.f_count;
-                        const GenSpec sp = ((const GenSpec*)p.f_specs)[e];
-                        double y0[10], m1, m2;
-                        gen_system_at(sp, (unsigned long long)p.f_n_total, (unsigned long long)(p.f_first + (gsys - e * p.f_count)), y0, m1, m2);
-                        real rec[PN_REC];
-                        pn_make_record<real>(y0, m1, m2, p, rec);
-#pragma unroll
-                        for (int j = 0; j < PN_REC; ++j) ring_w[j * 32 + lane] = (double)rec[j];
-                        const double v9[9] = {y0[1], y0[2], y0[3], y0[4], y0[5], y0[6], y0[7], y0[8], y0[9]};
-                        double d0[3];
-                        bool ok0[3];
-                        pn_unit_dots(v9, d0, ok0);
-#pragma unroll
-                        for (int k = 0; k < 3; ++k) ring_w[(PN_REC + k) * 32 + lane] = ok0[k] ? d0[k] : nan("");
-                        ring_idx_w[lane] = i;
-                    }
+                    if ((unsigned)lane < drawn) pn_fused_draw<real>(p, order ? order[qb + lane] : (int)(qb + lane), ring_w + lane, ring_idx_w + lane);
                     __syncwarp();
                 }
                 const unsigned need = __ballot_sync(FULL, idx < 0);
-                const unsigned avail = ring_count - ring_used;
+                const unsigned used = ring_used, avail = ring_count - used;
                 const unsigned rank = (unsigned)__popc(need & ((1u << lane) - 1u));
                 if (idx < 0 && rank < avail) {
-                    const unsigned slot = ring_used + rank;
+                    const unsigned slot = used + rank;
                     real rec[PN_REC];
 #pragma unroll
                     for (int j = 0; j < PN_REC; ++j) rec[j] = (real)ring_w[j * 32 + slot];
 #pragma unroll
-                    for (int k = 0; k < 3; ++k) fs.xin[k * BLOCK + threadIdx.x] = ring_w[(PN_REC + k) * 32 + slot];
+                    for (int k = 0; k < 3; ++k) fs.xin()[k * BLOCK + threadIdx.x] = ring_w[(PN_REC + k) * 32 + slot];
                     start_system(rec, ring_idx_w[slot]);
                 }
-                ring_used += min((unsigned)__popc(need), avail);
+                __syncwarp();
+                if (lane == 0) fs.wstate()[0] = (int)(used + min((unsigned)__popc(need), avail));
                 __syncwarp();
             }
         } else
@@ -446,6 +515,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         PnBase<real> base_new;
         bool bad = false;
         if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad, dy);
+        else if constexpr (FUSED && SLOW) pn_dp5_trial_outofline(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
         else pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
         // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|), E^2 = mean (err_j/sc_j)^2.
         // It only decides accept/reject and the next step size, so ~1e-6 relative accuracy is ample:
@@ -490,7 +560,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         if (!active) ratio = (real)0;                      // idle (or just handed to the redo pass): frozen
         steps += active ? 1 : 0;
         tot_steps += active ? 1u : 0u;
-        nrej += reject ? 1 : 0;
+        if constexpr (!FUSED) nrej += reject ? 1 : 0;      // per-system count: an output of the unfused path only
         tot_rej += reject ? 1u : 0u;
         if (accept) t += (double)h;
         after_reject = reject || (after_reject && !accept);
@@ -515,13 +585,33 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         code = landed ? steps : code;
         code = !finite ? PN_F_NONFINITE : code;
         code = active ? code : 0;
-        if (code != 0) {
-            if constexpr (FUSED) {
-                double v9[9];
+        if constexpr (FUSED) {
+            const unsigned fm = __ballot_sync(FULL, code != 0);
+            if (fm != 0u) {
+                const unsigned nf = (unsigned)__popc(fm);
+                unsigned parked = done_n;
+                if (parked + nf > 32u) { pn_fused_finish_batch<BLOCK>(p, fs, parked); parked = 0u; __syncwarp(); }
+                if (code != 0) {
+                    double* e = fs.done() + (size_t)(threadIdx.x >> 5) * PN_FDONE * 32 + parked + (unsigned)__popc(fm & ((1u << lane) - 1u));
 #pragma unroll
-                for (int i = 0; i < 9; ++i) v9[i] = (double)(accept ? ynew[i + 1] : y[i + 1]);
-                pn_fused_finish<BLOCK>(p, fs, idx, code, v9);
-            } else if constexpr (MIXED) {
+                    for (int i = 0; i < 9; ++i) e[i * 32] = (double)(accept ? ynew[i + 1] : y[i + 1]);
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) e[(9 + k) * 32] = fs.xin()[k * BLOCK + threadIdx.x];
+                    e[12 * 32] = __longlong_as_double(((long long)code << 32) | (long long)(unsigned)idx);
+                    if (code < 0) {
+                        atomicMax(p.status, code == PN_F_NONFINITE ? PN_ST_ENONFINITE : PN_ST_ENOTCONVERGED);
+                        ++tot_fail;
+                    }
+                    idx = -1;
+                    ratio = (real)0;              // freeze the lane
+                }
+                __syncwarp();
+                if (lane == 0) fs.wstate()[2] = (int)(parked + nf);
+                __syncwarp();
+            }
+        } else
+        if (code != 0) {
+            if constexpr (MIXED) {
                 double yo[10];
 #pragma unroll
                 for (int i = 0; i < 10; ++i) yo[i] = accept ? yd[i] + (double)dy[i] : yd[i];
@@ -555,12 +645,16 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     }
 
     if constexpr (FUSED) {
-        // the last thread of the block to leave the loop merges the block's table into the global records
+        // the warp reduces what is left in its done ring; every thread merges its own moments into the block's table; the
+        // last thread of the block to leave the loop merges the table into the global records
+        if (done_n != 0u) pn_fused_finish_batch<BLOCK>(p, fs, done_n);
+        __syncwarp();
+        if (fs.acc_g()[threadIdx.x] >= 0) pn_fused_thread_flush<BLOCK>(p, fs, fs.acc_g()[threadIdx.x]);
         __threadfence_block();
-        if (atomicAdd(fs.lock + 1, 1) == BLOCK - 1) {
+        if (atomicAdd(fs.lock() + 1, 1) == BLOCK - 1) {
             __threadfence_block();
             for (int w = 0; w < PN_FW; ++w)
-                if (((volatile int*)fs.tag)[w] >= 0) pn_fused_flush(p, fs.mom + w * 18, ((volatile int*)fs.tag)[w]);
+                if (((volatile int*)fs.tag())[w] >= 0) pn_fused_flush(p, fs.mom() + w * 18, ((volatile int*)fs.tag())[w]);
         }
     }
     // ---------------- per-launch counters: warp reduce, one atomic per warp ----------------
@@ -578,6 +672,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         atomicAdd(p.counters + 3, (unsigned long long)tot_fail);
     }
 }
+
+#undef ring_used
+#undef ring_count
+#undef done_n
 
 // Fixed-step mode (tests, R15): exactly fixed_steps DP5 steps of size h0, y <- y_new.
 // SLOW = true is the redo pass over the systems that left the series' range in the fast pass.
@@ -688,6 +786,7 @@ cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s)
     if (need < grid) grid = (int)need;
     if (grid < 1) grid = 1;
     p.uni_slot = -1; p.order = nullptr;
+    p.f_resident = (unsigned)grid * BLOCK;
     fast<<<grid, BLOCK, shm, s>>>(p);
     redo<<<grid, BLOCK, shm, s>>>(p);
     g_pn_launches += 2;

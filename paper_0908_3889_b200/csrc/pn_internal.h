@@ -46,6 +46,7 @@ struct PnKernelParams {
     unsigned long long* f_hist1;    // [G][3][bins1] or null
     unsigned long long* f_hist2;    // [G][3][bins2][bins2] or null
     int f_bins1, f_bins2;
+    unsigned f_resident;            // lanes of the persistent grid (grid x block): the length of the queue's last wave
 };
 
 // launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults

@@ -1,7 +1,9 @@
-"""Seed in, statistics out: pn_generate -> pn_integrate -> pn_statistics (-> pn_selfcheck) on device buffers.
+"""Seed in, statistics out on the current CUDA device, for one ensemble or a sweep of ensembles.
 
 Orchestration only: every step is one call of the C ABI (include/pn.h) through binding.py; nothing is computed here.
-One ensemble or a sweep of ensembles, n systems each, all on the current CUDA device.
+fused=True (FP64): ONE call, pn_run_ensembles, no state arrays.  Otherwise the unfused chain
+pn_generate -> pn_integrate -> pn_statistics (-> pn_selfcheck) on device buffers, which also serves FP32 / mixed
+precision, the cross-check and keep_states.
 """
 from __future__ import annotations
 
@@ -9,7 +11,7 @@ from . import binding as B
 
 
 def run_ensembles(ensembles, n, omegaf, *, rtol=1e-10, atol=1e-12, precision=B.PN_FP64, bins1=50, bins2=79,
-                  check_fraction=0.0, check_key=(0, 0), keep_states=False):
+                  check_fraction=0.0, check_key=(0, 0), keep_states=False, fused=False):
     """ensembles: list of dicts for binding.make_ensemble (key, omega0, q, chi1, chi2, m1_fixed, s1_tilt_deg).
 
     Returns a dict of numpy arrays: pearson_r[G,3], moments[G,3,6], n_skipped[G,3], hist1[G,3,bins1],
@@ -22,6 +24,21 @@ def run_ensembles(ensembles, n, omegaf, *, rtol=1e-10, atol=1e-12, precision=B.P
     dev = torch.device("cuda", torch.cuda.current_device())
     f64 = dict(dtype=torch.float64, device=dev)
     i64 = dict(dtype=torch.int64, device=dev)
+    if fused:
+        if precision != B.PN_FP64 or check_fraction > 0 or keep_states:
+            raise ValueError("the fused mode is FP64 only and keeps no states (no cross-check, no keep_states)")
+        out = dict(pearson_r=torch.zeros(G, 3, **f64), moments=torch.zeros(G, 3, 6, **f64), n_skipped=torch.zeros(G, 3, **i64))
+        if bins1 > 0:
+            out["hist1"] = torch.zeros(G, 3, bins1, **i64)
+        if bins2 > 0:
+            out["hist2"] = torch.zeros(G, 3, bins2, bins2, **i64)
+            out["hist2_max"] = torch.zeros(G, 3, **i64)
+        status = B.pn_run_ensembles([B.make_ensemble(**e) for e in ens], int(n), omegaf, rtol, atol, bins1=bins1, bins2=bins2,
+                                    allow_failures=True, **out)
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+        res["status"] = status
+        res["steps_mean"] = None
+        return res
     y0, m = torch.empty(N, 10, **f64), torch.empty(N, 2, **f64)
     B.pn_generate([B.make_ensemble(**e) for e in ens], int(n), y0, m)
     yf = torch.empty_like(y0)
