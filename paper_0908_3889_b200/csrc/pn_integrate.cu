@@ -20,9 +20,13 @@ __device__ __forceinline__ float pn_err_norm2(const double (&y)[10], const doubl
 #pragma unroll
     for (int i = 0; i < 10; ++i) {
         const double at = (double)((i >= 1 && i <= 3) ? atS1 : ((i >= 4 && i <= 6) ? atS2 : atol1));
-        const unsigned ha = (unsigned)__double2hiint(y[i]) & 0x7fffffffu, hb = (unsigned)__double2hiint(ynew[i]) & 0x7fffffffu;
-        const double m = hb > ha ? ynew[i] : y[i];          // larger magnitude to ~1e-6 (high words only)
-        const double sc = fma(rt, fabs(m), at);
+        // larger magnitude to ~1e-6: the high words of two doubles order like floats of the same bit patterns (sign,
+        // then exponent, then mantissa), so ONE FMNMX with |.| modifiers picks the larger high word; the low word is
+        // dropped (the scale is then low by < 2^-20, the accuracy class of the MUFU reciprocal below).  A zero or tiny
+        // component (|y| < 2^-1015) reads as a float denormal or zero and stays that.
+        const float mh = fmaxf(fabsf(__int_as_float(__double2hiint(y[i]))), fabsf(__int_as_float(__double2hiint(ynew[i]))));
+        const double m = __hiloint2double(__float_as_int(mh), 0);
+        const double sc = fma(rt, m, at);
         double r;
         asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(sc));
         const double q = err[i] * r;

@@ -178,7 +178,7 @@ __device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, dou
         r = fma(b.r0 * e, S, b.r0);
         lnx = fma(-e, Q, b.l0);
     }
-    v = x * (r * r);
+    v = (x * r) * r;      // the caller's v2 = x r is the same product (CSE): v costs one multiply
 }
 template <bool SLOW>
 __device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float, float& v, float& lnx, float& r, bool&)
@@ -192,7 +192,7 @@ __device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float, 
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(l2 * (-1.0f / 3.0f)));
     const float e = fmaf(-x * r0, r0 * r0, 1.0f);
     r0 = fmaf(r0 * e, 1.0f / 3.0f, r0);
-    v = x * (r0 * r0);
+    v = (x * r0) * r0;
     r = r0;
 }
 
@@ -211,7 +211,7 @@ __device__ __forceinline__ void pn_powers(f2 x, const PnBase<f2>&, f2, f2& v, f2
     f2 r0(ra, rb);
     const f2 e = pn_fma(-(x * r0), r0 * r0, f2(1.0f));
     r0 = pn_fma(r0 * e, f2(1.0f / 3.0f), r0);
-    v = x * (r0 * r0);
+    v = (x * r0) * r0;
     r = r0;
 }
 
@@ -279,11 +279,11 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     const real beta = sc.hBc * x2;
     f[1] = beta * c1x; f[2] = beta * c1y; f[3] = beta * c1z;
     f[4] = beta * c2x; f[5] = beta * c2y; f[6] = beta * c2z;
-    // Eq. (3): L_dot = -v/(eta M^2) (S1_dot + S2_dot) = (G v beta) (c_1 + c_2)
-    const real gb = (c.G * v) * beta;
-    f[7] = gb * (c1x + c2x);
-    f[8] = gb * (c1y + c2y);
-    f[9] = gb * (c1z + c2z);
+    // Eq. (3): L_dot = -v/(eta M^2) (S1_dot + S2_dot)
+    const real gv = c.G * v;
+    f[7] = gv * (f[1] + f[4]);
+    f[8] = gv * (f[2] + f[5]);
+    f[9] = gv * (f[3] + f[6]);
 }
 
 // ---- pair-packed FP32 layout (pn_integrate_packed.cu) -------------------------------------------------------------
@@ -343,10 +343,11 @@ __device__ __forceinline__ void pn_rhs(const f2 (&y)[5], const PnConsts<float>& 
     const float beta = sc.hBc * x2;
     const f2 c1(c1x, c1y), c2(c2x, c2y);
     // Eq. (3)
-    const float gb = (c.G * v) * beta;
+    const float gv = c.G * v;
     f[0] = f2(beta) * c1;
     f[1] = f2(beta) * c2;
-    f[2] = f2(gb) * (c1 + c2);
-    f[3] = f2(f0, beta * c1z);
-    f[4] = f2(beta * c2z, gb * (c1z + c2z));
+    f[2] = f2(gv) * (f[0] + f[1]);
+    const float f3 = beta * c1z, f6 = beta * c2z;
+    f[3] = f2(f0, f3);
+    f[4] = f2(f6, gv * (f3 + f6));
 }
