@@ -75,7 +75,7 @@ static Ctx* ctx_for(void* stream)
 }
 
 // layout of g_small: [0..3] counters (u64), then queue (u32), status (i32)
-struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned int queue2; unsigned int redo_count; unsigned long long skipped[3]; int nonuniform; int pad; };
+struct Small { unsigned long long counters[4]; unsigned int queue; int status; unsigned int queue2; unsigned int redo_count; unsigned long long skipped[3]; int nonuniform; int pad; double uni_row[PN_UNI_ROW]; };
 
 static int ensure_events(Ctx& c)
 {
@@ -178,6 +178,7 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     // A system with an ACCEPTED step beyond the range goes to the wide-range redo pass.
     p.emax = 0.03;
     if (!fixed && rtol > 1e-10) { p.emax = pow(1e-3 * rtol / 0.0852, 1.0 / 9.0); if (p.emax > 0.2) p.emax = 0.2; }
+    pn_host_series(o.term_mask, p.qc);
     p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
     p.fixed_steps = fixed ? o.fixed_steps : 0;
     p.mask = o.term_mask;
@@ -188,7 +189,7 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     }
     p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
     p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = (int*)c.redo.p;
-    p.nonuniform = &small->nonuniform;
+    p.nonuniform = &small->nonuniform; p.uni_row = small->uni_row;
     p.uni_slot = c.slot;
     CK(pn_launch_integrate(p, precision, o.block_threads, o.grid_blocks, s, o.variant));
     CK(cudaEventRecord(c.ev[2], s));
@@ -521,11 +522,12 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
     p.tau = o.tau_land > 0.0 ? o.tau_land : 1e-13;
     p.emax = 0.03;
     if (rtol > 1e-10) { p.emax = pow(1e-3 * rtol / 0.0852, 1.0 / 9.0); if (p.emax > 0.2) p.emax = 0.2; }
+    pn_host_series(o.term_mask, p.qc);
     p.max_steps = o.max_steps > 0 ? o.max_steps : 10000000;
     p.mask = o.term_mask;
     p.queue = &small->queue; p.counters = small->counters; p.status = &small->status;
     p.queue2 = &small->queue2; p.redo_count = &small->redo_count; p.redo_list = redo_list;
-    p.nonuniform = &small->nonuniform;
+    p.nonuniform = &small->nonuniform; p.uni_row = small->uni_row;
     p.uni_slot = -1;
     p.f_specs = c.gen_specs.p; p.f_n_total = n_total; p.f_first = first; p.f_count = count;
     p.f_mom = f_mom; p.f_lock = f_lock; p.f_skipped = f_skip; p.f_hist1 = d.hist1; p.f_hist2 = d.hist2;

@@ -46,10 +46,10 @@
 // pair-packed FP32 kernel (pn_integrate_packed.cu) passes vec = f2, NV = 5: the ten components of ONE system in five
 // register pairs, so that every stage sum below is a packed FFMA2 (two components per issue slot); pn_rhs has an
 // overload for that layout.
-template <bool SLOW, typename real, bool WANT_DY = false, typename vec = real, int NV = 10>
+template <bool SLOW, typename real, bool WANT_DY = false, typename vec = real, int NV = 10, bool FOLD = false>
 __device__ __forceinline__ void pn_dp5_trial(const vec (&y)[NV], const vec (&K1)[NV], real h,
                                              const PnConsts<real>& c, const PnUni<real>& u, const PnBase<real>& base,
-                                             vec (&ynew)[NV], vec (&K7)[NV], vec (&err)[NV], PnBase<real>& base_new, bool& bad,
+                                             vec (&ynew)[NV], vec (&K7)[NV], vec (&err)[NV], PnBase<real>& base_new, PnFlag& bad,
                                              vec* dy = nullptr)
 {
     vec K2[NV], K3[NV], K4[NV], K5[NV], K6[NV], ys[NV];
@@ -58,25 +58,25 @@ __device__ __forceinline__ void pn_dp5_trial(const vec (&y)[NV], const vec (&K1)
     pn_make_scaled(c, h, sc);
 #pragma unroll
     for (int i = 0; i < NV; ++i) ys[i] = pn_fma((vec)DP_A21, K1[i], y[i]);
-    pn_rhs<SLOW>(ys, c, u, sc, base, K2, r_tmp, l_tmp, bad);
+    pn_rhs<SLOW, FOLD>(ys, c, u, sc, base, K2, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < NV; ++i) ys[i] = pn_fma((vec)DP_A32, K2[i], pn_fma((vec)DP_A31, K1[i], y[i]));
-    pn_rhs<SLOW>(ys, c, u, sc, base, K3, r_tmp, l_tmp, bad);
+    pn_rhs<SLOW, FOLD>(ys, c, u, sc, base, K3, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < NV; ++i)
         ys[i] = pn_fma((vec)DP_A43, K3[i], pn_fma((vec)DP_A42, K2[i], pn_fma((vec)DP_A41, K1[i], y[i])));
-    pn_rhs<SLOW>(ys, c, u, sc, base, K4, r_tmp, l_tmp, bad);
+    pn_rhs<SLOW, FOLD>(ys, c, u, sc, base, K4, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < NV; ++i)
         ys[i] = pn_fma((vec)DP_A54, K4[i],
                        pn_fma((vec)DP_A53, K3[i], pn_fma((vec)DP_A52, K2[i], pn_fma((vec)DP_A51, K1[i], y[i]))));
-    pn_rhs<SLOW>(ys, c, u, sc, base, K5, r_tmp, l_tmp, bad);
+    pn_rhs<SLOW, FOLD>(ys, c, u, sc, base, K5, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < NV; ++i)
         ys[i] = pn_fma((vec)DP_A65, K5[i],
                        pn_fma((vec)DP_A64, K4[i],
                               pn_fma((vec)DP_A63, K3[i], pn_fma((vec)DP_A62, K2[i], pn_fma((vec)DP_A61, K1[i], y[i])))));
-    pn_rhs<SLOW>(ys, c, u, sc, base, K6, r_tmp, l_tmp, bad);
+    pn_rhs<SLOW, FOLD>(ys, c, u, sc, base, K6, r_tmp, l_tmp, bad);
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
         if (WANT_DY) {
@@ -93,8 +93,8 @@ __device__ __forceinline__ void pn_dp5_trial(const vec (&y)[NV], const vec (&K1)
                         pn_fma((vec)DP_E5, K5[i],
                                pn_fma((vec)DP_E4, K4[i], pn_fma((vec)DP_E3, K3[i], (vec)DP_E1 * K1[i]))));
     }
-    pn_rhs<SLOW>(ynew, c, u, sc, base, K7, r_tmp, l_tmp, bad);
-    base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.l0 = l_tmp;
+    pn_rhs<SLOW, FOLD>(ynew, c, u, sc, base, K7, r_tmp, l_tmp, bad);
+    base_new.r0 = r_tmp; base_new.r03 = r_tmp * r_tmp * r_tmp; base_new.k6b = l_tmp;
 #pragma unroll
     for (int i = 0; i < NV; ++i) err[i] = pn_fma((vec)DP_E7, K7[i], err[i]);
 }

@@ -54,7 +54,7 @@ __device__ __forceinline__ float pn_err_norm2(const float (&y)[10], const float 
 // (where one lane works and 31 wait): the per-system constants (~10 FP64 divides), the base powers
 // (rcbrt + log), the scaled seed slope K1 = h0 f(y0) and the norm-scaled atol.  One contiguous record of
 // PN_REC reals per system (FP64 320 B, FP32 160 B), so a lane's refill is 20 (10) 16-byte loads.
-//   [0..9] y0   [10..19] K1 = h0 f(y0)   [20..34] PnConsts   [35..37] PnBase   [38] atol |S1|   [39] atol |S2|
+//   [0..9] y0   [10..19] K1 = h0 f(y0)   [20..34] PnConsts   [35..37] PnBase (r0, r0^3, k6b)   [38] atol |S1|   [39] atol |S2|
 // A record with [38] < 0 marks a system the seed kernel has already failed (bad input).
 // The seed record of one valid system: constants, base powers, K1 = h0 f(y0), norm-scaled atol (layout above).
 template <typename real>
@@ -69,10 +69,10 @@ __device__ __forceinline__ void pn_make_record(const double (&y0)[10], double m1
     pn_make_uni<real>(p.mask, u);
     u.emax = (real)p.emax;
     pn_make_consts<real>(m1, m2, p.mask, c);
-    pn_base_init(c.M * y[0], base);
+    pn_base_init(c.M * y[0], c.c6, u.cl, base);
     const real h = p.h0 > 0.0 ? (real)p.h0 : (real)10 * c.M;      // first step (R13); same expression at refill
     real r_tmp, l_tmp;
-    bool bad_tmp = false;
+    PnFlag bad_tmp;
     PnScaled<real> sc;
     pn_make_scaled(c, h, sc);
     pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad_tmp);      // K1 = h0 f(y0)
@@ -88,7 +88,7 @@ __device__ __forceinline__ void pn_make_record(const double (&y0)[10], double m1
     out[20] = c.M; out[21] = c.c2; out[22] = c.c4; out[23] = c.c5; out[24] = c.c6; out[25] = c.c7;
     out[26] = c.p1; out[27] = c.p2; out[28] = c.q1; out[29] = c.q2; out[30] = c.K0; out[31] = c.A1;
     out[32] = c.A2; out[33] = c.Bc; out[34] = c.G;
-    out[35] = base.r0; out[36] = base.r03; out[37] = base.l0;
+    out[35] = base.r0; out[36] = base.r03; out[37] = base.k6b;
     out[38] = (real)(p.atol * (s1 > 0.0 ? s1 : 1.0));
     out[39] = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
 }
@@ -140,6 +140,23 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     if (m1 != p.masses[0] || m2 != p.masses[p.n]) *p.nonuniform = 1;      // benign race: every writer stores 1
     real out[PN_REC];
     pn_make_record<real>(y0, m1, m2, p, out);
+    if (i == 0 && p.uni_slot >= 0) {
+        // the uniform-mass kernel's constants, in the form it evaluates the brace of Eq. (1) in: everything
+        // the brace is linear in arrives multiplied by KB = K0/Bc (pn_rhs.cuh, FOLD), so omega_dot = (beta v^5) brace'
+        //   [0..14] PnConsts (c2 ... c7, p1, p2, q1, q2 folded)   [15] c0'   [16] c3'   [17] cl'   [18..24] qc'   [25] KB
+        PnConsts<double> c;
+        PnUni<double> u;
+        pn_make_uni<double>(p.mask, u);
+        pn_make_consts<double>(m1, m2, p.mask, c);
+        const double KB = c.K0 / c.Bc;
+        double* row = p.uni_row;
+        row[0] = c.M; row[1] = KB * c.c2; row[2] = KB * c.c4; row[3] = KB * c.c5; row[4] = KB * c.c6; row[5] = KB * c.c7;
+        row[6] = KB * c.p1; row[7] = KB * c.p2; row[8] = KB * c.q1; row[9] = KB * c.q2; row[10] = c.K0; row[11] = c.A1;
+        row[12] = c.A2; row[13] = c.Bc; row[14] = c.G; row[15] = KB * u.c0; row[16] = KB * u.c3; row[17] = KB * u.cl;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) row[18 + k] = KB * p.qc[k];
+        row[25] = KB;
+    }
     using vec = typename PnVec<real>::type;           // 16-byte stores
     vec* dst = (vec*)rec;
     constexpr int W = 16 / (int)sizeof(real);
@@ -160,7 +177,7 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
 // The launcher copies system 0's record into the row on the stream and launches BOTH the uniform-mass and the generic
 // kernel (p.uni_slot >= 0 marks such a pair); each looks at the seed kernel's verdict and the one that does not apply
 // returns at once, so no host synchronisation is needed and async calls keep the fast path.
-__constant__ double pn_uni_table[PN_UNI_SLOTS][16];
+__constant__ double pn_uni_table[PN_UNI_SLOTS][PN_UNI_ROW];
 
 // ---- fused ensemble mode (FUSED = true; pn_run_ensembles): seed in, statistics out ----------------
 // The work pull DRAWS the system (counter-based Philox + sphere sampling, pn_gen.cuh: the same bits as pn_generate)
@@ -358,7 +375,7 @@ __device__ __noinline__ void pn_fused_finish_batch(const PnKernelParams& p, cons
 // results are the same and nothing spills.
 __device__ __noinline__ void pn_dp5_trial_outofline(const double (&y)[10], const double (&K1)[10], double h, const PnConsts<double>& c,
                                                     const PnUni<double>& u, const PnBase<double>& base, double (&ynew)[10],
-                                                    double (&K7)[10], double (&err)[10], PnBase<double>& base_new, bool& bad)
+                                                    double (&K7)[10], double (&err)[10], PnBase<double>& base_new, PnFlag& bad)
 {
     pn_dp5_trial<true>(y, K1, h, c, u, base, ynew, K7, err, base_new, bad);
 }
@@ -398,17 +415,24 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
     u.emax = (real)p.emax;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) u.qc[k] = (real)p.qc[k];
     pn_make_consts<real>(0.5, 0.5, 0u, c);
+    real KB = (real)1;               // UNI: the factor K0/Bc the brace constants of the table row carry (pn_rhs.cuh, FOLD)
     if constexpr (UNI >= 0) {
         const double* uc = pn_uni_table[UNI];
         c.M = (real)uc[0]; c.c2 = (real)uc[1]; c.c4 = (real)uc[2]; c.c5 = (real)uc[3]; c.c6 = (real)uc[4]; c.c7 = (real)uc[5];
         c.p1 = (real)uc[6]; c.p2 = (real)uc[7]; c.q1 = (real)uc[8]; c.q2 = (real)uc[9]; c.K0 = (real)uc[10];
         c.A1 = (real)uc[11]; c.A2 = (real)uc[12]; c.Bc = (real)uc[13]; c.G = (real)uc[14];
+        u.c0 = (real)uc[15]; u.c3 = (real)uc[16]; u.cl = (real)uc[17];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) u.qc[k] = (real)uc[18 + k];
+        KB = (real)uc[25];
     }
 #pragma unroll
     for (int i = 0; i < 10; ++i) { y[i] = (real)0; k1[i] = (real)0; yd[i] = 0.0; }
     y[0] = (real)0.01; y[9] = (real)1; yd[0] = 0.01; yd[9] = 1.0;
-    pn_base_init(c.M * y[0], base);
+    pn_base_init(c.M * y[0], c.c6, u.cl, base);
     real h = (real)0;
     float atS1 = fmaxf((float)p.atol, 1e-30f), atS2 = atS1;
     double t = 0.0;
@@ -431,7 +455,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
             c.p1 = rec[26]; c.p2 = rec[27]; c.q1 = rec[28]; c.q2 = rec[29]; c.K0 = rec[30]; c.A1 = rec[31];
             c.A2 = rec[32]; c.Bc = rec[33]; c.G = rec[34];
         }
-        base.r0 = rec[35]; base.r03 = rec[36]; base.l0 = rec[37];
+        base.r0 = rec[35]; base.r03 = rec[36]; base.k6b = UNI >= 0 ? KB * rec[37] : rec[37];
         atS1 = fmaxf((float)rec[38], 1e-30f); atS2 = fmaxf((float)rec[39], 1e-30f);   // keeps every scale > 0 (atol = 0 is allowed)
         t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
         idx = i;
@@ -517,10 +541,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         // ---------------- one DP5(4) trial step, all lanes, one basic block ----------------
         real ynew[10], k7[10], err[10], dy[10];
         PnBase<real> base_new;
-        bool bad = false;
-        if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad, dy);
-        else if constexpr (FUSED && SLOW) pn_dp5_trial_outofline(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
-        else pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
+        PnFlag flag;
+        if constexpr (MIXED) pn_dp5_trial<SLOW, real, true>(y, k1, h, c, u, base, ynew, k7, err, base_new, flag, dy);
+        else if constexpr (FUSED && SLOW) pn_dp5_trial_outofline(y, k1, h, c, u, base, ynew, k7, err, base_new, flag);
+        else pn_dp5_trial<SLOW, real, false, real, 10, (UNI >= 0)>(y, k1, h, c, u, base, ynew, k7, err, base_new, flag);
+        const bool bad = flag.out_of_range(u.emax);
         // scaled RMS error norm (R6): sc_j = atol N_j + rtol max(|y_j|, |ynew_j|), E^2 = mean (err_j/sc_j)^2.
         // It only decides accept/reject and the next step size, so ~1e-6 relative accuracy is ample:
         // FP64: the larger magnitude is picked by comparing the high words (integer pipe), 1/sc_j is the raw
@@ -644,7 +669,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
         }
         base.r0 = accept ? base_new.r0 : base.r0;
         base.r03 = accept ? base_new.r03 : base.r03;
-        base.l0 = accept ? base_new.l0 : base.l0;
+        base.k6b = accept ? base_new.k6b : base.k6b;
         h *= ratio;
     }
 
@@ -708,19 +733,21 @@ __global__ void __launch_bounds__(BLOCK) pn_integrate_fixed_kernel(const PnKerne
     PnUni<real> u;
     pn_make_uni<real>(p.mask, u);
     u.emax = (real)p.emax;
-    pn_base_init(c.M * y[0], base);
+#pragma unroll
+    for (int k = 0; k < 7; ++k) u.qc[k] = (real)p.qc[k];
+    pn_base_init(c.M * y[0], c.c6, u.cl, base);
     const real h = (real)(p.h0 > 0.0 ? p.h0 : 10.0 * (m1 + m2));
     real r_tmp, l_tmp;
     PnScaled<real> sc;
     pn_make_scaled(c, h, sc);
-    bool bad = false;
-    pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, bad);
+    PnFlag flag0;
+    pn_rhs<true>(y, c, u, sc, base, k1, r_tmp, l_tmp, flag0);
     double t = 0.0;
     for (int s = 0; s < p.fixed_steps; ++s) {
         real ynew[10], k7[10], err[10];
-        bad = false;
-        pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
-        if (!SLOW && bad) {
+        PnFlag flag;
+        pn_dp5_trial<SLOW>(y, k1, h, c, u, base, ynew, k7, err, base_new, flag);
+        if (!SLOW && flag.out_of_range(u.emax)) {
             p.redo_list[atomicAdd(p.redo_count, 1u)] = i;
             return;
         }
@@ -836,8 +863,8 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
             p.uni_slot = slot;
             // uniform-mass fast path, decided on the device: system 0's constants (bitwise those of its seed record) go
             // into the __constant__ table on the stream, then both kernels of the pair are launched
-            if ((e = cudaMemcpyToSymbolAsync(pn_uni_table, (const double*)p.seed + 20, 15 * sizeof(double),
-                                             (size_t)p.uni_slot * 16 * sizeof(double), cudaMemcpyDeviceToDevice, s)) != cudaSuccess)
+            if ((e = cudaMemcpyToSymbolAsync(pn_uni_table, p.uni_row, PN_UNI_ROW * sizeof(double),
+                                             (size_t)p.uni_slot * PN_UNI_ROW * sizeof(double), cudaMemcpyDeviceToDevice, s)) != cudaSuccess)
                 return e;
             static_assert(PN_UNI_SLOTS == 4, "one instantiation of the uniform-mass kernel per table row");
             if (slot == 0) e = launch_adaptive<double, 128, 2, false, false, 0>(p, grid_blocks, s);

@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_pairs_kernel(const P
 #pragma unroll
     for (int j = 0; j < 5; ++j) { y[j] = f2(0.0f); k1[j] = f2(0.0f); }
     pn_pair_set<0>(y, 0.01f); pn_pair_set<9>(y, 1.0f);
-    pn_base_init(0.01f, base);
+    pn_base_init(0.01f, 0.0f, 0.0f, base);
     float h = 0.0f;
     const float rtol = (float)p.rtol, atol1 = fmaxf((float)p.atol, 1e-30f);
     float atS1 = atol1, atS2 = atol1;
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_pairs_kernel(const P
         // ---------------- one DP5(4) trial step, all lanes, one basic block; stage sums packed ----------------
         f2 ynew[5], k7[5], err[5];
         PnBase<float> base_new;
-        bool bad = false;
+        PnFlag bad;
         pn_dp5_trial<false, float, false, f2, 5>(y, k1, h, c, u, base, ynew, k7, err, base_new, bad);
         // scaled RMS error norm (R6): scales and ratios packed, the sum in component order as in the scalar kernel
         f2 q[5];

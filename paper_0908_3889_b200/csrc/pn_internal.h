@@ -4,6 +4,7 @@
 
 #define PN_ORDER_BUCKETS 2048
 #define PN_UNI_SLOTS 4
+#define PN_UNI_ROW 32
 
 // Arguments of the integrator kernels.  All arrays are DEVICE pointers in SoA layout with stride n:
 // y0[c*n + i], masses[j*n + i], yf[c*n + i].
@@ -20,6 +21,7 @@ struct PnKernelParams {
     double omega0;       // > 0: every initial omega must match it to 1e-12 relative
     double omegaf, rtol, atol, h0, tau;
     double emax;         // FP64 fast kernel: range of the cbrt/log series, |1 - x/x0| <= emax (pn_rhs.cuh)
+    double qc[7];        // FP64 fast kernel: cl / k, the log series with its coefficient folded in (pn_host_series, pn_rhs.cuh)
     int max_steps;
     int fixed_steps;
     unsigned mask;
@@ -30,6 +32,7 @@ struct PnKernelParams {
     unsigned long long* counters;   // [0] trial steps [1] rejected [2] landing trials [3] failed systems
     int* status;                    // worst pn_status seen on the device (atomicMax)
     int* nonuniform;                // set by the seed kernel if some system's masses differ from system 0's (or system 0 is bad)
+    double* uni_row;                // [PN_UNI_ROW] written by the seed kernel: system 0's constants in the form the uniform-mass kernel reads
     int uni_slot;                   // FP64 uniform-mass path: slot of the __constant__ table that holds system 0's PnConsts; < 0: off
     float* keys;                    // [n] or null: expected-cost keys written by the seed kernel (queue ordering)
     unsigned int* order_scratch;    // [PN_ORDER_BUCKETS + 2]: bucket cursors, then the bit patterns of the smallest / largest key
@@ -48,6 +51,15 @@ struct PnKernelParams {
     int f_bins1, f_bins2;
     unsigned f_resident;            // lanes of the persistent grid (grid x block): the length of the queue's last wave
 };
+
+// cl / k, k = 1 ... 7, for PnKernelParams::qc: cl = -(856/105)(2/3) is the coefficient of ln(M omega) in the v^6 term of
+// Eq. (1) (pn_rhs.cuh: pn_make_uni; term_mask bit 6 switches the 3PN term off, mask 0 means all terms)
+static inline void pn_host_series(unsigned mask, double (&qc)[7])
+{
+    const bool on = mask == 0 || ((mask >> 6) & 1u);
+    const double cl = on ? -(856.0 / 105.0) * (2.0 / 3.0) : 0.0;
+    for (int k = 0; k < 7; ++k) qc[k] = cl / (double)(k + 1);
+}
 
 // launchers (pn_integrate.cu); block_threads / grid_blocks = 0 choose the defaults
 // variant bits (pn_options.variant): 1 = always the generic FP64 kernel (per-lane constants), 2 = always the scalar FP32 kernel

@@ -47,6 +47,16 @@ struct PnUni {
     real c3;   // 4 pi, spin-independent part of the v^3 coefficient
     real cl;   // coefficient of ln(x) inside the v^6 term: -(856/105)(2/3)
     real emax; // FP64 fast kernel: largest |1 - x/x0| the cbrt/log series are trusted for (set by the launcher)
+    real qc[7]; // FP64 fast kernel: cl / k, k = 1 ... 7: the log series with cl folded in (set by the launcher, pn_powers)
+};
+// Range flag of a trial step.  `bad`: a stage left the range of the wide-range (SLOW) evaluation.  `emx`: the FP64 fast
+// path's running maximum of |e| = |1 - x/x0| over the stages, kept as the float whose bits are the HIGH word of |e|
+// (high words of doubles order like floats): one FMNMX per stage instead of a DSETP, compared with emax once per step.
+struct PnFlag {
+    bool bad; float emx;
+    __device__ __forceinline__ PnFlag() : bad(false), emx(0.0f) {}
+    __device__ __forceinline__ bool out_of_range(double emax) const { return bad || emx > __int_as_float(__double2hiint(emax)); }
+    __device__ __forceinline__ bool out_of_range(float) const { return bad; }
 };
 template <typename real>
 __device__ __forceinline__ void pn_make_uni(unsigned mask, PnUni<real>& u)
@@ -56,6 +66,8 @@ __device__ __forceinline__ void pn_make_uni(unsigned mask, PnUni<real>& u)
     u.c3 = (real)((mask >> 3) & 1u ? 4.0 * 3.14159265358979323846 : 0.0);
     u.cl = (real)((mask >> 6) & 1u ? -(856.0 / 105.0) * (2.0 / 3.0) : 0.0);
     u.emax = (real)0.03;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) u.qc[k] = (real)0;      // the FP64 kernels take them from the launch parameters (uniform operands)
 }
 
 template <typename real>
@@ -102,34 +114,37 @@ __device__ __forceinline__ void pn_make_consts(double m1, double m2, unsigned ma
 // accumulates in r; l0 is chained once per accepted step with a truncation error < 3e-15 at the switch
 // point |e| = 0.03, beyond which the trial step is repeated with the library functions (rare).  ~22 FMA-pipe
 // instructions per stage.  FP32 uses cbrtf and the MUFU log directly.
-template <typename real> struct PnBase { real r0, r03, l0; };
+// k6b = c6 + cl ln x0: the coefficient of v^6 in the brace of Eq. (1) AT the base point.  The log enters the RHS only
+// through k6 = c6 + cl ln x, so the series carries cl (k6 = k6b - e sum_k (cl/k) e^{k-1}) and one FMA per evaluation
+// (forming ln x, then cl ln x + c6) is saved.
+template <typename real> struct PnBase { real r0, r03, k6b; };
 
-__device__ __forceinline__ void pn_base_init(double x, PnBase<double>& b)
+__device__ __forceinline__ void pn_base_init(double x, double c6, double cl, PnBase<double>& b)
 {
     b.r0 = rcbrt(x);
     b.r03 = b.r0 * b.r0 * b.r0;
-    b.l0 = log(x);
+    b.k6b = fma(cl, log(x), c6);
 }
-__device__ __forceinline__ void pn_base_init(float, PnBase<float>& b) { b.r0 = b.r03 = b.l0 = 0.0f; }
-__device__ __forceinline__ void pn_base_init(f2, PnBase<f2>& b) { b.r0 = b.r03 = b.l0 = f2(0.0f); }
+__device__ __forceinline__ void pn_base_init(float, float, float, PnBase<float>& b) { b.r0 = b.r03 = b.k6b = 0.0f; }
 
-// r = x^{-1/3}, lnx = ln x  ->  returned so that an accepted step can adopt them as the next base.
-// SLOW = false: series only, branch-free; `bad` is raised when |e| is outside the series' range, and the
-// caller then repeats the whole trial step with SLOW = true (library rcbrt/log), so the hot loop stays one
+// r = x^{-1/3} and k6 = c6 + cl ln x  ->  returned so that an accepted step can adopt them as the next base.
+// SLOW = false: series only, branch-free; the running maximum of |e| is kept in `flag`, and when it leaves the series'
+// range the caller repeats the whole trial step with SLOW = true (wide-range evaluation), so the hot loop stays one
 // basic block.
 template <bool SLOW>
-__device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, double emax, double& v, double& lnx, double& r, bool& bad)
+__device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, double c6, const PnUni<double>& u, double& k6, double& r, PnFlag& flag)
 {
     if (SLOW) {
         // wide-range, call-free evaluation about the same base, exact to rounding for x/x0 in [0.4, 2]:
         //   x^{-1/3} = r0 u,  u = rho^{-1/3} by five cubically convergent iterations u <- u (1 + d/3 + 2 d^2/9),
         //              d = 1 - rho u^3,  rho = x/x0 = 1 - e
         //   ln x     = l0 + 2 atanh(w),  w = (rho - 1)/(rho + 1) = -e/(2 - e);  1/(2 - e) by Newton, no divide
+        //   (k6b stands for c6 + cl l0, so k6 = k6b + cl 2 atanh(w))
         // Outside that range (omega more than doubled or halved inside ONE step) e is clamped, the values are
-        // finite but wrong, and `bad` tells the caller to reject the step.
+        // finite but wrong, and `flag.bad` tells the caller to reject the step.
         const double e_raw = fma(-x, b.r03, 1.0);
         const double e = fmin(fmax(e_raw, -1.0), 0.6);
-        bad = bad || (e_raw < -1.0) || (e_raw > 0.6);
+        flag.bad = flag.bad || (e_raw < -1.0) || (e_raw > 0.6);
         const double rho = 1.0 - e;
         double uu = 1.0;
 #pragma unroll
@@ -146,12 +161,14 @@ __device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, dou
         double A = 1.0 / 45.0;
 #pragma unroll
         for (int k = 21; k >= 1; --k) A = fma(A, w2, 1.0 / (double)(2 * k + 1));
-        lnx = fma(2.0 * w, fma(A, w2, 1.0), b.l0);
+        k6 = fma(u.cl, (2.0 * w) * fma(A, w2, 1.0), b.k6b);
     } else {
         const double e = fma(-x, b.r03, 1.0);
-        bad = bad || (fabs(e) > emax);      // false for NaN: a non-finite state is reported as such, not redone
+        // range check without a DSETP: running maximum of the high words of |e| (NaN is ignored: a non-finite state is
+        // reported as such, not redone)
+        flag.emx = fmaxf(flag.emx, fabsf(__int_as_float(__double2hiint(e))));
         // (1-e)^{-1/3} = 1 + e S(e),  S = sum_{k=1..9} s_k e^{k-1},  s_k = prod_{j<k}(1/3 + j)/k!
-        // log1p(-e)    =   - e Q(e),  Q = sum_{k=1..9} e^{k-1}/k
+        // log1p(-e)    =   - e Q(e),  Q = sum_{k=1..7} e^{k-1}/k;  the series carries cl: qc_k = cl/k
         // truncation s10 e^9 < 6.1e-17 for |e| <= 0.03.  Even/odd split in e halves the dependent FMA chains.
         // emax = 0.03 at rtol <= 1e-10 and in fixed-step mode; at looser tolerances it grows as rtol^{1/9}, which keeps
         // the truncation below 1e-3 rtol: a run at rtol 1e-7 need not evaluate f to 1e-16.
@@ -165,54 +182,27 @@ __device__ __forceinline__ void pn_powers(double x, const PnBase<double>& b, dou
         // ln x enters only through cl ln(x) x^2 in the brace (|cl| = 5.4, x^2 <= 2.5e-3 for omega <= 0.05/M), so an
         // absolute error of 8e-14 in ln x (the e^8/8 term at the |e| = 0.03 limit; 1e-17 at the typical |e| < 0.01)
         // is below 1.1e-15 relative in omega_dot: Q stops at e^6/7.
-#ifdef PN_LOG_FULL
-        double Qa = 1.0 / 9.0, Qb = 1.0 / 8.0;
-        Qa = fma(Qa, e2, 1.0 / 7.0);  Qb = fma(Qb, e2, 1.0 / 6.0);
-#else
-        double Qa = 1.0 / 7.0, Qb = 1.0 / 6.0;
-#endif
-        Qa = fma(Qa, e2, 1.0 / 5.0);  Qb = fma(Qb, e2, 1.0 / 4.0);
-        Qa = fma(Qa, e2, 1.0 / 3.0);  Qb = fma(Qb, e2, 1.0 / 2.0);
-        Qa = fma(Qa, e2, 1.0);
+        double Qa = u.qc[6], Qb = u.qc[5];
+        Qa = fma(Qa, e2, u.qc[4]);  Qb = fma(Qb, e2, u.qc[3]);
+        Qa = fma(Qa, e2, u.qc[2]);  Qb = fma(Qb, e2, u.qc[1]);
+        Qa = fma(Qa, e2, u.qc[0]);
         const double Q = fma(Qb, e, Qa);
         r = fma(b.r0 * e, S, b.r0);
-        lnx = fma(-e, Q, b.l0);
+        k6 = fma(-e, Q, b.k6b);
     }
-    v = (x * r) * r;      // the caller's v2 = x r is the same product (CSE): v costs one multiply
 }
 template <bool SLOW>
-__device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float, float& v, float& lnx, float& r, bool&)
+__device__ __forceinline__ void pn_powers(float x, const PnBase<float>&, float c6, const PnUni<float>& u, float& k6, float& r, PnFlag&)
 {
     // x > 0 always (omega > 0, M > 0): one lg2 serves both functions, no special-case code (cbrtf carries branches
     // for 0, inf and denormals).  ln x = lg2(x) ln 2; x^{-1/3} = ex2(-lg2(x)/3) polished by one Newton step
-    // r <- r + r (1 - x r^3)/3 (seed error ~2e-7 -> ~1e-13, below float rounding); v = x r^2.
+    // r <- r + r (1 - x r^3)/3 (seed error ~2e-7 -> ~1e-13, below float rounding).
     float l2, r0;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(x));
-    lnx = l2 * 0.693147180559945f;
+    k6 = fmaf(u.cl, l2 * 0.693147180559945f, c6);
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r0) : "f"(l2 * (-1.0f / 3.0f)));
     const float e = fmaf(-x * r0, r0 * r0, 1.0f);
-    r0 = fmaf(r0 * e, 1.0f / 3.0f, r0);
-    v = (x * r0) * r0;
-    r = r0;
-}
-
-// packed FP32 (two systems per lane): the special-function unit is per component, the polish and the powers are packed
-template <bool SLOW>
-__device__ __forceinline__ void pn_powers(f2 x, const PnBase<f2>&, f2, f2& v, f2& lnx, f2& r, bool&)
-{
-    float la, lb, ra, rb;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(la) : "f"(x.v.x));
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lb) : "f"(x.v.y));
-    const f2 l2(la, lb);
-    lnx = l2 * f2(0.693147180559945f);
-    const f2 t = l2 * f2(-1.0f / 3.0f);
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ra) : "f"(t.v.x));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(rb) : "f"(t.v.y));
-    f2 r0(ra, rb);
-    const f2 e = pn_fma(-(x * r0), r0 * r0, f2(1.0f));
-    r0 = pn_fma(r0 * e, f2(1.0f / 3.0f), r0);
-    v = (x * r0) * r0;
-    r = r0;
+    r = fmaf(r0 * e, 1.0f / 3.0f, r0);
 }
 
 // The slopes are produced already multiplied by the step size h ("scaled slopes" K = h f): the four
@@ -228,19 +218,21 @@ __device__ __forceinline__ void pn_make_scaled(const PnConsts<real>& c, real h, 
     s.hK0 = h * c.K0; s.hBc = h * c.Bc;
 }
 
-// K = h f(y).  ~70 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and
-// lnx_out = ln x of this evaluation are handed back for the base update of an accepted step.
-template <bool SLOW, typename real>
+// K = h f(y).  ~65 FMA-pipe instructions plus pn_powers; no memory traffic.  r_out = x^{-1/3} and k6_out = c6 + cl ln x
+// of this evaluation are handed back for the base update of an accepted step.
+// FOLD (the uniform-mass FP64 kernel): the constants of the brace (c2 ... c7, p, q in `c`; c0, c3, cl, qc in `u`) arrive
+// multiplied by K0/Bc, so that omega_dot = (beta v^5) brace' with beta = h Bc x^2 (needed anyway): one multiply fewer.
+template <bool SLOW, bool FOLD = false, typename real>
 __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>& c, const PnUni<real>& u,
                                        const PnScaled<real>& sc, const PnBase<real>& base,
-                                       real (&f)[10], real& r_out, real& lnx_out, bool& bad)
+                                       real (&f)[10], real& r_out, real& k6_out, PnFlag& flag)
 {
     const real x = c.M * y[0];
-    real v, lnx, r;
-    pn_powers<SLOW>(x, base, u.emax, v, lnx, r, bad);
-    r_out = r; lnx_out = lnx;
-    // x^{2/3} straight from r = x^{-1/3} (one multiply after r, not two): the powers are ready earlier in the chain
-    const real x2 = x * x, v2 = x * r, v4 = v2 * v2, v5 = v4 * v;
+    real k6, r;
+    pn_powers<SLOW>(x, base, c.c6, u, k6, r, flag);
+    r_out = r; k6_out = k6;
+    // x^{2/3} straight from r = x^{-1/3}, v = x^{1/3} from it with one more multiply
+    const real x2 = x * x, v2 = x * r, v = v2 * r, v4 = v2 * v2, v5 = v4 * v;
 
     const real S1x = y[1], S1y = y[2], S1z = y[3];
     const real S2x = y[4], S2y = y[5], S2z = y[6];
@@ -253,14 +245,14 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     // Eq. (1): coefficients of v^3, v^4, v^6 carry the spin-orbit, spin-spin, log pieces
     const real k3 = pn_fma(c.p1, LS1, pn_fma(c.p2, LS2, u.c3));
     const real k4 = pn_fma(c.q1, S12, pn_fma(c.q2 * LS1, LS2, c.c4));
-    const real k6 = pn_fma(u.cl, lnx, c.c6);
     // Estrin form, brace = c0 + v2 (c2 + k3 v) + v4 ((k4 + c5 v) + v2 (k6 + c7 v)): the same six FMAs as Horner's
     // rule in a dependency chain of three instead of six
     const real e67 = pn_fma(c.c7, v, k6), e45 = pn_fma(c.c5, v, k4), e23 = pn_fma(k3, v, c.c2);
     const real hi = pn_fma(e67, v2, e45);
     real B = pn_fma(e23, v2, u.c0);
     B = pn_fma(hi, v4, B);
-    f[0] = (sc.hK0 * (v5 * x2)) * B;
+    const real beta = sc.hBc * x2;
+    f[0] = FOLD ? (beta * v5) * B : (sc.hK0 * (v5 * x2)) * B;
 
     // Eq. (4) over beta = h x^2/(2M^3): Omega_1/beta = gamma1 L + S2, Omega_2/beta = gamma2 L + S1.  gamma_i needs only
     // r and a dot product, so the cross products below do not wait for the powers of v; -3 is an immediate operand, so
@@ -276,7 +268,6 @@ __device__ __forceinline__ void pn_rhs(const real (&y)[10], const PnConsts<real>
     const real c2x = pn_fma(O2y, S2z, -(O2z * S2y));
     const real c2y = pn_fma(O2z, S2x, -(O2x * S2z));
     const real c2z = pn_fma(O2x, S2y, -(O2y * S2x));
-    const real beta = sc.hBc * x2;
     f[1] = beta * c1x; f[2] = beta * c1y; f[3] = beta * c1z;
     f[4] = beta * c2x; f[5] = beta * c2y; f[6] = beta * c2z;
     // Eq. (3): L_dot = -v/(eta M^2) (S1_dot + S2_dot)
@@ -299,16 +290,16 @@ __device__ constexpr int PN_PAIR_HALF[10] = {0, 0, 1, 1, 0, 1, 0, 0, 1, 1};
 template <int I> __device__ __forceinline__ float pn_pair_get(const f2 (&a)[5]) { return f2_get<PN_PAIR_HALF[I]>(a[PN_PAIR_OF[I]]); }
 template <int I> __device__ __forceinline__ void pn_pair_set(f2 (&a)[5], float x) { f2_set<PN_PAIR_HALF[I]>(a[PN_PAIR_OF[I]], x); }
 
-template <bool SLOW>
+template <bool SLOW, bool FOLD = false>
 __device__ __forceinline__ void pn_rhs(const f2 (&y)[5], const PnConsts<float>& c, const PnUni<float>& u,
                                        const PnScaled<float>& sc, const PnBase<float>& base,
-                                       f2 (&f)[5], float& r_out, float& lnx_out, bool& bad)
+                                       f2 (&f)[5], float& r_out, float& k6_out, PnFlag& flag)
 {
     const float x = c.M * y[3].v.x;
-    float v, lnx, r;
-    pn_powers<SLOW>(x, base, u.emax, v, lnx, r, bad);
-    r_out = r; lnx_out = lnx;
-    const float x2 = x * x, v2 = x * r, v4 = v2 * v2, v5 = v4 * v;
+    float k6, r;
+    pn_powers<SLOW>(x, base, c.c6, u, k6, r, flag);
+    r_out = r; k6_out = k6;
+    const float x2 = x * x, v2 = x * r, v = v2 * r, v4 = v2 * v2, v5 = v4 * v;
 
     const float S1x = y[0].v.x, S1y = y[0].v.y, S1z = y[3].v.y;
     const float S2x = y[1].v.x, S2y = y[1].v.y, S2z = y[4].v.x;
@@ -320,7 +311,6 @@ __device__ __forceinline__ void pn_rhs(const f2 (&y)[5], const PnConsts<float>& 
 
     const float k3 = fmaf(c.p1, LS1, fmaf(c.p2, LS2, u.c3));
     const float k4 = fmaf(c.q1, S12, fmaf(c.q2 * LS1, LS2, c.c4));
-    const float k6 = fmaf(u.cl, lnx, c.c6);
     const float e67 = fmaf(c.c7, v, k6), e45 = fmaf(c.c5, v, k4), e23 = fmaf(k3, v, c.c2);
     const float hi = fmaf(e67, v2, e45);
     float B = fmaf(e23, v2, u.c0);

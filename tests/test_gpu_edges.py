@@ -176,23 +176,39 @@ def test_loose_tolerance_uses_the_redo_pass(pn, oracle):
     assert (np.abs(g["final"] - r["final"]) / comp_scale(y0[:64])).max() <= 1e-11
 
 
-def test_uniform_mass_fast_path_is_bit_identical(pn):
-    """FP64 batches whose systems all have the masses of system 0 run a kernel that takes the 15 mass-dependent
-    constants as kernel parameters.  Same constants, same arithmetic: the results are bit-identical to
-    the generic kernel's; one deviating system anywhere in the batch switches the whole launch to the generic kernel."""
+def close_runs(a, b, frac_same_steps=0.98):
+    """Two FP64 runs of the same systems whose arithmetic differs only in rounding (constants folded differently): the
+    same step sequence for almost every system, final states equal to rounding-error growth there (1e-11), and to the
+    integration tolerance (1e-8) for the few systems where an accept/reject decision with E within rounding of 1 fell
+    the other way."""
+    same = a["steps"] == b["steps"]
+    assert same.mean() >= frac_same_steps, same.mean()
+    assert np.abs(a["final"][same] - b["final"][same]).max() <= 1e-11
+    assert np.abs(a["final"] - b["final"]).max() <= 1e-8
+    assert np.abs(a["time"] / b["time"] - 1).max() <= 1e-9
+
+
+def test_uniform_mass_fast_path_matches_the_generic_kernel(pn):
+    """FP64 batches whose systems all have the masses of system 0 run a kernel that takes the mass-dependent constants
+    from a __constant__ table row, with the factor K0/Bc folded into the constants of the brace of Eq. (1)
+    (one multiply fewer per evaluation), so its results equal the generic kernel's to rounding, not to the bit; one
+    deviating system anywhere in the batch switches the whole launch to the generic kernel, bit for bit."""
     cfg = W.with_size(W.CONFIGS["C4"], 3000 + 17)
     y0, m = W.generate(cfg)
     a = gpu_integrate(pn, y0, m, cfg)
     b = gpu_integrate(pn, y0, m, cfg, variant=1)          # pn_options.variant bit 0: always the generic kernel
+    assert not np.array_equal(a["final"], b["final"])     # the fast path did run
+    close_runs(a, b)
+    a2 = gpu_integrate(pn, y0, m, cfg)
     for k in ("final", "steps", "time", "rejected"):
-        assert np.array_equal(a[k], b[k]), k
-    # a batch that is uniform except for its last system, and one whose system 0 is invalid
+        assert np.array_equal(a[k], a2[k]), k              # and is deterministic
+    # a batch that is uniform except for its last system, and one whose system 0 is invalid: the generic kernel runs
     m2 = m.copy(); m2[-1] = [0.5, 0.5]
     c = gpu_integrate(pn, y0, m2, cfg)
-    assert np.array_equal(c["final"][:-1], a["final"][:-1]) and not np.array_equal(c["final"][-1], a["final"][-1])
+    assert np.array_equal(c["final"][:-1], b["final"][:-1]) and not np.array_equal(c["final"][-1], b["final"][-1])
     m3 = m.copy(); m3[0, 0] = -1.0
     d = gpu_integrate(pn, y0, m3, cfg, allow_failures=True)
-    assert d["steps"][0] == -5 and np.array_equal(d["final"][1:], a["final"][1:])
+    assert d["steps"][0] == -5 and np.array_equal(d["final"][1:], b["final"][1:])
 
 
 def test_large_batch_2_26_systems(pn):
@@ -283,7 +299,7 @@ def test_async_calls_keep_their_status_and_scratch(pn):
     ref3 = gpu_integrate(pn, y3, m3, cfg3)
     ref4 = gpu_integrate(pn, y4, m4, cfg4)
     ref4g = gpu_integrate(pn, y4, m4, cfg4, variant=1)
-    assert np.array_equal(ref4["final"], ref4g["final"])
+    close_runs(ref4, ref4g)
 
     def bufs(n):
         return (torch.full((n, 10), float("nan"), dtype=torch.float64, device=dev), torch.zeros(n, dtype=torch.int32, device=dev))
