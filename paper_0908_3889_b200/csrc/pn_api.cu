@@ -532,6 +532,11 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
     p.f_specs = c.gen_specs.p; p.f_n_total = n_total; p.f_first = first; p.f_count = count;
     p.f_mom = f_mom; p.f_lock = f_lock; p.f_skipped = f_skip; p.f_hist1 = d.hist1; p.f_hist2 = d.hist2;
     p.f_bins1 = bins1; p.f_bins2 = bins2;
+    // ONE ensemble with fixed masses (every ensemble of the paper's section V; the 3.6e8-system uniformity run): the
+    // uniform-mass fast kernel, constants from this stream context's row of the table.  Several ensembles
+    // share chunks, so they take the generic kernel (a launch per ensemble would pay a drain tail per ensemble).
+    const bool fixed_masses = ens[0].m1_fixed > 0.0 || !(ens[0].q_hi > ens[0].q_lo);
+    const int uni_slot = (G == 1 && fixed_masses && !(o.variant & 1)) ? c.slot : -1;
     CK(cudaEventRecord(c.ev[1], s));
     for (long long lo = 0; lo < N; lo += chunk) {
         if (lo > 0) {                    // fresh work counters for every chunk; step counters and status accumulate
@@ -540,7 +545,7 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
         }
         p.n = (int)(N - lo < chunk ? N - lo : chunk);
         p.f_base = lo;
-        CK(pn_launch_fused(p, o.grid_blocks, s));
+        CK(pn_launch_fused(p, o.grid_blocks, s, uni_slot, 0));
     }
     CK(cudaEventRecord(c.ev[2], s));
     if (d.pearson_r || d.moments) CK(pn_launch_stats_merge(f_mom, 1, (int)G, d.moments, d.pearson_r, s));

@@ -93,6 +93,34 @@ __device__ __forceinline__ void pn_make_record(const double (&y0)[10], double m1
     out[39] = (real)(p.atol * (s2 > 0.0 ? s2 : 1.0));
 }
 
+// The uniform-mass kernel's constants, in the form it evaluates the brace of Eq. (1) in: everything the
+// brace is linear in arrives multiplied by KB = K0/Bc (pn_rhs.cuh, FOLD), so omega_dot = (beta v^5) brace'
+//   [0..14] PnConsts (c2 ... c7, p1, p2, q1, q2 folded)   [15] c0'   [16] c3'   [17] cl'   [18..24] qc'   [25] KB
+__device__ __forceinline__ void pn_write_uni_row(double m1, double m2, const PnKernelParams& p, double* row)
+{
+    PnConsts<double> c;
+    PnUni<double> u;
+    pn_make_uni<double>(p.mask, u);
+    pn_make_consts<double>(m1, m2, p.mask, c);
+    const double KB = c.K0 / c.Bc;
+    row[0] = c.M; row[1] = KB * c.c2; row[2] = KB * c.c4; row[3] = KB * c.c5; row[4] = KB * c.c6; row[5] = KB * c.c7;
+    row[6] = KB * c.p1; row[7] = KB * c.p2; row[8] = KB * c.q1; row[9] = KB * c.q2; row[10] = c.K0; row[11] = c.A1;
+    row[12] = c.A2; row[13] = c.Bc; row[14] = c.G; row[15] = KB * u.c0; row[16] = KB * u.c3; row[17] = KB * u.cl;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) row[18 + k] = KB * p.qc[k];
+    row[25] = KB;
+}
+
+// fused mode, one fixed-mass ensemble: the row from the masses pn_gen.cuh gives every system of ensemble e (one thread)
+__global__ void pn_fused_row_kernel(const PnKernelParams p, int e)
+{
+    const GenSpec sp = ((const GenSpec*)p.f_specs)[e];
+    double m1, m2;
+    if (sp.m1_fixed > 0.0) { m1 = sp.m1_fixed; m2 = __dsub_rn(1.0, m1); }
+    else { const double d = __dadd_rn(1.0, sp.q_lo); m1 = __ddiv_rn(1.0, d); m2 = __ddiv_rn(sp.q_lo, d); }
+    pn_write_uni_row(m1, m2, p, p.uni_row);
+}
+
 template <typename real>
 __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
 {
@@ -140,23 +168,7 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     if (m1 != p.masses[0] || m2 != p.masses[p.n]) *p.nonuniform = 1;      // benign race: every writer stores 1
     real out[PN_REC];
     pn_make_record<real>(y0, m1, m2, p, out);
-    if (i == 0 && p.uni_slot >= 0) {
-        // the uniform-mass kernel's constants, in the form it evaluates the brace of Eq. (1) in: everything
-        // the brace is linear in arrives multiplied by KB = K0/Bc (pn_rhs.cuh, FOLD), so omega_dot = (beta v^5) brace'
-        //   [0..14] PnConsts (c2 ... c7, p1, p2, q1, q2 folded)   [15] c0'   [16] c3'   [17] cl'   [18..24] qc'   [25] KB
-        PnConsts<double> c;
-        PnUni<double> u;
-        pn_make_uni<double>(p.mask, u);
-        pn_make_consts<double>(m1, m2, p.mask, c);
-        const double KB = c.K0 / c.Bc;
-        double* row = p.uni_row;
-        row[0] = c.M; row[1] = KB * c.c2; row[2] = KB * c.c4; row[3] = KB * c.c5; row[4] = KB * c.c6; row[5] = KB * c.c7;
-        row[6] = KB * c.p1; row[7] = KB * c.p2; row[8] = KB * c.q1; row[9] = KB * c.q2; row[10] = c.K0; row[11] = c.A1;
-        row[12] = c.A2; row[13] = c.Bc; row[14] = c.G; row[15] = KB * u.c0; row[16] = KB * u.c3; row[17] = KB * u.cl;
-#pragma unroll
-        for (int k = 0; k < 7; ++k) row[18 + k] = KB * p.qc[k];
-        row[25] = KB;
-    }
+    if (i == 0 && p.uni_slot >= 0) pn_write_uni_row(m1, m2, p, p.uni_row);
     using vec = typename PnVec<real>::type;           // 16-byte stores
     vec* dst = (vec*)rec;
     constexpr int W = 16 / (int)sizeof(real);
@@ -790,11 +802,12 @@ static cudaError_t launch_adaptive(const PnKernelParams& p, int grid_blocks, cud
 // One chunk of a fused ensemble run: the fast kernel draws and integrates systems [p.f_base, p.f_base + p.n); the redo
 // pass re-draws and re-integrates those that left the range of the cbrt/log series (their chunk-local indices are in
 // p.redo_list).  p.queue, p.queue2, p.redo_count must be zero on entry.
-cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s)
+// fast fused kernel (UNI = -1: generic; >= 0: one fixed-mass ensemble, constants from row UNI of the table) + redo pass
+template <int UNI>
+static cudaError_t launch_fused_pair(PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
-    if (p.n <= 0) return cudaSuccess;
     constexpr int BLOCK = 128, MINB = 2;
-    auto fast = pn_integrate_adaptive_kernel<double, BLOCK, MINB, false, false, -1, true>;
+    auto fast = pn_integrate_adaptive_kernel<double, BLOCK, MINB, false, false, UNI, true>;
     auto redo = pn_integrate_adaptive_kernel<double, BLOCK, MINB, true, false, -1, true>;
     const int shm = (int)PnFusedSmem<BLOCK>::bytes();
     static int grid_full[64] = {0};
@@ -822,6 +835,27 @@ cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s)
     redo<<<grid, BLOCK, shm, s>>>(p);
     g_pn_launches += 2;
     return cudaGetLastError();
+}
+
+// uni_slot >= 0: every system of this launch belongs to ONE ensemble with fixed masses (ensemble uni_ens): its constants go
+// into row uni_slot of the uniform-mass table (one-thread kernel, then a device-to-device copy on the stream) and the fast
+// kernel is the uniform-mass instantiation; the redo pass stays generic
+cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s, int uni_slot, int uni_ens)
+{
+    if (p.n <= 0) return cudaSuccess;
+    if (uni_slot < 0) return launch_fused_pair<-1>(p, grid_blocks, s);
+    cudaError_t e;
+    pn_fused_row_kernel<<<1, 1, 0, s>>>(p, uni_ens);
+    ++g_pn_launches;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = cudaMemcpyToSymbolAsync(pn_uni_table, p.uni_row, PN_UNI_ROW * sizeof(double),
+                                     (size_t)uni_slot * PN_UNI_ROW * sizeof(double), cudaMemcpyDeviceToDevice, s)) != cudaSuccess)
+        return e;
+    static_assert(PN_UNI_SLOTS == 4, "one instantiation of the uniform-mass kernel per table row");
+    if (uni_slot == 0) return launch_fused_pair<0>(p, grid_blocks, s);
+    if (uni_slot == 1) return launch_fused_pair<1>(p, grid_blocks, s);
+    if (uni_slot == 2) return launch_fused_pair<2>(p, grid_blocks, s);
+    return launch_fused_pair<3>(p, grid_blocks, s);
 }
 
 cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,

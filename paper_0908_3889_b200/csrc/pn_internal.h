@@ -65,8 +65,9 @@ static inline void pn_host_series(unsigned mask, double (&qc)[7])
 // variant bits (pn_options.variant): 1 = always the generic FP64 kernel (per-lane constants), 2 = always the scalar FP32 kernel
 cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_threads, int grid_blocks,
                                 cudaStream_t s, int variant);
-// fused ensemble run (pn_integrate.cu): one chunk of systems [p.f_base, p.f_base + p.n); fast kernel + redo pass
-cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s);
+// fused ensemble run (pn_integrate.cu): one chunk of systems [p.f_base, p.f_base + p.n); fast kernel + redo pass;
+// uni_slot >= 0: all of them in the fixed-mass ensemble uni_ens -> the uniform-mass fast kernel with table row uni_slot
+cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s, int uni_slot, int uni_ens);
 // pair-packed FP32 integrator (pn_integrate_packed.cu); the seed records must be float ones written with rec_pairs = 1
 cudaError_t pn_launch_integrate_packed(const PnKernelParams& p, int grid_blocks, cudaStream_t s);
 // staging + histogram + peak (pn_aux.cu)

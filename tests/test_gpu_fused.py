@@ -92,6 +92,27 @@ def test_fused_equals_the_unfused_chain(pn):
         same(f2, c2, cnt)
 
 
+def test_fused_single_fixed_mass_ensemble_takes_the_uniform_mass_kernel(pn):
+    """ONE ensemble with fixed masses (every ensemble of the paper's section V) runs the uniform-mass instantiation of the
+    fused kernel (constants from the __constant__ table, brace constants folded).  The unfused chain
+    takes the uniform-mass kernel for such a batch too, so the two still agree exactly; against the generic fused kernel
+    (pn_options.variant bit 0) the arithmetic differs in rounding: same n, r to 1e-9, histogram counts off by a few
+    systems next to a bin edge at most."""
+    for spec in (SWEEP[0], SWEEP[2]):
+        n = 6000 + 13
+        st_c, c, kc = chain(pn, [spec], n, 0, n, 0.05, 1e-10, 1e-12, 50, 31)
+        st_f, f, kf = fused(pn, [spec], n, 0, n, 0.05, 1e-10, 1e-12, 50, 31)
+        st_g, g, kg = fused(pn, [spec], n, 0, n, 0.05, 1e-10, 1e-12, 50, 31, variant=1)
+        assert st_c == st_f == st_g == 0
+        same(f, c, n)
+        assert kf["trial_steps"] == kc["trial_steps"] and kf["rejected"] == kc["rejected"]
+        assert not np.array_equal(f["moments"], g["moments"])          # the uniform-mass kernel did run
+        assert np.array_equal(f["moments"][..., 0], g["moments"][..., 0]) and np.array_equal(f["n_skipped"], g["n_skipped"])
+        assert np.allclose(f["pearson_r"], g["pearson_r"], rtol=0, atol=1e-9, equal_nan=True)
+        assert np.abs(f["hist1"] - g["hist1"]).sum() <= 4 and np.abs(f["hist2"] - g["hist2"]).sum() <= 8
+        assert abs(kf["trial_steps"] / kg["trial_steps"] - 1) < 1e-3
+
+
 def test_fused_against_the_oracle_chain(pn, oracle):
     specs = SWEEP[:2]
     n = 700
