@@ -535,6 +535,14 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
     // ONE ensemble with fixed masses (every ensemble of the paper's section V; the 3.6e8-system uniformity run): the
     // uniform-mass fast kernel, constants from this stream context's row of the table.  Several ensembles
     // share chunks, so they take the generic kernel (a launch per ensemble would pay a drain tail per ensemble).
+    if (!o.input_order && N > 1024) {
+        // longest-expected-first queue order inside every chunk: keys + order, 8 bytes per system of a chunk
+        const size_t nc = (size_t)(N < chunk ? N : chunk);
+        if ((rc = c.keys.ensure(sizeof(float) * nc)) != PN_OK) return rc;
+        if ((rc = c.order.ensure(sizeof(int) * nc)) != PN_OK) return rc;
+        if ((rc = c.ord_scr.ensure(sizeof(unsigned) * (PN_ORDER_BUCKETS + 2))) != PN_OK) return rc;
+        p.keys = (float*)c.keys.p; p.order_out = (int*)c.order.p; p.order_scratch = (unsigned*)c.ord_scr.p;
+    }
     const bool fixed_masses = ens[0].m1_fixed > 0.0 || !(ens[0].q_hi > ens[0].q_lo);
     const int uni_slot = (G == 1 && fixed_masses && !(o.variant & 1)) ? c.slot : -1;
     CK(cudaEventRecord(c.ev[1], s));

@@ -111,6 +111,50 @@ __device__ __forceinline__ void pn_write_uni_row(double m1, double m2, const PnK
     row[25] = KB;
 }
 
+// Expected cost of a system: the number of precession cycles of the faster-precessing body,
+//   key = (4 + 3 m_big/m_small)/eta (1/(M omega_0) - 1/(M omega_f))      (Eq. (4) over Eq. (1) at leading order),
+// times a spin correction: the precession rate goes with |J| ~ |L| + (S1 + S2).L^, |L| = eta M^{5/3} omega^{-1/3}; integrated
+// over the inspiral (dt = d omega / omega_dot, omega_dot ~ omega^{11/3}) the spin part is
+// (3/2) S_par (omega_0^{-2/3} - omega_f^{-2/3}) / (eta M^{5/3}) next to 1/omega_0 - 1/omega_f.  Taken at half weight
+// (measured step counts follow it with a slope of 0.44 on C2) and clamped: the order only needs to be approximate.
+// The bucket sort that follows issues the queue longest-expected-first.  Positive floats order like their bit patterns, so
+// the range of the keys is found with integer atomics: one pair per warp.  Bad inputs get key 0 (last in the queue; the
+// refill skips them) and stay out of the range.  Called by whole warps (`in`: the thread has a system).
+__device__ __forceinline__ void pn_write_cost_key(const PnKernelParams& p, int i, bool in, bool bad_input, const double (&y0)[10],
+                                                  double m1, double m2)
+{
+    const double M = m1 + m2, eta = m1 * m2 / (M * M);
+    double key = (4.0 + 3.0 * fmax(m1, m2) / fmin(m1, m2)) / eta * (1.0 / (M * y0[0]) - 1.0 / (M * p.omegaf));
+    const double s_par = (y0[1] + y0[4]) * y0[7] + (y0[2] + y0[5]) * y0[8] + (y0[3] + y0[6]) * y0[9];
+    const double r0 = rcbrt(y0[0]), rf = rcbrt(p.omegaf);
+    const double rel = 1.5 * (r0 * r0 - rf * rf) / (eta * M * cbrt(M * M) * (1.0 / y0[0] - 1.0 / p.omegaf));
+    key *= fmax(1.0 + 0.5 * s_par * rel, 0.3);
+    const bool key_ok = !bad_input && key > 0.0 && key < 3e38;
+    const float kf = key_ok ? (float)key : 0.0f;
+    if (in) p.keys[i] = kf;
+    const unsigned kb = __float_as_uint(kf);
+    const unsigned lo = __reduce_min_sync(0xffffffffu, key_ok ? kb : 0xffffffffu);
+    const unsigned hi = __reduce_max_sync(0xffffffffu, key_ok ? kb : 0u);
+    if ((threadIdx.x & 31) == 0) {
+        if (lo != 0xffffffffu) atomicMin(p.order_scratch + PN_ORDER_BUCKETS, lo);
+        if (hi != 0u) atomicMax(p.order_scratch + PN_ORDER_BUCKETS + 1, hi);
+    }
+}
+
+// fused mode: the expected-cost keys of the chunk's systems, drawn exactly as the integrator will draw them (pn_gen.cuh)
+__global__ void __launch_bounds__(128) pn_fused_keys_kernel(const PnKernelParams p)
+{
+    const int i = blockIdx.x * 128 + threadIdx.x;
+    const bool in = i < p.n;
+    const long long gsys = p.f_base + (in ? i : p.n - 1);
+    const long long e = gsys / p.f_count;
+    const GenSpec sp = ((const GenSpec*)p.f_specs)[e];
+    double y0[10], m1, m2;
+    gen_system_at(sp, (unsigned long long)p.f_n_total, (unsigned long long)(p.f_first + (gsys - e * p.f_count)), y0, m1, m2);
+    const bool bad_input = !(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0);
+    pn_write_cost_key(p, i, in, bad_input, y0, m1, m2);
+}
+
 // fused mode, one fixed-mass ensemble: the row from the masses pn_gen.cuh gives every system of ensemble e (one thread)
 __global__ void pn_fused_row_kernel(const PnKernelParams p, int e)
 {
@@ -133,35 +177,7 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     const double m1 = p.masses[ii], m2 = p.masses[(size_t)p.n + ii];
     const bool bad_input = !(m1 > 0.0) || !(m2 > 0.0) || !(y0[0] < p.omegaf) || !(y0[0] > 0.0) ||
                            (p.omega0 > 0.0 && !(fabs(y0[0] - p.omega0) <= 1e-12 * p.omega0));
-    if (p.keys) {
-        // expected cost: the number of precession cycles of the faster-precessing body,
-        //   key = (4 + 3 m_big/m_small)/eta (1/(M omega_0) - 1/(M omega_f))      (Eq. (4) over Eq. (1) at leading order);
-        // the bucket sort that follows issues the queue longest-expected-first.  Positive floats order like their bit
-        // patterns, so the range of the keys is found with integer atomics: one pair per warp.  Bad inputs get key 0
-        // (last in the queue; the refill skips them) and stay out of the range.
-        const double M = m1 + m2, eta = m1 * m2 / (M * M);
-        double key = (4.0 + 3.0 * fmax(m1, m2) / fmin(m1, m2)) / eta * (1.0 / (M * y0[0]) - 1.0 / (M * p.omegaf));
-        // spin correction: the precession rate goes with |J| ~ |L| + (S1 + S2).L^, |L| = eta M^{5/3} omega^{-1/3}; integrated
-        // over the inspiral (dt = d omega / omega_dot, omega_dot ~ omega^{11/3}) the spin part is
-        // (3/2) S_par (omega_0^{-2/3} - omega_f^{-2/3}) / (eta M^{5/3}) next to 1/omega_0 - 1/omega_f.  Taken at half weight
-        // (measured step counts follow it with a slope of 0.44 on C2) and clamped: the order only needs to be approximate.
-        {
-            const double s_par = (y0[1] + y0[4]) * y0[7] + (y0[2] + y0[5]) * y0[8] + (y0[3] + y0[6]) * y0[9];
-            const double r0 = rcbrt(y0[0]), rf = rcbrt(p.omegaf);
-            const double rel = 1.5 * (r0 * r0 - rf * rf) / (eta * M * cbrt(M * M) * (1.0 / y0[0] - 1.0 / p.omegaf));
-            key *= fmax(1.0 + 0.5 * s_par * rel, 0.3);
-        }
-        const bool key_ok = !bad_input && key > 0.0 && key < 3e38;
-        const float kf = key_ok ? (float)key : 0.0f;
-        if (in) p.keys[i] = kf;
-        const unsigned kb = __float_as_uint(kf);
-        const unsigned lo = __reduce_min_sync(0xffffffffu, key_ok ? kb : 0xffffffffu);
-        const unsigned hi = __reduce_max_sync(0xffffffffu, key_ok ? kb : 0u);
-        if ((threadIdx.x & 31) == 0) {
-            if (lo != 0xffffffffu) atomicMin(p.order_scratch + PN_ORDER_BUCKETS, lo);
-            if (hi != 0u) atomicMax(p.order_scratch + PN_ORDER_BUCKETS + 1, hi);
-        }
-    }
+    if (p.keys) pn_write_cost_key(p, i, in, bad_input, y0, m1, m2);
     if (!in) return;
     real* rec = (real*)p.seed + (size_t)i * PN_REC;
     real y[10], k1[10];
@@ -408,7 +424,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_adaptive_kernel(cons
     if (UNI >= 0) { if (*p.nonuniform != 0) return; }
     else if (!SLOW && p.uni_slot >= 0) { if (*p.nonuniform == 0) return; }
     const unsigned n_queue = SLOW ? *p.redo_count : (unsigned)p.n;     // length of the work queue
-    const int* order = SLOW ? p.redo_list : (FUSED ? nullptr : p.order);      // fused: queue order is index order
+    const int* order = SLOW ? p.redo_list : p.order;      // null: index order
     if (SLOW && n_queue == 0u) return;
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -839,7 +855,7 @@ static cudaError_t launch_fused_pair(PnKernelParams& p, int grid_blocks, cudaStr
     const long long need = ((long long)p.n + BLOCK - 1) / BLOCK;
     if (need < grid) grid = (int)need;
     if (grid < 1) grid = 1;
-    p.uni_slot = -1; p.order = nullptr;
+    p.uni_slot = -1;
     p.f_resident = (unsigned)grid * BLOCK;
     fast<<<grid, BLOCK, shm, s>>>(p);
     redo<<<grid, BLOCK, shm, s>>>(p);
@@ -853,8 +869,18 @@ static cudaError_t launch_fused_pair(PnKernelParams& p, int grid_blocks, cudaStr
 cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s, int uni_slot, int uni_ens)
 {
     if (p.n <= 0) return cudaSuccess;
-    if (uni_slot < 0) return launch_fused_pair<-1>(p, grid_blocks, s);
     cudaError_t e;
+    p.order = nullptr;
+    if (p.keys) {
+        // queue order, longest expected first: 8 bytes of scratch per system of the chunk
+        if ((e = pn_launch_order_init(p.order_scratch, s)) != cudaSuccess) return e;
+        pn_fused_keys_kernel<<<(p.n + 127) / 128, 128, 0, s>>>(p);
+        ++g_pn_launches;
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        if ((e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s)) != cudaSuccess) return e;
+        p.order = p.order_out;
+    }
+    if (uni_slot < 0) return launch_fused_pair<-1>(p, grid_blocks, s);
     pn_fused_row_kernel<<<1, 1, 0, s>>>(p, uni_ens);
     ++g_pn_launches;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;

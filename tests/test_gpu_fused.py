@@ -85,6 +85,10 @@ def test_fused_equals_the_unfused_chain(pn):
     # counts are reproducible run to run; moments to rounding
     st_g, g, _ = fused(pn, SWEEP, n_total, first, count, 0.05, 1e-10, 1e-12, 50, 79)
     same(g, f, count)
+    # the queue is issued longest-expected-first inside every chunk (keys from a draw-only pass); the order changes nothing
+    st_h, h, kh = fused(pn, SWEEP, n_total, first, count, 0.05, 1e-10, 1e-12, 50, 79, input_order=True)
+    same(h, f, count)
+    assert kh["trial_steps"] == kf["trial_steps"]
     # without histograms, without moments, tiny ensembles (fewer systems than one draw), one system
     for cnt in (1, 31, 33):
         _, c2, _ = chain(pn, SWEEP[:2], 64, 5, cnt, 0.05, 1e-10, 1e-12, 0, 0)
