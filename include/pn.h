@@ -100,8 +100,8 @@ typedef struct pn_options {
     void* stream;          /* cudaStream_t, or NULL for the default stream */
     int block_threads;     /* tuning: threads per block of the integrator (0: default) */
     int grid_blocks;       /* tuning: blocks of the persistent grid (0: SMs x resident blocks) */
-    int variant;           /* tests / tuning: kernel selection bits, results are unchanged.  1: always the generic FP64
-                              kernel (per-lane constants) even for uniform-mass batches; 2: always the
+    int variant;           /* tests / tuning: kernel selection bits, results are unchanged (FP64 bit 0: to rounding).  1: always
+                              the generic kernel (per-lane constants) even for uniform-mass batches; 2: always the
                               scalar FP32 kernel instead of the packed two-systems-per-lane one */
 } pn_options;
 

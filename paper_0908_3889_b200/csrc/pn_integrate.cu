@@ -194,7 +194,14 @@ __global__ void __launch_bounds__(128) pn_seed_kernel(const PnKernelParams p)
     if (m1 != p.masses[0] || m2 != p.masses[p.n]) *p.nonuniform = 1;      // benign race: every writer stores 1
     real out[PN_REC];
     pn_make_record<real>(y0, m1, m2, p, out);
-    if (i == 0 && p.uni_slot >= 0) pn_write_uni_row(m1, m2, p, p.uni_row);
+    if (i == 0 && p.uni_slot >= 0) {
+        if (sizeof(real) == 8) pn_write_uni_row(m1, m2, p, p.uni_row);
+        else {                                   // FP32: the record's own constants, as floats (pn_integrate_packed.cu)
+            float* row = (float*)p.uni_row;
+#pragma unroll
+            for (int k = 0; k < 15; ++k) row[k] = (float)out[20 + k];
+        }
+    }
     using vec = typename PnVec<real>::type;           // 16-byte stores
     vec* dst = (vec*)rec;
     constexpr int W = 16 / (int)sizeof(real);
@@ -924,6 +931,7 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
         // queue order: longest expected first
         if (p.keys && (e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s)) != cudaSuccess) return e;
     }
+    const int ctx_slot = p.uni_slot;
     const int slot = (precision == 0 && block_threads != 256 && !(variant & 1)) ? p.uni_slot : -1;
     p.uni_slot = -1;                 // >= 0 only for the kernel pair below
     if (precision == 0) {
@@ -954,5 +962,5 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
     // asked for (pn_options.variant bit 1, or an explicit block shape); the results are bit-identical
     if (block_threads == 128) return launch_adaptive<float, 128, 4, false>(p, grid_blocks, s);
     if (block_threads == 256 || (variant & 2)) return launch_adaptive<float, 256, 2, false>(p, grid_blocks, s);
-    return pn_launch_integrate_packed(p, grid_blocks, s);         // its seed records were written with rec_pairs = 1 above
+    return pn_launch_integrate_packed(p, grid_blocks, s, (variant & 1) ? -1 : ctx_slot);     // its seed records were written with rec_pairs = 1 above
 }

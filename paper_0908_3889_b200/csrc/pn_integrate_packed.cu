@@ -35,9 +35,18 @@ __device__ __forceinline__ void pn_pairs_fill(const float (&rec)[PN_REC], f2 (&y
 
 #define PN_PK_CHUNKS (PN_REC / 4)       /* 16-byte chunks of a float record */
 
-template <int BLOCK, int MINB>
+// UNI >= 0: every system of the batch has the masses of system 0 (checked by the seed kernel, as for the FP64 kernels,
+// DESIGN.md 7.8): the 15 mass-dependent constants come from row UNI of this table -- uniform-register operands instead of
+// per-lane registers (126 -> 114 registers, ~50 three-register FFMAs per trial step become two-register ones).  The row
+// holds the very floats of system 0's seed record, so the results are bit-identical to the generic instantiation's.  The
+// launcher starts both instantiations; the one that does not apply returns at once.
+__constant__ float pn_uni_f[PN_UNI_SLOTS][32];
+
+template <int BLOCK, int MINB, int UNI = -1>
 __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_pairs_kernel(const PnKernelParams p)
 {
+    if (UNI >= 0) { if (*p.nonuniform != 0) return; }
+    else if (p.uni_slot >= 0) { if (*p.nonuniform == 0) return; }
     const unsigned n_queue = (unsigned)p.n;
     const int* order = p.order;
     const unsigned FULL = 0xffffffffu;
@@ -52,6 +61,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_pairs_kernel(const P
     pn_make_uni<float>(p.mask, u);
     u.emax = (float)p.emax;
     pn_make_consts<float>(0.5, 0.5, 0u, c);
+    if constexpr (UNI >= 0) {
+        const float* uc = pn_uni_f[UNI];
+        c.M = uc[0]; c.c2 = uc[1]; c.c4 = uc[2]; c.c5 = uc[3]; c.c6 = uc[4]; c.c7 = uc[5]; c.p1 = uc[6]; c.p2 = uc[7];
+        c.q1 = uc[8]; c.q2 = uc[9]; c.K0 = uc[10]; c.A1 = uc[11]; c.A2 = uc[12]; c.Bc = uc[13]; c.G = uc[14];
+    }
 #pragma unroll
     for (int j = 0; j < 5; ++j) { y[j] = f2(0.0f); k1[j] = f2(0.0f); }
     pn_pair_set<0>(y, 0.01f); pn_pair_set<9>(y, 1.0f);
@@ -120,7 +134,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_pairs_kernel(const P
                 // rec[38] < 0: bad input, already failed and stored by the seed kernel; the lane stays idle and takes the
                 // system after it once that one's record has arrived
                 if (!(rec[38] < 0.0f)) {
-                    pn_pairs_fill(rec, y, k1, c, atS1, atS2);
+                    if constexpr (UNI >= 0) { PnConsts<float> unused; pn_pairs_fill(rec, y, k1, unused, atS1, atS2); }
+                    else pn_pairs_fill(rec, y, k1, c, atS1, atS2);
                     h = p.h0 > 0.0 ? (float)p.h0 : 10.0f * c.M;      // first step (R13)
                     t = 0.0; steps = 0; nrej = 0; nland = 0; after_reject = false; landing = false;
                     idx = nxt;
@@ -238,10 +253,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) pn_integrate_pairs_kernel(const P
     }
 }
 
-cudaError_t pn_launch_integrate_packed(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
+template <int UNI>
+static cudaError_t launch_pairs(const PnKernelParams& p, int grid_blocks, cudaStream_t s)
 {
     constexpr int BLOCK = 256, MINB = 2;
-    auto kern = pn_integrate_pairs_kernel<BLOCK, MINB>;
+    auto kern = pn_integrate_pairs_kernel<BLOCK, MINB, UNI>;
     const int shm = 2 * PN_PK_CHUNKS * BLOCK * 16;      // record prefetch buffers: 80 KB per block
     static int grid_full[64] = {0};
     int dev = 0;
@@ -263,4 +279,25 @@ cudaError_t pn_launch_integrate_packed(const PnKernelParams& p, int grid_blocks,
     kern<<<grid, BLOCK, shm, s>>>(p);
     ++g_pn_launches;
     return cudaGetLastError();
+}
+
+// uni_slot >= 0: the seed kernel has put system 0's constants (floats) at the head of p.uni_row; they go into row uni_slot of
+// the table on the stream and both the uniform-mass and the generic instantiation are launched (decided on the device)
+cudaError_t pn_launch_integrate_packed(PnKernelParams& p, int grid_blocks, cudaStream_t s, int uni_slot)
+{
+    p.uni_slot = -1;
+    if (uni_slot < 0) return launch_pairs<-1>(p, grid_blocks, s);
+    cudaError_t e;
+    if ((e = cudaMemcpyToSymbolAsync(pn_uni_f, p.uni_row, 32 * sizeof(float), (size_t)uni_slot * 32 * sizeof(float),
+                                     cudaMemcpyDeviceToDevice, s)) != cudaSuccess)
+        return e;
+    p.uni_slot = uni_slot;
+    static_assert(PN_UNI_SLOTS == 4, "one instantiation of the uniform-mass kernel per table row");
+    if (uni_slot == 0) e = launch_pairs<0>(p, grid_blocks, s);
+    else if (uni_slot == 1) e = launch_pairs<1>(p, grid_blocks, s);
+    else if (uni_slot == 2) e = launch_pairs<2>(p, grid_blocks, s);
+    else e = launch_pairs<3>(p, grid_blocks, s);
+    if (e == cudaSuccess) e = launch_pairs<-1>(p, grid_blocks, s);
+    p.uni_slot = -1;
+    return e;
 }

@@ -69,7 +69,7 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
 // uni_slot >= 0: all of them in the fixed-mass ensemble uni_ens -> the uniform-mass fast kernel with table row uni_slot
 cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s, int uni_slot, int uni_ens);
 // pair-packed FP32 integrator (pn_integrate_packed.cu); the seed records must be float ones written with rec_pairs = 1
-cudaError_t pn_launch_integrate_packed(const PnKernelParams& p, int grid_blocks, cudaStream_t s);
+cudaError_t pn_launch_integrate_packed(PnKernelParams& p, int grid_blocks, cudaStream_t s, int uni_slot);
 // staging + histogram + peak (pn_aux.cu)
 cudaError_t pn_launch_aos_to_soa(const double* aos, double* soa, int n, int width, cudaStream_t s);
 cudaError_t pn_launch_soa_to_aos(const double* soa, double* aos, int n, int width, cudaStream_t s);

@@ -196,6 +196,16 @@ def test_packed_fp32_kernel_is_bit_identical_to_the_scalar_one(pn):
         b = gpu_integrate(pn, y0, m, cfg, precision=1, variant=2, input_order=io)
         for k in ("final", "steps", "time", "rejected"):
             assert np.array_equal(a[k], b[k]), (io, k)
+    # C4f is a uniform-mass batch: the default run above took the uniform-mass instantiation (constants from the
+    # __constant__ table: the very floats of system 0's record); the generic one (variant bit 0) gives the same bits, and
+    # one deviating system sends the whole launch to the generic instantiation
+    c = gpu_integrate(pn, y0, m, cfg, precision=1, variant=1)
+    m2 = m.copy(); m2[-1] = [0.5, 0.5]
+    d = gpu_integrate(pn, y0, m2, cfg, precision=1)
+    for k in ("final", "steps", "time", "rejected"):
+        assert np.array_equal(a[k], c[k]), k
+        assert np.array_equal(a[k][:-1], d[k][:-1]), k
+    assert not np.array_equal(a["final"][-1], d["final"][-1])
     # failures and bad inputs land in the same slots with the same codes
     cfg = W.with_size(W.CONFIGS["C3"], 777)
     y0, m = W.generate(cfg)
