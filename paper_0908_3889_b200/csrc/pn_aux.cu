@@ -160,20 +160,26 @@ __device__ __forceinline__ int pn_order_bucket(float key, float kmax, float scal
     const int b = (int)((kmax - key) * scale);
     return max(0, min(PN_ORDER_BUCKETS - 1, b));
 }
-__device__ __forceinline__ void pn_order_range(const unsigned* scratch, float& kmax, float& scale)
+// flat: a batch with many systems per lane (n >= n_flat) whose keys span less than a factor 2 (equal masses: only the spin
+// term differs) stays in input order: its
+// drain tail is < 0.5 % of the run either way, and neighbouring systems finishing close in time keep the SoA result
+// stores and the record reads sector-efficient (C4f: 8.71 -> 8.46 ms, DRAM traffic 3.9 -> 1.2 GB)
+__device__ __forceinline__ void pn_order_range(const unsigned* scratch, int n, int n_flat, float& kmax, float& scale)
 {
     const unsigned lo = scratch[PN_ORDER_BUCKETS], hi = scratch[PN_ORDER_BUCKETS + 1];
     const float kmin = lo == 0xffffffffu ? 0.0f : __uint_as_float(lo);
     kmax = __uint_as_float(hi);
     scale = kmax > kmin ? (float)(PN_ORDER_BUCKETS - 1) / (kmax - kmin) : 0.0f;     // all keys equal: one bucket
+    if (n_flat > 0 && n >= n_flat && kmax < 2.0f * kmin) scale = -1.0f;      // flat: the callers write the identity order
 }
 
-__global__ void __launch_bounds__(PN_ORD_THREADS) pn_order_count_kernel(const float* __restrict__ keys, int n, unsigned* __restrict__ scratch)
+__global__ void __launch_bounds__(PN_ORD_THREADS) pn_order_count_kernel(const float* __restrict__ keys, int n, int n_flat, unsigned* __restrict__ scratch)
 {
     __shared__ unsigned cnt[PN_ORDER_BUCKETS];
     for (int b = threadIdx.x; b < PN_ORDER_BUCKETS; b += PN_ORD_THREADS) cnt[b] = 0u;
     float kmax, scale;
-    pn_order_range(scratch, kmax, scale);
+    pn_order_range(scratch, n, n_flat, kmax, scale);
+    if (scale < 0.0f) return;                    // flat (uniform decision): nothing to count
     __syncthreads();
     const int base = blockIdx.x * (PN_ORD_THREADS * PN_ORD_ITEMS);
 #pragma unroll
@@ -211,15 +217,23 @@ __global__ void __launch_bounds__(1024) pn_order_scan_kernel(unsigned* __restric
     for (int k = 0; k < PER; ++k) { scratch[threadIdx.x * PER + k] = start; start += v[k]; }
 }
 
-__global__ void __launch_bounds__(PN_ORD_THREADS) pn_order_scatter_kernel(const float* __restrict__ keys, int n, unsigned* __restrict__ scratch,
+__global__ void __launch_bounds__(PN_ORD_THREADS) pn_order_scatter_kernel(const float* __restrict__ keys, int n, int n_flat, unsigned* __restrict__ scratch,
                                                                           int* __restrict__ order)
 {
     __shared__ unsigned cnt[PN_ORDER_BUCKETS];       // systems of this block per bucket, then the block's first position in it
     for (int b = threadIdx.x; b < PN_ORDER_BUCKETS; b += PN_ORD_THREADS) cnt[b] = 0u;
     float kmax, scale;
-    pn_order_range(scratch, kmax, scale);
-    __syncthreads();
+    pn_order_range(scratch, n, n_flat, kmax, scale);
     const int base = blockIdx.x * (PN_ORD_THREADS * PN_ORD_ITEMS);
+    if (scale < 0.0f) {                          // flat: input order
+#pragma unroll
+        for (int k = 0; k < PN_ORD_ITEMS; ++k) {
+            const int i = base + k * PN_ORD_THREADS + threadIdx.x;
+            if (i < n) order[i] = i;
+        }
+        return;
+    }
+    __syncthreads();
     int bucket[PN_ORD_ITEMS];
     unsigned rank[PN_ORD_ITEMS];
 #pragma unroll
@@ -252,13 +266,13 @@ cudaError_t pn_launch_order_init(unsigned int* scratch, cudaStream_t s)
     return cudaMemsetAsync(scratch + PN_ORDER_BUCKETS, 0xff, sizeof(unsigned), s);      // running minimum starts at 0xffffffff
 }
 
-cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch, int* order, cudaStream_t s)
+cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch, int* order, cudaStream_t s, int n_flat)
 {
     if (n <= 0) return cudaSuccess;
     const int per = PN_ORD_THREADS * PN_ORD_ITEMS, grid = (n + per - 1) / per;
-    pn_order_count_kernel<<<grid, PN_ORD_THREADS, 0, s>>>(keys, n, scratch);
+    pn_order_count_kernel<<<grid, PN_ORD_THREADS, 0, s>>>(keys, n, n_flat, scratch);
     pn_order_scan_kernel<<<1, 1024, 0, s>>>(scratch);
-    pn_order_scatter_kernel<<<grid, PN_ORD_THREADS, 0, s>>>(keys, n, scratch, order);
+    pn_order_scatter_kernel<<<grid, PN_ORD_THREADS, 0, s>>>(keys, n, n_flat, scratch, order);
     g_pn_launches += 3;
     return cudaGetLastError();
 }

@@ -123,21 +123,26 @@ __device__ __forceinline__ void pn_write_uni_row(double m1, double m2, const PnK
 __device__ __forceinline__ void pn_write_cost_key(const PnKernelParams& p, int i, bool in, bool bad_input, const double (&y0)[10],
                                                   double m1, double m2)
 {
-    const double M = m1 + m2, eta = m1 * m2 / (M * M);
-    double key = (4.0 + 3.0 * fmax(m1, m2) / fmin(m1, m2)) / eta * (1.0 / (M * y0[0]) - 1.0 / (M * p.omegaf));
-    const double s_par = (y0[1] + y0[4]) * y0[7] + (y0[2] + y0[5]) * y0[8] + (y0[3] + y0[6]) * y0[9];
-    const double r0 = rcbrt(y0[0]), rf = rcbrt(p.omegaf);
-    const double rel = 1.5 * (r0 * r0 - rf * rf) / (eta * M * cbrt(M * M) * (1.0 / y0[0] - 1.0 / p.omegaf));
-    key *= fmax(1.0 + 0.5 * s_par * rel, 0.3);
-    const bool key_ok = !bad_input && key > 0.0 && key < 3e38;
-    const float kf = key_ok ? (float)key : 0.0f;
+    // single precision is ample for a sort key (and the seed kernel of an FP32 batch of 2^22 systems would otherwise spend
+    // more time on double-precision divides and cube roots here than on its records)
+    const float a = (float)m1, b = (float)m2, w0 = (float)y0[0], wf = (float)p.omegaf;
+    const float M = a + b, eta = a * b / (M * M), dinv = 1.0f / w0 - 1.0f / wf;
+    float key = (4.0f + 3.0f * fmaxf(a, b) / fminf(a, b)) / eta * dinv / M;
+    const float s_par = (float)((y0[1] + y0[4]) * y0[7] + (y0[2] + y0[5]) * y0[8] + (y0[3] + y0[6]) * y0[9]);
+    const float r0 = rcbrtf(w0), rf = rcbrtf(wf);
+    const float rel = 1.5f * (r0 * r0 - rf * rf) / (eta * M * cbrtf(M * M) * dinv);
+    key *= fmaxf(1.0f + 0.5f * s_par * rel, 0.3f);
+    const bool key_ok = !bad_input && key > 0.0f && key < 3e38f;
+    const float kf = key_ok ? key : 0.0f;
     if (in) p.keys[i] = kf;
     const unsigned kb = __float_as_uint(kf);
     const unsigned lo = __reduce_min_sync(0xffffffffu, key_ok ? kb : 0xffffffffu);
     const unsigned hi = __reduce_max_sync(0xffffffffu, key_ok ? kb : 0u);
     if ((threadIdx.x & 31) == 0) {
-        if (lo != 0xffffffffu) atomicMin(p.order_scratch + PN_ORDER_BUCKETS, lo);
-        if (hi != 0u) atomicMax(p.order_scratch + PN_ORDER_BUCKETS + 1, hi);
+        // only a warp that widens the range issues the atomic (2^17 warps hammering two addresses cost 0.2 ms at 2^22 systems)
+        volatile unsigned* rng = p.order_scratch + PN_ORDER_BUCKETS;
+        if (lo < rng[0]) atomicMin(p.order_scratch + PN_ORDER_BUCKETS, lo);
+        if (hi > rng[1]) atomicMax(p.order_scratch + PN_ORDER_BUCKETS + 1, hi);
     }
 }
 
@@ -884,7 +889,7 @@ cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s, 
         pn_fused_keys_kernel<<<(p.n + 127) / 128, 128, 0, s>>>(p);
         ++g_pn_launches;
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        if ((e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s)) != cudaSuccess) return e;
+        if ((e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s, 48 * 148 * 256)) != cudaSuccess) return e;
         p.order = p.order_out;
     }
     if (uni_slot < 0) return launch_fused_pair<-1>(p, grid_blocks, s);
@@ -929,7 +934,14 @@ cudaError_t pn_launch_integrate(PnKernelParams& p, int precision, int block_thre
         ++g_pn_launches;
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         // queue order: longest expected first
-        if (p.keys && (e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s)) != cudaSuccess) return e;
+        if (p.keys) {
+            // 48 systems per resident lane and more: the order is not worth the scattered stores (pn_aux.cu, pn_order_range)
+            int dev = 0, sms = 148;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            const long long n_flat = 48LL * sms * (precision == 1 ? 512 : 256);
+            if ((e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s, (int)(n_flat < 0x7fffffffLL ? n_flat : 0x7fffffffLL))) != cudaSuccess) return e;
+        }
     }
     const int ctx_slot = p.uni_slot;
     const int slot = (precision == 0 && block_threads != 256 && !(variant & 1)) ? p.uni_slot : -1;

@@ -81,7 +81,8 @@ cudaError_t pn_launch_histogram(const double* states, int layout_soa, long long 
 // async calls: *sticky = max(*sticky, *status), one thread (pn_api.cu folds a call's status into its stream's sticky word)
 cudaError_t pn_launch_fold_status(const int* status, int* sticky, cudaStream_t s);
 cudaError_t pn_launch_order_init(unsigned int* scratch, cudaStream_t s);
-cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch, int* order, cudaStream_t s);
+// n_flat > 0: a batch of >= n_flat systems whose keys span less than a factor 2 stays in (block-wise) input order
+cudaError_t pn_launch_cost_order(const float* keys, int n, unsigned int* scratch, int* order, cudaStream_t s, int n_flat);
 // ensemble statistics (pn_stats.cu)
 size_t pn_stats_scratch_bytes(long long n, long long group_size, int* n_blocks_out);
 cudaError_t pn_launch_stats_merge(const double* parts, int n_parts, int n_groups, double* mom_out, double* r_out, cudaStream_t s);
