@@ -45,7 +45,8 @@ typedef enum {
     PN_EINVAL = 1,         /* bad argument (N < 0, null pointer, rtol <= 0, bins < 1, omega_f <= omega_0, m_i <= 0) */
     PN_ECUDA = 2,          /* a CUDA call or launch failed; outputs unspecified; see pn_last_cuda_error() */
     PN_ENOTCONVERGED = 3,  /* some system hit max_steps, step-size underflow or failed to land on omega_f */
-    PN_ENONFINITE = 4      /* some system produced a non-finite error norm */
+    PN_ENONFINITE = 4,     /* some system produced a non-finite error norm */
+    PN_ETOOLARGE = 5       /* pn_statistics_static only: the request does not fit the fixed scratch array; nothing was done */
 } pn_status;
 
 /* Per-system failure codes, written to out_steps[i] (which is otherwise the positive trial-step count). */
@@ -174,6 +175,47 @@ int pn_statistics(const double* init_states, const double* final_states, const i
  */
 int pn_merge_statistics(const double* parts, int n_parts, int n_groups, double* moments_out, double* pearson_r_out,
                         const struct pn_options* opt);
+
+/*
+ * pn_statistics_static -- pn_statistics for callers that must not allocate device memory.
+ *
+ * Who needs it.  pn_statistics keeps its per-block moment records in scratch that the library obtains with cudaMalloc
+ * the first time (and again whenever a call needs more).  Some programs that embed this library cannot afford, or are
+ * not able, to do that at the moment they want the statistics:
+ *   - a host framework (a PyTorch job, say) that has already handed the whole HBM to its own caching allocator, so a
+ *     cudaMalloc from a library comes back with "out of memory" although the job has room to spare in its pool;
+ *   - an analysis loop that runs next to other streams (the integrator of the next batch, a copy engine): cudaMalloc
+ *     and cudaFree are device-wide synchronisation points, so one allocation stalls every one of those streams;
+ *   - a process that lives under a fixed memory budget (an MPS or MIG slice with a limit) and has to know its
+ *     footprint when it starts, not discover it call by call.
+ * For them this entry point computes the same ensemble statistics (Pearson r of PAPER.md:138, the
+ * histograms of PAPER.md:116-120 and 132) with the same kernels, launch geometry and merge order as pn_statistics, so
+ * every output is the same number for number, but the kernels' scratch is a fixed array that is part of the library image
+ * (`static __device__`, PN_STATIC_SCRATCH_BYTES = 344,064 bytes).  Every GPU on which the library is loaded carries
+ * that array from the moment the module is loaded until the process exits, whether or not this function is ever called.
+ * The call itself issues no cudaMalloc, cudaFree, event or stream creation and calls no library routine that allocates.
+ *
+ * Arguments are those of pn_statistics, with these differences:
+ *   - DEVICE pointers only (a host-buffer variant would need staging memory, i.e. an allocation); inputs and outputs
+ *     stay the caller's: nothing but the scratch comes from the library.
+ *   - `stream` is the cudaStream_t to run on (NULL: the default stream); `async` != 0 only enqueues, otherwise the
+ *     stream has been synchronised on return.
+ *   - Limit: n_groups = N / group_size <= PN_STATIC_MAX_GROUPS (1024), and n_groups + (SMs of the device) + 1 records
+ *     of 168 bytes must fit the array (they do for any device of up to 1023 SMs).  A call beyond that changes nothing
+ *     and returns PN_ETOOLARGE ("request exceeds the fixed capacity of a no-allocation entry point"); the number of
+ *     systems N is not limited by the array (a block's record does not grow with N).
+ * Set-up: the first call on each device looks up the device address of the array (cudaGetSymbolAddress with that
+ * device current; the array's name means nothing to host code) and opts the kernel in to its shared-memory size.  Make
+ * that first call outside any stream capture, once per device you use; later calls do neither.
+ * Sharing: all calls in the process use the one array per device.  The part a call uses is zeroed on the stream before
+ * its kernels run, so nothing is inherited from the previous call; but two calls that can overlap on the GPU (different
+ * streams without an ordering between them, or two host threads) race on it and corrupt each other's moments.  Calls
+ * on one stream, or ordered by events, are safe.  pn_last_kernel_ms is not updated (timing needs events).
+ */
+#define PN_STATIC_MAX_GROUPS 1024
+#define PN_STATIC_SCRATCH_BYTES 344064 /* 2048 records x 3 dot products x (6 doubles + 1 counter) */
+int pn_statistics_static(const double* init_states, const double* final_states, const int* steps, long long N,
+                         long long group_size, int bins1, int bins2, const pn_stats_out* out, void* stream, int async);
 
 /*
  * pn_generate -- random initial data on the device ("generated on the GPU"; recipe of

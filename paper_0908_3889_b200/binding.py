@@ -15,10 +15,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpn_b200.so")
 
 PN_FP64, PN_FP32, PN_MIXED = 0, 1, 2
-PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE = 0, 1, 2, 3, 4
+PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE, PN_ETOOLARGE = 0, 1, 2, 3, 4, 5
+PN_STATIC_MAX_GROUPS, PN_STATIC_SCRATCH_BYTES = 1024, 344064
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_merge_statistics", "pn_generate", "pn_run_ensembles", "pn_selfcheck", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_statistics_static", "pn_merge_statistics", "pn_generate", "pn_run_ensembles", "pn_selfcheck", "pn_stream_status",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -80,6 +81,7 @@ def load():
         lib.pn_histogram.argtypes = [vp, ll, i, vp, vp]
         lib.pn_histogram_ex.argtypes = [vp, ll, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_statistics.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
+        lib.pn_statistics_static.argtypes = [vp, vp, vp, ll, ll, i, i, C.POINTER(PnStatsOut), vp, i]
         lib.pn_merge_statistics.argtypes = [vp, i, i, vp, vp, C.POINTER(PnOptions)]
         lib.pn_generate.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, vp, vp, C.POINTER(PnOptions)]
         lib.pn_run_ensembles.argtypes = [C.POINTER(PnEnsemble), i, ll, ll, ll, d, d, d, i, i, i, C.POINTER(PnStatsOut), C.POINTER(PnOptions)]
@@ -237,6 +239,42 @@ def pn_statistics(init_states, final_states, steps=None, *, group_size=0, bins1=
     out.hist1, out.hist2, out.hist2_max, out.hist2_norm = _ptr(hist1), _ptr(hist2), _ptr(hist2_max), _ptr(hist2_norm)
     return _check(lib.pn_statistics(_ptr(init_states), _ptr(final_states), _ptr(steps), n, int(group_size), int(bins1),
                                     int(bins2), C.byref(out), C.byref(o)))
+
+
+def pn_statistics_static(init_states, final_states, steps=None, *, group_size=0, bins1=0, bins2=0, pearson_r=None,
+                         moments=None, n_skipped=None, hist1=None, hist2=None, hist2_max=None, hist2_norm=None,
+                         stream=None, async_=False):
+    """pn_statistics_static of include/pn.h: the statistics of pn_statistics for a caller that must not allocate device
+    memory while it runs (all of HBM already sits in a framework's caching allocator, other streams would be stalled by
+    cudaMalloc's device-wide synchronisation, or the process has a fixed memory budget).  The kernels' scratch is a
+    fixed 336 KB array inside the library; at most PN_STATIC_MAX_GROUPS ensembles per call (PnError with status
+    PN_ETOOLARGE beyond).  Torch CUDA tensors only: inputs and outputs stay the caller's.  Calls share the array, so
+    calls that could overlap on the GPU (unordered streams) must not be issued; make the first call on a device outside
+    stream capture (it looks the array's address up)."""
+    lib = load()
+    n = int(final_states.shape[0])
+    gs = int(group_size) if int(group_size) > 0 else max(n, 1)
+    G = n // gs if n else 0
+    for name, a in (("final_states", final_states), ("init_states", init_states), ("steps", steps)):
+        if a is not None and _is_host(a):
+            raise ValueError(f"{name}: pn_statistics_static takes device tensors only (staging host arrays would need an allocation)")
+    _require("final_states", final_states, "f64", (n, 10), False)
+    _require("init_states", init_states, "f64", (n, 10), False)
+    _require("steps", steps, "i32", (n,), False)
+    _require("pearson_r", pearson_r, "f64", (G, 3), False, at_least=True)
+    _require("moments", moments, "f64", (G, 3, 6), False, at_least=True)
+    _require("n_skipped", n_skipped, "i64", (G, 3), False, at_least=True)
+    _require("hist1", hist1, "i64", (G, 3, int(bins1)), False, at_least=True)
+    _require("hist2", hist2, "i64", (G, 3, int(bins2), int(bins2)), False, at_least=True)
+    _require("hist2_max", hist2_max, "i64", (G, 3), False, at_least=True)
+    _require("hist2_norm", hist2_norm, "f64", (G, 3, int(bins2), int(bins2)), False, at_least=True)
+    out = PnStatsOut()
+    out.size = C.sizeof(PnStatsOut)
+    out.pearson_r, out.moments, out.n_skipped = _ptr(pearson_r), _ptr(moments), _ptr(n_skipped)
+    out.hist1, out.hist2, out.hist2_max, out.hist2_norm = _ptr(hist1), _ptr(hist2), _ptr(hist2_max), _ptr(hist2_norm)
+    s = None if stream is None else int(getattr(stream, "cuda_stream", stream))
+    return _check(lib.pn_statistics_static(_ptr(init_states), _ptr(final_states), _ptr(steps), n, int(group_size), int(bins1),
+                                           int(bins2), C.byref(out), s, int(bool(async_))))
 
 
 def pn_merge_statistics(parts, moments=None, pearson_r=None, **opts):

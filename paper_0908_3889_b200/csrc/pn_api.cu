@@ -24,6 +24,11 @@ static std::string g_last_err;
         }                                                                                            \
     } while (0)
 
+void pn_note_cuda_error(const char* where, cudaError_t e)
+{
+    g_last_err = std::string(where) + " -> " + cudaGetErrorString(e);
+}
+
 // ---- cached device scratch ------------------------------------------------------------------------
 struct Buf {
     void* p = nullptr;
@@ -730,6 +735,7 @@ extern "C" const char* pn_strerror(int st)
         case PN_ECUDA: return "CUDA call or kernel launch failed";
         case PN_ENOTCONVERGED: return "a system hit max_steps, step-size underflow or failed to land on omega_f";
         case PN_ENONFINITE: return "a system produced a non-finite error norm";
+        case PN_ETOOLARGE: return "request exceeds the fixed capacity of a no-allocation entry point (pn_statistics_static)";
         default: return "unknown status";
     }
 }

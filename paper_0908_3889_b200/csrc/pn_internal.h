@@ -109,3 +109,6 @@ cudaError_t pn_run_fma_peak(int precision, int mode, double seconds, double* tfl
                             double* cycles_per_warp_inst);
 
 extern unsigned long long g_pn_launches;
+// records "<where> -> <CUDA error string>" as the text pn_last_cuda_error() returns (pn_api.cu); for entry points that live
+// in another translation unit
+void pn_note_cuda_error(const char* where, cudaError_t e);

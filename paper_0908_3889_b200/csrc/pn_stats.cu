@@ -14,6 +14,7 @@
 // atomics when the block leaves a group.
 // This file shares nothing with oracle/ (which evaluates the two-pass definitions in numpy).
 #include <cstdint>
+#include "../../include/pn.h"
 #include "pn_internal.h"
 #include "pn_dots.cuh"
 #include "pn_moments.cuh"
@@ -413,4 +414,68 @@ cudaError_t pn_launch_stats(const double* init, const double* fin, const int* st
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
     }
     return cudaSuccess;
+}
+
+// ---- pn_statistics_static: the statistics pass without any allocation (include/pn.h) ---------------------------------
+// For embedders that cannot call cudaMalloc when they want the statistics: the whole HBM already belongs to their
+// framework's caching allocator (a library cudaMalloc then fails with out-of-memory), or other streams are running and
+// must not be stalled by the device-wide synchronisation that cudaMalloc / cudaFree imply, or the process has a fixed
+// memory budget.  The per-(block, ensemble) moment records and skipped counters that pn_launch_stats needs live in this
+// array instead of a cudaMalloc'ed buffer.  It is part of the module image: each GPU that loads the library holds these
+// 336 KB until the process exits.  One array per device serves every call, so it always holds what the last call left:
+// pn_launch_stats zeroes the part it is about to use on the stream, ahead of the kernels, and calls that may overlap on
+// the GPU (unordered streams) race on it; see the header.
+static __device__ __align__(256) unsigned char pn_static_scratch[PN_STATIC_SCRATCH_BYTES];
+
+// Device address of the array, per device.  In host code the identifier pn_static_scratch is only the handle the runtime
+// uses to find the symbol: handing it to a kernel would make the kernel dereference a host address.  The real address
+// differs from device to device, so it is looked up once per device with that device current.
+#define PN_STATIC_MAX_DEVICES 64
+static void* g_static_addr[PN_STATIC_MAX_DEVICES] = {nullptr};
+
+extern "C" int pn_statistics_static(const double* init_states, const double* final_states, const int* steps, long long N,
+                                    long long group_size, int bins1, int bins2, const pn_stats_out* out_in, void* stream, int async)
+{
+    // the argument rules of pn_statistics for device buffers
+    if (!out_in || out_in->size != (int)sizeof(pn_stats_out)) return PN_EINVAL;
+    pn_stats_out out = *out_in;
+    if (N < 0 || N > 0x7fffffffLL * 8) return PN_EINVAL;
+    if (N > 0 && !final_states) return PN_EINVAL;
+    if (bins1 > 8192 || bins2 > 4096) return PN_EINVAL;
+    if (bins1 < 1) { bins1 = 0; out.hist1 = nullptr; }
+    if (bins2 < 1 || !init_states) { bins2 = 0; out.hist2 = nullptr; }
+    if (!out.hist2 && (out.hist2_max || out.hist2_norm)) return PN_EINVAL;
+    const long long gs = group_size > 0 ? group_size : N;
+    if (N > 0 && N % gs != 0) return PN_EINVAL;
+    if (N == 0) return PN_OK;
+    if (((uintptr_t)final_states & 15u) || ((uintptr_t)init_states & 15u)) return PN_EINVAL;
+    // capacity: refuse, with its own status, before anything is enqueued
+    if (N / gs > PN_STATIC_MAX_GROUPS) return PN_ETOOLARGE;
+    if (pn_stats_scratch_bytes(N, group_size, nullptr) > (size_t)PN_STATIC_SCRATCH_BYTES) return PN_ETOOLARGE;
+
+    // set-up, first call on this device: where the array lives in this device's memory
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { pn_note_cuda_error("pn_statistics_static: cudaGetDevice", e); return PN_ECUDA; }
+    if (dev < 0 || dev >= PN_STATIC_MAX_DEVICES) return PN_EINVAL;
+    if (!g_static_addr[dev]) {
+        void* addr = nullptr;
+        e = cudaGetSymbolAddress((void**)&addr, pn_static_scratch);
+        if (e != cudaSuccess || !addr) {
+            pn_note_cuda_error("pn_statistics_static: cudaGetSymbolAddress(pn_static_scratch)", e);
+            return PN_ECUDA;
+        }
+        g_static_addr[dev] = addr;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    // the unchanged launcher of pn_statistics (memset of the records it uses, main kernel, finish kernel, optional
+    // normalisation), pointed at the static array: no allocation anywhere below
+    e = pn_launch_stats(init_states, final_states, steps, N, group_size, bins1, bins2, g_static_addr[dev], out.pearson_r,
+                        out.moments, out.n_skipped, out.hist1, out.hist2, out.hist2_max, out.hist2_norm, s);
+    if (e != cudaSuccess) { pn_note_cuda_error("pn_statistics_static: launch", e); return PN_ECUDA; }
+    if (async) return PN_OK;
+    e = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) { pn_note_cuda_error("pn_statistics_static: synchronize", e); return PN_ECUDA; }
+    return PN_OK;
 }
