@@ -263,8 +263,8 @@ int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long
  *               hist2 [G][3][bins2][bins2], hist2_max, hist2_norm; any member may be NULL.  DEVICE pointers (host with
  *               opt->host_buffers).  bins1 <= 2^24, bins2 <= 4096.
  *   opt         h0, max_steps, term_mask, tau_land, input_order, host_buffers, async, stream, grid_blocks, variant bit 0 are honoured.
- *               A call with ONE ensemble of fixed masses runs the uniform-mass kernel (as pn_integrate does for such a
- *               batch); several ensembles share launches and run the generic one.
+ *               A call whose ensembles ALL have the same fixed masses (one ensemble, or an equal-mass sweep over chi) runs
+ *               the uniform-mass kernel, exactly when pn_integrate would for the concatenated batch; otherwise the generic one.
  * Results equal the chain pn_generate -> pn_integrate -> pn_statistics on the same arguments: n, n_skipped and every
  * histogram count exactly (and reproducibly); means, M2x, M2y, Cxy and r to rounding (the order in which partial moments
  * are merged depends on timing: r agrees to ~1e-13, not bit for bit).  The queue of every chunk of 2^22 systems is issued

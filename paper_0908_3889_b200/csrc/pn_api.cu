@@ -537,9 +537,10 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
     p.f_specs = c.gen_specs.p; p.f_n_total = n_total; p.f_first = first; p.f_count = count;
     p.f_mom = f_mom; p.f_lock = f_lock; p.f_skipped = f_skip; p.f_hist1 = d.hist1; p.f_hist2 = d.hist2;
     p.f_bins1 = bins1; p.f_bins2 = bins2;
-    // ONE ensemble with fixed masses (every ensemble of the paper's section V; the 3.6e8-system uniformity run): the
-    // uniform-mass fast kernel, constants from this stream context's row of the table.  Several ensembles
-    // share chunks, so they take the generic kernel (a launch per ensemble would pay a drain tail per ensemble).
+    // Ensembles that all have the SAME fixed masses (every ensemble of an equal-mass sweep over chi of the paper's section V;
+    // the 3.6e8-system uniformity run): the uniform-mass fast kernel, constants from this stream context's row of the table
+    // (DESIGN.md 7.8).  Ensembles with different masses share chunks, so they take the generic kernel (a launch per ensemble
+    // would pay a drain tail per ensemble).
     if (!o.input_order && N > 1024) {
         // longest-expected-first queue order inside every chunk: keys + order, 8 bytes per system of a chunk
         const size_t nc = (size_t)(N < chunk ? N : chunk);
@@ -548,8 +549,21 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
         if ((rc = c.ord_scr.ensure(sizeof(unsigned) * (PN_ORDER_BUCKETS + 2))) != PN_OK) return rc;
         p.keys = (float*)c.keys.p; p.order_out = (int*)c.order.p; p.order_scratch = (unsigned*)c.ord_scr.p;
     }
-    const bool fixed_masses = ens[0].m1_fixed > 0.0 || !(ens[0].q_hi > ens[0].q_lo);
-    const int uni_slot = (G == 1 && fixed_masses && !(o.variant & 1)) ? c.slot : -1;
+    // The same decision the unfused chain takes over the concatenated batch (pn_seed_kernel compares every system's masses
+    // with system 0's): uniform iff EVERY ensemble of the call has fixed masses and they are the same pair of doubles.  The
+    // masses are formed here exactly as pn_fused_row_kernel / the generator form them (one rounded operation each).
+    auto fixed_pair = [](const pn_ensemble& x, double& m1, double& m2) {
+        if (x.m1_fixed > 0.0) { m1 = x.m1_fixed; m2 = 1.0 - m1; return true; }
+        if (!(x.q_hi > x.q_lo)) { const double dq = 1.0 + x.q_lo; m1 = 1.0 / dq; m2 = x.q_lo / dq; return true; }
+        return false;
+    };
+    double um1 = 0.0, um2 = 0.0;
+    bool fixed_masses = fixed_pair(ens[0], um1, um2);
+    for (int e = 1; e < n_ensembles && fixed_masses; ++e) {
+        double a = 0.0, b = 0.0;
+        fixed_masses = fixed_pair(ens[e], a, b) && a == um1 && b == um2;
+    }
+    const int uni_slot = (fixed_masses && !(o.variant & 1)) ? c.slot : -1;
     CK(cudaEventRecord(c.ev[1], s));
     for (long long lo = 0; lo < N; lo += chunk) {
         if (lo > 0) {                    // fresh work counters for every chunk; step counters and status accumulate

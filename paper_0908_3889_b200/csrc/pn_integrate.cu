@@ -889,7 +889,12 @@ cudaError_t pn_launch_fused(PnKernelParams& p, int grid_blocks, cudaStream_t s, 
         pn_fused_keys_kernel<<<(p.n + 127) / 128, 128, 0, s>>>(p);
         ++g_pn_launches;
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        if ((e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s, 48 * 148 * 256)) != cudaSuccess) return e;
+        // 48 systems per resident lane and more with near-equal keys: input order (as pn_launch_integrate; SMs of THIS device)
+        int dev = 0, sms = 148;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        const long long n_flat = 48LL * sms * 256;
+        if ((e = pn_launch_cost_order(p.keys, p.n, p.order_scratch, p.order_out, s, (int)(n_flat < 0x7fffffffLL ? n_flat : 0x7fffffffLL))) != cudaSuccess) return e;
         p.order = p.order_out;
     }
     if (uni_slot < 0) return launch_fused_pair<-1>(p, grid_blocks, s);

@@ -117,6 +117,33 @@ def test_fused_single_fixed_mass_ensemble_takes_the_uniform_mass_kernel(pn):
         assert abs(kf["trial_steps"] / kg["trial_steps"] - 1) < 1e-3
 
 
+def test_fused_equal_mass_sweep_takes_the_same_kernel_as_the_chain(pn):
+    """Several ensembles that all have the SAME fixed masses (an equal-mass sweep over chi): the unfused
+    chain's seed kernel finds the concatenated batch uniform and runs the uniform-mass kernel, so the fused call must take
+    its uniform-mass instantiation too (it decides over ALL ensembles of the call), or step sequences and bin-edge counts
+    could differ.  Exact agreement of every count and of the trial-step totals; and one ensemble with other
+    masses in the call sends both sides to the generic kernel, again in exact agreement."""
+    chis = (0.3, 0.7, 1.0)
+    by_m1 = [dict(key=(21, k), omega0=0.02, q=(1.0, 1.0), chi1=(c, c), chi2=(c, c), m1_fixed=0.5) for k, c in enumerate(chis)]
+    by_q = [dict(key=(22, k), omega0=0.02, q=(1.0, 1.0), chi1=(c, c), chi2=(c, c)) for k, c in enumerate(chis)]
+    mixed = by_m1[:2] + [dict(key=(23, 0), omega0=0.02, q=(1.0, 1.0), chi1=(1.0, 1.0), chi2=(1.0, 1.0), m1_fixed=0.6)]
+    n = 3000 + 7
+    for specs, uniform in ((by_m1, True), (by_q, True), (by_m1[:1] + by_q[1:], True), (mixed, False)):
+        st_c, c, kc = chain(pn, specs, n, 0, n, 0.05, 1e-10, 1e-12, 50, 31)
+        st_f, f, kf = fused(pn, specs, n, 0, n, 0.05, 1e-10, 1e-12, 50, 31)
+        assert st_c == st_f == 0
+        same(f, c, n)
+        assert kf["trial_steps"] == kc["trial_steps"] and kf["rejected"] == kc["rejected"] and kf["landing_trials"] == kc["landing_trials"]
+        # the generic kernel (variant bit 0) rounds differently from the uniform-mass one: same n, r to 1e-9
+        _, g, kg = fused(pn, specs, n, 0, n, 0.05, 1e-10, 1e-12, 50, 31, variant=1)
+        if uniform:
+            assert not np.array_equal(f["moments"], g["moments"])      # the uniform-mass kernel did run
+        else:
+            assert kg["trial_steps"] == kf["trial_steps"]              # both are the generic kernel
+        assert np.array_equal(f["moments"][..., 0], g["moments"][..., 0])
+        assert np.allclose(f["pearson_r"], g["pearson_r"], rtol=0, atol=1e-9, equal_nan=True)
+
+
 def test_fused_against_the_oracle_chain(pn, oracle):
     specs = SWEEP[:2]
     n = 700
