@@ -341,6 +341,23 @@ def run_ours(args, cfg):
                                 "unfused_chain_ms_kernels": chain_ms, "pearson_r": fo["pearson_r"].cpu().numpy()[0].tolist(),
                                 "hist1_equals_unfused": bool(torch.equal(fo["hist1"], out["hist1"])),
                                 "hist2_equals_unfused": bool(torch.equal(fo["hist2"], out["hist2"]))}
+            # a sweep of 16 ensembles in ONE fused call (r against chi at equal masses), n/16 systems each:
+            # the default queue order for more than 4 ensembles (index order) next to the cost order it replaces
+            # (pn_options.variant bit 2; interleaved ensembles thrash the blocks' moment tables)
+            ns = max(n // 16, 1)
+            sweep = [pn.make_ensemble((20090826, k), cfg.omega0, q=(1.0, 1.0), chi1=((k + 1) / 16,) * 2, chi2=((k + 1) / 16,) * 2,
+                                      m1_fixed=0.5) for k in range(16)]
+            so = dict(pearson_r=torch.zeros(16, 3, dtype=torch.float64, device=dev), hist1=torch.zeros(16, 3, cfg.bins, dtype=torch.int64, device=dev))
+            sw = {}
+            for name, var in (("ms_kernels", 0), ("ms_kernels_cost_order", 4)):
+                t = []
+                for i in range(2):
+                    pn.pn_run_ensembles(sweep, ns, cfg.omegaf, cfg.rtol, cfg.atol, bins1=cfg.bins, variant=var, **so)
+                    t.append(pn.pn_last_kernel_ms()["integrate"])
+                sw[name] = float(min(t))
+            sw.update(ensembles=16, systems_per_ensemble=ns, inspirals_per_sec=16 * ns / (sw["ms_kernels"] * 1e-3),
+                      pearson_r_s1s2=[float(x) for x in so["pearson_r"][:, 0].cpu().numpy()])
+            widened["fused_sweep"] = sw
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

@@ -103,7 +103,8 @@ typedef struct pn_options {
     int grid_blocks;       /* tuning: blocks of the persistent grid (0: SMs x resident blocks) */
     int variant;           /* tests / tuning: kernel selection bits, results are unchanged (FP64 bit 0: to rounding).  1: always
                               the generic kernel (per-lane constants) even for uniform-mass batches; 2: always the
-                              scalar FP32 kernel instead of the packed two-systems-per-lane one */
+                              scalar FP32 kernel instead of the packed two-systems-per-lane one; 4: pn_run_ensembles
+                              orders the queue by cost even for more than 4 ensembles (measurement only: several times slower) */
 } pn_options;
 
 /* Same as pn_integrate with explicit options (opt == NULL: defaults). */
@@ -267,9 +268,10 @@ int pn_generate(const pn_ensemble* ens, int n_ensembles, long long n_total, long
  *               the uniform-mass kernel, exactly when pn_integrate would for the concatenated batch; otherwise the generic one.
  * Results equal the chain pn_generate -> pn_integrate -> pn_statistics on the same arguments: n, n_skipped and every
  * histogram count exactly (and reproducibly); means, M2x, M2y, Cxy and r to rounding (the order in which partial moments
- * are merged depends on timing: r agrees to ~1e-13, not bit for bit).  The queue of every chunk of 2^22 systems is issued
- * longest-expected-first like pn_integrate's (a draw-only pass writes the keys: 8 bytes of scratch per system of a chunk;
- * opt->input_order != 0: index order, no scratch).
+ * are merged depends on timing: r agrees to ~1e-13, not bit for bit).  For a call of at most 4 ensembles the queue of every
+ * chunk of 2^22 systems is issued longest-expected-first like pn_integrate's (a draw-only pass writes the keys: 8 bytes of
+ * scratch per system of a chunk; opt->input_order != 0: index order, no scratch).  A call of more ensembles is issued in
+ * index order: cost order would interleave the ensembles and make the blocks' 4-entry moment tables thrash.
  * Returns the worst per-system status like pn_integrate; pn_last_counters / pn_last_kernel_ms()[1] refer to the run.
  */
 int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long long n_total, long long first, long long count,

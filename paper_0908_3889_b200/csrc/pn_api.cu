@@ -541,7 +541,12 @@ extern "C" int pn_run_ensembles(const pn_ensemble* ens, int n_ensembles, long lo
     // the 3.6e8-system uniformity run): the uniform-mass fast kernel, constants from this stream context's row of the table
     // (DESIGN.md 7.8).  Ensembles with different masses share chunks, so they take the generic kernel (a launch per ensemble
     // would pay a drain tail per ensemble).
-    if (!o.input_order && N > 1024) {
+    // Cost order mixes the ensembles of a chunk: consecutive finishes of a thread then belong to arbitrary ensembles, and
+    // with more ensembles than the block's table holds (PN_FW) nearly every finish evicts a table entry into the global
+    // record under the ensemble's global lock.  Measured on a B200, 2^20 systems, equal-mass chi sweep: 16 ensembles 335 ms
+    // in cost order against 61.6 ms in index order, 64 ensembles 133 against 63 ms; up to 4 ensembles the two orders take
+    // the same time (profiles/r3_fused_sweep_order.md).  So: cost order only while every ensemble has a table entry.
+    if (!o.input_order && N > 1024 && (G <= PN_FW || (o.variant & 4))) {
         // longest-expected-first queue order inside every chunk: keys + order, 8 bytes per system of a chunk
         const size_t nc = (size_t)(N < chunk ? N : chunk);
         if ((rc = c.keys.ensure(sizeof(float) * nc)) != PN_OK) return rc;

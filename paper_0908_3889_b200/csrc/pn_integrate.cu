@@ -237,8 +237,9 @@ __constant__ double pn_uni_table[PN_UNI_SLOTS][PN_UNI_ROW];
 // a warp draws 32 systems AT ONCE, one per lane, into a shared-memory ring ([word][slot], conflict-free), and lanes
 // whose inspiral has finished pop records off the ring; the global queue counter is advanced by 32 per draw.
 // Statistics, three levels.  (1) Every THREAD keeps Welford moments (n, xbar, ybar, M2x, M2y, Cxy) per dot product in
-// its own shared-memory words, for one ensemble at a time: a finished system is added without any lock (queue order is
-// index order, so a thread's ensembles only grow).  (2) When its ensemble changes, and at kernel exit, a thread merges
+// its own shared-memory words, for one ensemble at a time: a finished system is added without any lock.  (In index order a
+// thread's ensembles only grow; in cost order they alternate, which is why pn_run_ensembles orders the queue by cost only
+// for calls of at most PN_FW ensembles, pn_api.cu.)  (2) When its ensemble changes, and at kernel exit, a thread merges
 // them (pairwise update) into the BLOCK's table of PN_FW ensembles under a shared-memory spin lock.  (3) A table entry
 // that has to make room, and every entry when the last thread of the block leaves, is merged into the ensemble's
 // global record under a per-ensemble global spin lock: a few hundred uncontended merges per ensemble.  (Tried before:
@@ -249,7 +250,6 @@ __constant__ double pn_uni_table[PN_UNI_SLOTS][PN_UNI_ROW];
 // integer atomics (one per finished system and dot product).  Counts are exact and reproducible; moments are
 // reproducible to rounding (the merge order depends on timing).
 #define PN_FREC (PN_REC + 4)      /* ring record: seed record + the three initial unit dot products (+ pad) */
-#define PN_FW 4                   /* ensembles a block accumulates at a time */
 #define PN_FDONE 13               /* done-ring record: 9 final components (S1, S2, L^), 3 initial dot products, {index, code} */
 template <int BLOCK> struct PnFusedSmem {
     // one base pointer; every array is at a compile-time offset (seven stored pointers would cost 14 registers in a

@@ -5,6 +5,7 @@
 #define PN_ORDER_BUCKETS 2048
 #define PN_UNI_SLOTS 4
 #define PN_UNI_ROW 32
+#define PN_FW 4                   /* fused mode: ensembles a block accumulates at a time (the block's moment table) */
 
 // Arguments of the integrator kernels.  All arrays are DEVICE pointers in SoA layout with stride n:
 // y0[c*n + i], masses[j*n + i], yf[c*n + i].
