@@ -314,6 +314,20 @@ int pn_selfcheck(const double* init_states, const double* masses, const double* 
 int pn_stream_status(void* stream);
 
 /*
+ * pn_stream_release -- gives back what the library holds for `stream` on the current device: its scratch context
+ * (device staging buffers, work counters, events, a pending async status, which is discarded) and its row of the
+ * uniform-mass constant table.  Synchronises the stream first.  Call it before destroying a stream the library has
+ * been used on: contexts are keyed by (device, stream handle), the runtime may hand the same handle value to a later
+ * stream, and that stream would otherwise inherit the old context (harmless for results, but with a stale pending
+ * status); and every stream ever used would keep its buffers until pn_shutdown.
+ * The table has 4 rows per device: the first 4 live (unreleased) streams of a device get one, further streams run the
+ * generic FP64 kernel even on uniform-mass batches, which is slower by a few percent and rounds differently
+ * (same step counts for ~98 % of systems, final states to ~1e-11).  A stream that was never used, or
+ * was already released, is a successful no-op.
+ */
+int pn_stream_release(void* stream);
+
+/*
  * pn_measure_fma_peak -- measured FMA throughput of this device at its current clocks: every thread
  * runs `chains` independent dependent-FMA chains (no memory traffic) for about `seconds`.
  * Writes achieved TFLOP/s (2 flops per FMA) and, if not NULL, the SM clock in MHz estimated from

@@ -19,7 +19,7 @@ PN_OK, PN_EINVAL, PN_ECUDA, PN_ENOTCONVERGED, PN_ENONFINITE, PN_ETOOLARGE = 0, 1
 PN_STATIC_MAX_GROUPS, PN_STATIC_SCRATCH_BYTES = 1024, 344064
 FAIL_MAXSTEPS, FAIL_HUNDERFLOW, FAIL_NONFINITE, FAIL_LANDING, FAIL_BADINPUT = -1, -2, -3, -4, -5
 
-EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_statistics_static", "pn_merge_statistics", "pn_generate", "pn_run_ensembles", "pn_selfcheck", "pn_stream_status",
+EXPORTS = ["pn_integrate", "pn_integrate_ex", "pn_histogram", "pn_histogram_ex", "pn_statistics", "pn_statistics_static", "pn_merge_statistics", "pn_generate", "pn_run_ensembles", "pn_selfcheck", "pn_stream_status", "pn_stream_release",
            "pn_measure_fma_peak", "pn_measure_fma_operands", "pn_last_counters", "pn_last_redo_count", "pn_last_kernel_ms", "pn_launch_count", "pn_strerror",
            "pn_last_cuda_error", "pn_shutdown", "pn_version"]
 
@@ -88,6 +88,7 @@ def load():
         lib.pn_selfcheck.argtypes = [vp, vp, vp, vp, ll, d, d, C.POINTER(C.c_ulonglong), d, d, C.POINTER(PnCheckOut), vp, ll,
                                      C.POINTER(PnOptions)]
         lib.pn_stream_status.argtypes = [vp]
+        lib.pn_stream_release.argtypes = [vp]
         lib.pn_measure_fma_peak.argtypes = [i, d, C.POINTER(d), C.POINTER(d)]
         lib.pn_measure_fma_operands.argtypes = [i, i, C.POINTER(d)]
         lib.pn_last_counters.argtypes = [C.POINTER(C.c_ulonglong)] * 4
@@ -362,6 +363,11 @@ def pn_selfcheck(init_states, masses, final_states, omegaf, *, fraction=0.01, ke
 
 def pn_stream_status(stream=None):
     return load().pn_stream_status(None if stream is None else int(getattr(stream, "cuda_stream", stream)))
+
+
+def pn_stream_release(stream=None):
+    """pn_stream_release of include/pn.h: frees the library's scratch context of `stream` (call before destroying it)."""
+    return _check(load().pn_stream_release(None if stream is None else int(getattr(stream, "cuda_stream", stream))))
 
 
 def pn_measure_fma_peak(precision=PN_FP64, seconds=0.25):

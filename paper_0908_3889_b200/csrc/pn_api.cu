@@ -63,20 +63,44 @@ struct Ctx {
                     &h_steps, &h_time, &h_rej, &h_counts, &st_scratch, &st_in, &st_out, &gen_specs, &gen_y, &gen_m, &ck_idx,
                     &ck_tmp, &ck_sub, &ck_out, &ck_in, &fu_scr};
 };
-static std::map<void*, Ctx*> g_ctx;
-static int g_next_slot = 0;
+// Contexts are keyed by (device, stream): the NULL stream (and any handle value) of two devices are different streams, and
+// the buffers, events and the __constant__ table row of a context belong to the device it was created on.
+typedef std::pair<int, void*> CtxKey;
+static std::map<CtxKey, Ctx*> g_ctx;
+#define PN_MAX_DEVICES 64
+static bool g_slot_used[PN_MAX_DEVICES][PN_UNI_SLOTS];     // rows of each device's uniform-mass table in use by a context
 static float g_ms[4] = {0, 0, 0, 0};
 static unsigned long long g_counters[4] = {0, 0, 0, 0};
 static unsigned g_redo_count = 0;   // systems that went through the redo pass in the last synchronous call
 
+static int current_device()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); dev = 0; }
+    return dev;
+}
+
 static Ctx* ctx_for(void* stream)
 {
-    auto it = g_ctx.find(stream);
+    const int dev = current_device();
+    auto it = g_ctx.find(CtxKey(dev, stream));
     if (it != g_ctx.end()) return it->second;
     Ctx* c = new Ctx();
-    c->slot = g_next_slot < PN_UNI_SLOTS ? g_next_slot++ : -1;
-    g_ctx[stream] = c;
+    // a row of this device's table, if one is free (pn_stream_release returns rows); none left: the generic kernel only
+    if (dev >= 0 && dev < PN_MAX_DEVICES)
+        for (int k = 0; k < PN_UNI_SLOTS && c->slot < 0; ++k)
+            if (!g_slot_used[dev][k]) { g_slot_used[dev][k] = true; c->slot = k; }
+    g_ctx[CtxKey(dev, stream)] = c;
     return c;
+}
+
+static int free_ctx(Ctx* c)
+{
+    int rc = PN_OK;
+    for (Buf* b : c->all) if (b->release() != PN_OK) rc = PN_ECUDA;
+    if (c->ev_ok) for (int i = 0; i < 5; ++i) cudaEventDestroy(c->ev[i]);
+    delete c;
+    return rc;
 }
 
 // layout of g_small: [0..3] counters (u64), then queue (u32), status (i32)
@@ -696,7 +720,7 @@ extern "C" int pn_stream_status(void* stream)
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
     int st = PN_OK;
-    auto it = g_ctx.find(stream);
+    auto it = g_ctx.find(CtxKey(current_device(), stream));
     if (it != g_ctx.end() && it->second->async_pending) {
         Ctx& c = *it->second;
         Small hs;
@@ -765,15 +789,22 @@ extern "C" int pn_shutdown(void)
 {
     int rc = PN_OK;
     if (cudaDeviceSynchronize() != cudaSuccess) rc = PN_ECUDA;
-    for (auto& kv : g_ctx) {
-        Ctx* c = kv.second;
-        for (Buf* b : c->all) if (b->release() != PN_OK) rc = PN_ECUDA;
-        if (c->ev_ok) for (int i = 0; i < 5; ++i) cudaEventDestroy(c->ev[i]);
-        delete c;
-    }
+    for (auto& kv : g_ctx) if (free_ctx(kv.second) != PN_OK) rc = PN_ECUDA;
     g_ctx.clear();
-    g_next_slot = 0;
+    memset(g_slot_used, 0, sizeof g_slot_used);
     return rc;
+}
+
+extern "C" int pn_stream_release(void* stream)
+{
+    auto it = g_ctx.find(CtxKey(current_device(), stream));
+    if (it == g_ctx.end()) return PN_OK;
+    CK(cudaStreamSynchronize((cudaStream_t)stream));
+    Ctx* c = it->second;
+    const int dev = it->first.first;
+    if (c->slot >= 0 && dev >= 0 && dev < PN_MAX_DEVICES) g_slot_used[dev][c->slot] = false;
+    g_ctx.erase(it);
+    return free_ctx(c);
 }
 
 extern "C" int pn_version(void) { return PN_VERSION; }

@@ -332,6 +332,53 @@ def test_async_calls_keep_their_status_and_scratch(pn):
     assert again["status"] == 0 and np.array_equal(again["final"], ref3["final"])
 
 
+def test_stream_release_recycles_contexts_and_table_rows(pn):
+    """pn_stream_release (include/pn.h): a device has 4 rows in the uniform-mass constant table, one per live stream
+    context.  A 5th live stream runs the generic kernel (rounding differs); releasing a stream returns its row, so any
+    number of short-lived streams keep the fast path, a released stream leaves no pending status behind, and a stream
+    that was never used is a no-op."""
+    dev = "cuda:0"
+    cfg = W.with_size(W.CONFIGS["C4"], 2000 + 9)
+    y, m = W.generate(cfg)
+    pn.pn_shutdown()                                       # forget the contexts of earlier tests
+    ref_u = gpu_integrate(pn, y, m, cfg)                   # default stream: row 0
+    ref_g = gpu_integrate(pn, y, m, cfg, variant=1)
+    assert not np.array_equal(ref_u["final"], ref_g["final"])          # the two kernels differ in rounding
+    d_y, d_m = torch.from_numpy(y).to(dev), torch.from_numpy(m).to(dev)
+
+    def run_on(s):
+        f = torch.full((cfg.n, 10), float("nan"), dtype=torch.float64, device=dev)
+        st = torch.zeros(cfg.n, dtype=torch.int32, device=dev)
+        s.wait_stream(torch.cuda.current_stream())
+        assert pn.pn_integrate(d_y, d_m, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, f, st, stream=s, async_=True) == 0
+        assert pn.pn_stream_status(s) == 0
+        return f.cpu().numpy()
+
+    # ten streams one after another, each released: every one gets a table row
+    for _ in range(10):
+        s = torch.cuda.Stream()
+        assert np.array_equal(run_on(s), ref_u["final"])
+        assert pn.pn_stream_release(s) == 0
+    # without release: rows 1-3 go to three streams, the next live stream has none and runs the generic kernel
+    held = [torch.cuda.Stream() for _ in range(4)]
+    for s in held[:3]:
+        assert np.array_equal(run_on(s), ref_u["final"])
+    assert np.array_equal(run_on(held[3]), ref_g["final"])
+    # ... until a row is given back (the context of held[3] was created without one: release it too)
+    assert pn.pn_stream_release(held[0]) == 0 and pn.pn_stream_release(held[3]) == 0
+    assert np.array_equal(run_on(held[3]), ref_u["final"])
+    # a pending async status dies with the context; an unused stream is a no-op
+    m_bad = m.copy(); m_bad[1, 0] = -1.0
+    f = torch.empty(cfg.n, 10, dtype=torch.float64, device=dev); st = torch.zeros(cfg.n, dtype=torch.int32, device=dev)
+    pn.pn_integrate(d_y, torch.from_numpy(m_bad).to(dev), 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, f, st, stream=held[1], async_=True)
+    assert pn.pn_stream_release(held[1]) == 0 and pn.pn_stream_status(held[1]) == 0
+    assert pn.pn_stream_release(torch.cuda.Stream()) == 0
+    for s in held[2:]:
+        pn.pn_stream_release(s)
+    again = gpu_integrate(pn, y, m, cfg)
+    assert np.array_equal(again["final"], ref_u["final"])
+
+
 def test_fma_microbenchmark_is_self_consistent(pn):
     """The FP64 peak and operand-port micro-benchmarks behind the roofline denominator: the SM clock
     estimated from the longest per-block clock64() span agrees with nvidia-smi, the throughput with 64 FMA lanes per SM
