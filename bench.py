@@ -370,12 +370,15 @@ def run_ours(args, cfg):
     peak_nominal = sms * lanes * 2 * sm_max * 1e6 / 1e12
     peak_prec = pn.PN_FP64 if prec == pn.PN_FP64 else pn.PN_FP32       # the pipe the slopes are computed on
     peak_meas, peak_mhz = pn.pn_measure_fma_peak(peak_prec, 0.5)
-    traffic, traffic_src = None, None
+    traffic, traffic_src, executed = None, None, None
     tj = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tj):
         ent = json.load(open(tj)).get(f"{cfg.name}:{n}")
         if ent:
             traffic, traffic_src = float(ent["dram_bytes_read"]) + float(ent["dram_bytes_write"]), ent["source"]
+            ex = ent.get("fp64_inst_per_trial_step")
+            if ex:       # what the captured kernel executes per trial step, in flops (FMA = 2), next to the fixed F_STEP
+                executed = dict(ex, flops=2 * ex["dfma"] + ex["dmul"] + ex["dadd"], source=ent["source"])
     flops_launch = float(np.mean(trial_steps)) * F_STEP + n * F_RHS
     k_ms = float(np.mean(kern_ms))
     achieved = flops_launch / (k_ms * 1e-3) / 1e12
@@ -404,6 +407,11 @@ def run_ours(args, cfg):
                      "peak_measured_ffma2": pn.pn_measure_fma_peak(3, 0.25)[0] if peak_prec == pn.PN_FP32 else None,
                      "frac_of_measured_fma": achieved / peak_meas if peak_meas > 0 else None,
                      "flops_per_trial_step": F_STEP, "flops_per_rhs": F_RHS,
+                     # F_STEP / F_RHS are a FIXED algorithmic count of the method, not a count of what this
+                     # kernel executes: they have not moved since r1 although the kernel now does less arithmetic per RHS
+                     # (folded constants, shared products) and more for cbrt / log than the count books (2 per stage).
+                     "flops_basis": "fixed algorithmic count, independent of the implementation (DESIGN.md 6.2)",
+                     "executed_fp64_per_trial_step": executed,
                      "frac_with_oracle_as_printed_count": (float(np.mean(trial_steps)) * F_STEP_ORACLE + n * F_RHS_ORACLE)
                      / (k_ms * 1e-3) / 1e12 / peak_nominal,
                      "fma_issue_cycles_by_register_sources": {str(k): pn.pn_measure_fma_operands(peak_prec, k) for k in (1, 2, 3)},

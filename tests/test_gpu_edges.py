@@ -176,16 +176,19 @@ def test_loose_tolerance_uses_the_redo_pass(pn, oracle):
     assert (np.abs(g["final"] - r["final"]) / comp_scale(y0[:64])).max() <= 1e-11
 
 
-def close_runs(a, b, frac_same_steps=0.98):
-    """Two FP64 runs of the same systems whose arithmetic differs only in rounding (constants folded differently): the
-    same step sequence for almost every system, final states equal to rounding-error growth there (1e-11), and to the
-    integration tolerance (1e-8) for the few systems where an accept/reject decision with E within rounding of 1 fell
-    the other way."""
+def close_runs(a, b, frac_same_steps=0.999, rtol=1e-10):
+    """Two FP64 runs of the same systems whose arithmetic differs only in rounding (constants folded differently).
+    Bounds, with the measurement behind them (B200, uniform-mass vs generic kernel, rtol 1e-10: C4 x 200,000 systems,
+    C2 x 20,000, C1 x 1024): the step sequence is the same unless an accept / reject decision with E within rounding of 1
+    falls the other way, which happened to 6.5e-5 of the systems at worst (asserted: at most 1e-3); with the same step
+    sequence the final states differ by accumulated rounding, 2.2e-13 at worst over ~1100 steps (asserted: 1e-2 rtol);
+    with a different one both are solutions within the tolerance and differ by less than one step's allowed local
+    error, measured 2.2e-13 (asserted: rtol); final times agreed to 2e-14 relative (asserted: 1e-2 rtol)."""
     same = a["steps"] == b["steps"]
     assert same.mean() >= frac_same_steps, same.mean()
-    assert np.abs(a["final"][same] - b["final"][same]).max() <= 1e-11
-    assert np.abs(a["final"] - b["final"]).max() <= 1e-8
-    assert np.abs(a["time"] / b["time"] - 1).max() <= 1e-9
+    assert np.abs(a["final"][same] - b["final"][same]).max() <= 1e-2 * rtol
+    assert np.abs(a["final"] - b["final"]).max() <= rtol
+    assert np.abs(a["time"] / b["time"] - 1).max() <= 1e-2 * rtol
 
 
 def test_uniform_mass_fast_path_matches_the_generic_kernel(pn):

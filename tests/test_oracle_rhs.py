@@ -217,3 +217,33 @@ def test_two_spin_precession_by_hand(oracle):
     assert np.abs(f[1:] - expect).max() < 2e-17 + 1e-14 * np.abs(expect).max()
     # a wrong "3" (say 2) would move S1_dot_y by 0.5*0.4/4/256 = 1.95e-4; a missing 1/M^2 would quadruple S1_dot_z
     assert abs(f[2] * 256 - 1.34) < 1e-13 and abs(f[3] * 256 + 0.03125) < 1e-15
+
+
+def test_spin_spin_term_of_eq1_by_hand(oracle):
+    """The two numbers of the 2PN spin-spin term of Eq. (1), -(1/48) eta chi_1 chi_2 (247 S^_1.S^_2 - 721 (L^.S^_1)(L^.S^_2))
+    (M omega)^{4/3}, each on its own (aligned spins only see 247 - 721, and the symmetries hold
+    for any pair of numbers).  The term is isolated as the difference of the (M omega)^{4/3} piece with and without the
+    spin terms (term_mask bit 4, bit 16), on states whose numbers are exact:
+
+    m = (1.2, 0.8): M = 2, eta = 0.24, m_1^2 = 1.44, m_2^2 = 0.64.  omega = 1/16: M omega = 1/8, (M omega)^{5/3} = 1/32,
+    (M omega)^{4/3} = 1/16.  Prefactor of the brace: omega^2 (96/5) eta (M omega)^{5/3} = (1/256)(19.2)(0.24)/32.
+    chi_1 = chi_2 = 1/2 (chi_1 chi_2 = 1/4), L^ = z.
+      (a) S^_1 = (0.6, 0, 0.8), S^_2 = (-0.8, 0, 0.6): S^_1.S^_2 = 0, (L^.S^_1)(L^.S^_2) = 0.48: only 721 survives,
+          term = -(1/48)(0.24)(1/4)(-721 * 0.48)/16 = +0.00125 * 346.08 / 16
+      (b) S^_1 = (1, 0, 0), S^_2 = (0.6, 0, 0.8): L^.S^_1 = 0, S^_1.S^_2 = 0.6: only 247 survives,
+          term = -(1/48)(0.24)(1/4)(247 * 0.6)/16 = -0.00125 * 148.2 / 16"""
+    m = np.array([[1.2, 0.8]])
+    pre = (1 / 256) * 19.2 * 0.24 / 32
+    with_spin, without = (1 << 4) | (1 << 16), (1 << 4)
+    cases = [((0.6, 0.0, 0.8), (-0.8, 0.0, 0.6), +0.00125 * 346.08 / 16),
+             ((1.0, 0.0, 0.0), (0.6, 0.0, 0.8), -0.00125 * 148.2 / 16)]
+    for s1, s2, term in cases:
+        y = np.concatenate([[1 / 16], 0.5 * 1.44 * np.array(s1), 0.5 * 0.64 * np.array(s2), [0, 0, 1.0]])[None]
+        d = oracle.rhs(y, m, term_mask=with_spin)[0, 0] - oracle.rhs(y, m, term_mask=without)[0, 0]
+        assert abs(d / (pre * term) - 1) < 1e-12, (d, pre * term)
+    # what a slip would do: 247 <-> 721 swapped changes (a) by the factor 247/721 and (b) by 721/247; a wrong sign
+    # between them leaves (a) and (b) with the wrong sign on one of the two; both are far outside 1e-12
+    # the non-spin part of the same order, for scale: 34103/18144 + 13661/2016 eta + 59/18 eta^2 at eta = 0.24
+    y = np.concatenate([[1 / 16], np.zeros(6), [0, 0, 1.0]])[None]
+    t4 = 34103 / 18144 + 13661 / 2016 * 0.24 + 59 / 18 * 0.24 ** 2
+    assert abs(oracle.rhs(y, m, term_mask=without)[0, 0] / (pre * t4 / 16) - 1) < 1e-12
