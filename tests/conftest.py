@@ -10,7 +10,6 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
-    config.addinivalue_line("markers", "slow: opt-in full-batch oracle comparisons (set PN_RUN_SLOW=1)")
 
 
 @pytest.fixture(scope="session")

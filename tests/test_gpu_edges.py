@@ -397,42 +397,3 @@ def test_fma_microbenchmark_is_self_consistent(pn):
     assert abs(cyc[0] - 2.0) < 0.25 and abs(cyc[1] - 2.0) < 0.1 and abs(cyc[2] - 3.0) < 0.15, cyc
     # the issue model of DESIGN.md 7.2: integer instructions do NOT issue in the shadow of a 2-cycle DFMA
     assert 3.3 < pn.pn_measure_fma_operands(pn.PN_FP64, 4) < 4.3        # 2 if they issued in the DFMA's shadow; measured 3.7
-
-
-@pytest.mark.slow
-def test_full_C2_batch_against_the_oracle_chain(pn, oracle, tmp_path_factory):
-    """Opt-in (PN_RUN_SLOW=1; ~1-2 minutes of host time): the WHOLE C2 batch (2^20 inspirals) through the oracle, once,
-    cached on disk under a hash of the inputs and options; then every one of the 3 x 2^20 final dot products and the three
-    50-bin histograms of the GPU chain (pn_integrate -> pn_histogram) against the oracle chain (counts
-    must agree except for systems whose dot product lies within 1e-7 of a bin edge)."""
-    import hashlib
-    import os
-
-    if os.environ.get("PN_RUN_SLOW", "0") != "1":
-        pytest.skip("set PN_RUN_SLOW=1 to run the full-batch oracle comparison")
-    cfg = W.CONFIGS["C2"]
-    y0, m = W.generate(cfg)
-    key = hashlib.sha256(y0.tobytes() + m.tobytes() + repr((cfg.omegaf, cfg.rtol, cfg.atol)).encode()).hexdigest()[:16]
-    cache = os.path.join(os.environ.get("PN_ORACLE_CACHE", "/tmp"), f"pn_oracle_C2_{key}.npz")
-    if os.path.exists(cache):
-        z = np.load(cache)
-        ref = dict(final=z["final"], time=z["time"], steps=z["steps"])
-    else:
-        ref = oracle.integrate(y0, m, cfg.omegaf, cfg.rtol, cfg.atol, n_threads=os.cpu_count() or 1)
-        np.savez(cache, final=ref["final"], time=ref["time"], steps=ref["steps"])
-    assert np.all(ref["steps"] > 0)
-    g = gpu_integrate(pn, y0, m, cfg)
-    assert g["status"] == 0
-    c_ref, _, d_ref = oracle.histogram(ref["final"], cfg.bins)
-    d_gpu = dots_of(oracle, g["final"])
-    assert np.abs(d_gpu - d_ref).max() <= 1e-7
-    assert np.abs(g["time"] / ref["time"] - 1).max() <= 1e-7
-    counts = torch.zeros(3, cfg.bins, dtype=torch.int64, device="cuda:0")
-    pn.pn_histogram(g["d_final"], cfg.bins, counts)
-    diff = np.abs(counts.cpu().numpy() - c_ref.astype(np.int64))
-    # systems within 1e-7 of a bin edge may fall either side (the oracle lists them)
-    edges = np.linspace(-1, 1, cfg.bins + 1)[1:-1]
-    near = [(np.abs(d_ref[:, k][:, None] - edges[None, :]).min(axis=1) <= 1e-7).sum() for k in range(3)]
-    for k in range(3):
-        assert diff[k].sum() <= 2 * near[k], (k, diff[k].sum(), near[k])
-    assert abs(g["steps"].mean() / ref["steps"].mean() - 1) < 0.01

@@ -159,6 +159,28 @@ def test_fused_against_the_oracle_chain(pn, oracle):
         assert np.abs(f["moments"][e, :, 1:3] - ref["moments"][0, :, 1:3]).max() < 1e-9
 
 
+def test_fused_uniform_mass_kernel_against_the_oracle_chain(pn, oracle):
+    """ONE fixed-mass ensemble selects the uniform-mass instantiation of the fused kernel (the one bench.py times as
+    widened.fused): compared directly with the oracle chain (generator oracle -> integrator oracle -> statistics oracle),
+    not through the unfused device chain.  4096 + 37 systems: several draws per warp and a ragged last one."""
+    n = 4096 + 37
+    for spec in (SWEEP[0], SWEEP[2]):
+        _, f, kf = fused(pn, [spec], n, 0, n, 0.05, 1e-10, 1e-12, 50, 20)
+        _, g, _ = fused(pn, [spec], n, 0, n, 0.05, 1e-10, 1e-12, 50, 20, variant=1)
+        assert not np.array_equal(f["moments"], g["moments"])          # the uniform-mass kernel did run
+        y0, m = G.generate(G.make_spec(**spec), n)
+        o = oracle.integrate(y0, m, 0.05, 1e-10, 1e-12)
+        ref = S.statistics(y0, o["final"], o["steps"], None, 50, 20)
+        defined = np.isfinite(ref["r"][0])
+        assert np.array_equal(defined, np.isfinite(f["pearson_r"][0]))
+        assert np.abs(f["pearson_r"][0] - ref["r"][0])[defined].max() < 1e-8
+        assert np.abs(f["hist1"][0] - ref["hist1"][0].astype(np.int64)).sum() <= 4
+        assert np.abs(f["hist2"][0] - ref["hist2"][0].astype(np.int64)).sum() <= 8
+        assert np.array_equal(f["moments"][0, :, 0], ref["moments"][0, :, 0])
+        assert np.abs(f["moments"][0, :, 1:3] - ref["moments"][0, :, 1:3]).max() < 1e-9
+        assert abs(kf["trial_steps"] / int(o["steps"].sum()) - 1) < 1e-3
+
+
 def test_fused_redo_pass_failures_and_host_buffers(pn):
     # loose tolerance: steps leave the range of the cbrt/log series, such systems go through the redo pass of the fused mode too
     st_c, c, kc = chain(pn, SWEEP[:2], 3000, 0, 3000, 0.05, 1e-3, 1e-5, 40, 0)
