@@ -5,7 +5,7 @@ One "step" = one pass of the whole hot path over one batch of synthetic inspiral
 (default: C2 of BASELINE.json, 2^20 equal-mass maximally spinning inspirals, FP64, omega 0.005->0.05,
 rtol 1e-10): stage-in, persistent DP5(4) integrator, stage-out, histogram kernel.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference] [--scaling weak|strong]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference] [--scaling weak|strong] [--fused]
 
 Prints ONE JSON line (see DESIGN.md 6 for every field).  Multi-GPU: one process per GPU.  Started
 under torchrun (RANK / LOCAL_RANK / WORLD_SIZE / MASTER_* in the environment) it uses those ranks; started as
@@ -193,10 +193,108 @@ def run_dry(args, cfg):
     counts[:, rank % cfg.bins] = n_mine                          # stand-in for this rank's histogram
     sharding.allreduce_counts(counts, dist if world > 1 else None)
     slowest = sharding.max_over_ranks(float(rank + 1), torch.device("cpu"), dist if world > 1 else None)
+    fused = None
+    if args.fused:
+        # --fused: the exchange of a sharded ensemble run (sharding.combine_statistics) with stand-in records: this rank's
+        # slice of ONE ensemble of n_total systems; the stand-in merge only adds the counts n of the gathered records
+        n_total = cfg.n * world if args.scaling == "weak" else cfg.n
+        lo, hi = sharding.shard_range(n_total, rank, world)
+        mom = torch.zeros(1, 3, 6, dtype=torch.float64)
+        mom[..., 0] = hi - lo
+        local = dict(moments=mom, hist1=torch.full((1, 3, cfg.bins), hi - lo, dtype=torch.int64))
+        res = sharding.combine_statistics(local, dist if world > 1 else None, lambda parts: (parts.sum(dim=0), parts.sum(dim=0)[..., 0]))
+        fused = {"systems_all_ranks": int(res["moments"][0, 0, 0].item()), "systems_expected": n_total,
+                 "hist1_cell": int(res["hist1"][0, 0, 0].item()), "slice_rank0": [lo, hi]}
     if rank == 0:
         print(json.dumps({"dry": True, "n_gpus": world, "scaling": args.scaling, "seed_rank0": gen_cfg.seed,
                           "systems_rank0": n_mine, "systems_all_ranks": int(counts[0].sum().item()), "systems_expected": total,
-                          "max_over_ranks": slowest, "config": {"workload": cfg.name}}))
+                          "max_over_ranks": slowest, "fused": fused, "config": {"workload": cfg.name}}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_fused(args, cfg):
+    """--fused: a step is ONE sharded fused ensemble run of the workload's ensemble (pipeline.run_ensembles(fused=True,
+    dist=...): seed in, statistics out, no state arrays; SURVEY.md 8(f) NEXT-1..3).  Weak scaling: the
+    ensemble has cfg.n systems per rank; strong: cfg.n in all.  Every rank integrates its slice of the variate stream;
+    the exchange per step is an int64 all-reduce of the counters and an all-gather of 18 doubles per ensemble.  Not the
+    BASELINE.json metric's configuration (that is the default mode): a line for the widened rows."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_0908_3889_b200 as pn
+    from paper_0908_3889_b200 import sharding
+
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    if cfg.precision not in ("fp64",):
+        raise SystemExit("bench.py --fused: the fused mode is FP64 only")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    d = dist if world > 1 else None
+    n_total = cfg.n * world if args.scaling == "weak" else cfg.n
+    spec = W.generator_spec(cfg)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        return pn.run_ensembles([spec], n_total, cfg.omegaf, rtol=cfg.rtol, atol=cfg.atol, bins1=cfg.bins, bins2=79, fused=True,
+                                dist=d, shard=(rank, world) if world > 1 else None)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(); flush.zero_()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    launches0 = pn.pn_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kern_ms, trial_steps = [], []
+    ev0.record(stream)
+    for _ in range(args.steps):
+        res = step()
+        kern_ms.append(pn.pn_last_kernel_ms()["integrate"]); trial_steps.append(pn.pn_last_counters()["trial_steps"])
+        flush.zero_()
+    ev1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms_step = sharding.max_over_ranks(ev0.elapsed_time(ev1), dev, d) / args.steps
+    steps_all = torch.tensor([float(np.mean(trial_steps))], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(steps_all)
+    if rank == 0:
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak = sms * FP64_LANES_PER_SM * 2 * float(clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+        n_mine = n_total // world
+        achieved = (float(np.mean(trial_steps)) * F_STEP + n_mine * F_RHS) / (float(np.mean(kern_ms)) * 1e-3) / 1e12
+        G = 1
+        print(json.dumps({
+            "metric": "inspirals_per_sec", "value": n_total / (ms_step * 1e-3), "unit": "inspirals/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling,
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic (drawn on the device from the seed)",
+            "comm": {"backend": "nccl" if world > 1 else None, "nranks": world,
+                     "exchange": "per step: int64 all-reduce of n_skipped, hist1, hist2; all-gather of 18 doubles per ensemble; max of the status"},
+            "config": {"workload": cfg.name, "mode": "fused ensemble run (pn_run_ensembles), sharded by slices of the variate stream",
+                       "n_inspirals": n_total, "n_inspirals_per_gpu": n_mine, "omega0": cfg.omega0, "omegaf": cfg.omegaf, "rtol": cfg.rtol,
+                       "atol": cfg.atol, "bins": cfg.bins, "bins2": 79, "parallelism": f"stream-sharded x{world}",
+                       "l2": "256 MiB memset between steps"},
+            "rhs_evals_per_sec": (6.0 * float(steps_all.item()) + n_total) / (ms_step * 1e-3),
+            "kernel_ms": {"integrate": float(np.mean(kern_ms))},
+            "roofline": {"bound": "alu", "kernel": "pn_integrate_adaptive_kernel<..., FUSED>", "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                         "flops_basis": "fixed algorithmic count, independent of the implementation (DESIGN.md 6.2)"},
+            # the call a user makes takes a seed and returns statistics: its end-to-end time IS the step
+            "e2e": {"value": n_total / (ms_step * 1e-3), "unit": "inspirals/s", "h2d_bytes_per_step": 88 * G,
+                    "d2h_bytes_per_step": int(8 * G * (3 + 18 + 3 + 3 * cfg.bins + 3 * 79 * 79 + 3)), "steps": args.steps},
+            "pearson_r": [float(x) for x in res["pearson_r"][0]], "status": int(res["status"]),
+            "gpu_launches": int(pn.pn_launch_count() - launches0), "clocks": clocks}))
     if world > 1:
         dist.destroy_process_group()
 
@@ -448,6 +546,8 @@ def main():
     ap.add_argument("--variant", type=int, default=0, help="pn_options.variant (kernel selection bits; not a bench line unless 0)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="weak: every rank its own full-size batch; strong: one batch split over the ranks")
+    ap.add_argument("--fused", action="store_true",
+                    help="a step is one sharded fused ensemble run (pn_run_ensembles through pipeline.run_ensembles): widened rows")
     ap.add_argument("--dry", action="store_true", help="launch / sharding / exchange logic only, on the CPU with gloo (tests)")
     args = ap.parse_args()
     cfg = W.CONFIGS[args.workload]
@@ -458,6 +558,8 @@ def main():
         run_dry(args, cfg)
     elif args.impl == "reference":
         run_reference(args, cfg)
+    elif args.fused:
+        run_fused(args, cfg)
     else:
         run_ours(args, cfg)
 

@@ -45,3 +45,38 @@ def allgather_moments(moments, dist=None):
     parts = [torch.empty_like(moments) for _ in range(dist.get_world_size())]
     dist.all_gather(parts, moments.contiguous())
     return torch.stack(parts).contiguous()
+
+
+_COUNTERS = ("n_skipped", "hist1", "hist2")
+
+
+def combine_statistics(local, dist=None, merge=None):
+    """Ensemble statistics over a run that is sharded per section 8 of DESIGN.md: every rank holds the statistics of ITS
+    slice [lo, hi) of every ensemble (pn_run_ensembles / pn_statistics outputs as tensors: 'moments' [G, 3, 6], and the
+    integer counters 'n_skipped', 'hist1', 'hist2' where present).  The exchange: the counters are summed by an integer
+    all-reduce; the moment records are all-gathered in rank order and merged by `merge(parts) -> (moments, pearson_r)`
+    (pn_merge_statistics on the GPUs; the arithmetic stays in the library).  Returns a new dict; every rank gets the
+    statistics of the whole run.  hist2_max is the largest cell of the summed bivariate histogram."""
+    out = dict(local)
+    for k in _COUNTERS:
+        if out.get(k) is not None:
+            out[k] = allreduce_counts(out[k].clone(), dist)
+    out["moments"], out["pearson_r"] = merge(allgather_moments(local["moments"], dist))
+    if out.get("hist2") is not None:
+        out["hist2_max"] = out["hist2"].flatten(2).amax(dim=2)
+    return out
+
+
+def merge_shards(locals_in_rank_order, merge):
+    """combine_statistics for shards that live in ONE process (tests; several shards run one after another on one GPU):
+    same sums, same merge order."""
+    import torch
+
+    out = dict(locals_in_rank_order[0])
+    for k in _COUNTERS:
+        if out.get(k) is not None:
+            out[k] = torch.stack([d[k] for d in locals_in_rank_order]).sum(dim=0)
+    out["moments"], out["pearson_r"] = merge(torch.stack([d["moments"] for d in locals_in_rank_order]).contiguous())
+    if out.get("hist2") is not None:
+        out["hist2_max"] = out["hist2"].flatten(2).amax(dim=2)
+    return out

@@ -80,3 +80,34 @@ def test_run_ensembles_pipeline(oracle):
         y0, m = G.generate(G.make_spec(**s), 4000)
         o = oracle.integrate(y0, m, OMEGAF, 1e-10, 1e-12)
         assert np.abs(S.statistics(y0, o["final"])["r"][0] - res["pearson_r"][e]).max() < 5e-4
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_sharded_sweep_equals_the_unsplit_call(fused):
+    """NEXT-3 "sharded over GPUs per 8(e)" on one GPU: the seven ensembles of the sweep, every ensemble's variate stream
+    split three ways (sharding.shard_range; what three ranks would run), each share through pipeline.run_ensembles, the
+    shares combined as the ranks combine them (counters summed, moment records merged by pn_merge_statistics in rank order)
+    == the unsplit call: every count exactly, means and r to rounding."""
+    import paper_0908_3889_b200 as pn
+    from paper_0908_3889_b200 import pipeline, sharding
+
+    sp, n, world = specs(), 3001, 3
+    kw = dict(rtol=1e-8, atol=1e-10, bins1=20, bins2=16, fused=fused)
+    whole = pn.run_ensembles(sp, n, OMEGAF, **kw)
+    shares = [pn.run_ensembles(sp, n, OMEGAF, shard=(k, world), **kw) for k in range(world)]
+    assert [s["shard"] for s in shares] == [(0, 1001), (1001, 2001), (2001, 3001)]
+    assert all(s["status"] == 0 for s in shares)
+    got = {k: v.cpu().numpy() for k, v in sharding.merge_shards(shares, pipeline._merge_on_device).items() if hasattr(v, "cpu")}
+    for k in ("n_skipped", "hist1", "hist2", "hist2_max"):
+        assert np.array_equal(got[k], whole[k]), k
+    assert np.array_equal(got["moments"][..., 0], whole["moments"][..., 0]) and np.all(got["moments"][..., 0] == n)
+    assert np.abs(got["moments"][..., 1:3] - whole["moments"][..., 1:3]).max() <= 1e-13
+    assert np.abs(got["moments"][..., 3:] - whole["moments"][..., 3:]).max() <= 1e-11 * n
+    assert np.abs(got["pearson_r"] - whole["pearson_r"]).max() <= 1e-12
+    # more ranks than systems: the empty shares are neutral
+    tiny = [pn.run_ensembles(sp[:2], 2, OMEGAF, shard=(k, 4), **kw) for k in range(4)]
+    assert [s["shard"] for s in tiny] == [(0, 1), (1, 2), (2, 2), (2, 2)]
+    t = sharding.merge_shards(tiny, pipeline._merge_on_device)
+    w = pn.run_ensembles(sp[:2], 2, OMEGAF, **kw)
+    assert np.array_equal(t["hist1"].cpu().numpy(), w["hist1"]) and np.array_equal(t["moments"][..., 0].cpu().numpy(), w["moments"][..., 0])
+    assert np.allclose(t["pearson_r"].cpu().numpy(), w["pearson_r"], rtol=0, atol=1e-12, equal_nan=True)
