@@ -105,6 +105,12 @@ typedef struct pn_options {
                               the generic kernel (per-lane constants) even for uniform-mass batches; 2: always the
                               scalar FP32 kernel instead of the packed two-systems-per-lane one; 4: pn_run_ensembles
                               orders the queue by cost even for more than 4 ensembles (measurement only: several times slower) */
+    int hist_bins;         /* pn_integrate_ex only.  hist_counts != NULL: the call also bins the final states it has just
+                              written, as pn_histogram(out_final, N, hist_bins, hist_counts, hist_skipped) would, while they
+                              are still on the device: a host-buffer caller does not upload the 80 bytes per system again
+                              (the state goes to the device once and comes back once).  1 <= hist_bins <= 2^24 */
+    unsigned long long* hist_counts;   /* [3][hist_bins] or NULL (no histogram); host pointer iff host_buffers */
+    unsigned long long* hist_skipped;  /* [3] or NULL */
 } pn_options;
 
 /* Same as pn_integrate with explicit options (opt == NULL: defaults). */

@@ -28,7 +28,8 @@ class PnOptions(C.Structure):
     _fields_ = [("size", C.c_int), ("fixed_steps", C.c_int), ("h0", C.c_double), ("max_steps", C.c_int),
                 ("term_mask", C.c_uint), ("tau_land", C.c_double), ("layout", C.c_int), ("host_buffers", C.c_int),
                 ("async_", C.c_int), ("input_order", C.c_int), ("out_time", C.c_void_p), ("out_rejected", C.c_void_p),
-                ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int), ("variant", C.c_int)]
+                ("stream", C.c_void_p), ("block_threads", C.c_int), ("grid_blocks", C.c_int), ("variant", C.c_int),
+                ("hist_bins", C.c_int), ("hist_counts", C.c_void_p), ("hist_skipped", C.c_void_p)]
 
 
 class PnStatsOut(C.Structure):
@@ -160,7 +161,7 @@ def _require(name, a, dtype, shape=None, host=None, at_least=False):
 
 def make_options(*, fixed_steps=0, h0=0.0, max_steps=0, term_mask=0, tau_land=0.0, layout=0, host_buffers=False,
                  async_=False, input_order=False, out_time=None, out_rejected=None, stream=None, block_threads=0,
-                 grid_blocks=0, variant=0) -> PnOptions:
+                 grid_blocks=0, variant=0, hist_bins=0, hist_counts=None, hist_skipped=None) -> PnOptions:
     o = PnOptions()
     o.size = C.sizeof(PnOptions)
     o.fixed_steps, o.h0, o.max_steps, o.term_mask, o.tau_land = int(fixed_steps), float(h0), int(max_steps), int(term_mask), float(tau_land)
@@ -168,6 +169,7 @@ def make_options(*, fixed_steps=0, h0=0.0, max_steps=0, term_mask=0, tau_land=0.
     o.out_time, o.out_rejected = _ptr(out_time), _ptr(out_rejected)
     o.stream = None if stream is None else int(getattr(stream, "cuda_stream", stream))
     o.block_threads, o.grid_blocks, o.variant = int(block_threads), int(grid_blocks), int(variant)
+    o.hist_bins, o.hist_counts, o.hist_skipped = int(hist_bins), _ptr(hist_counts), _ptr(hist_skipped)
     return o
 
 
@@ -186,6 +188,8 @@ def pn_integrate(init_states, masses, omega0, omegaf, rtol, atol, precision, out
     _require("out_steps", out_steps, "i32", (n,), host)
     _require("out_time", opts.get("out_time"), "f64", (n,), host)
     _require("out_rejected", opts.get("out_rejected"), "i32", (n,), host)
+    _require("hist_counts", opts.get("hist_counts"), "i64", (3, max(int(opts.get("hist_bins", 0)), 0)), host, at_least=True)
+    _require("hist_skipped", opts.get("hist_skipped"), "i64", (3,), host, at_least=True)
     if host:
         opts["host_buffers"] = True
     o = make_options(**opts)

@@ -132,7 +132,19 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
         o = *opt_in;
     }
     if (N < 0 || N > 0x7fffffffLL / 16) return PN_EINVAL;
-    if (N == 0) return PN_OK;
+    if (o.hist_counts && (o.hist_bins < 1 || o.hist_bins > (1 << 24))) return PN_EINVAL;
+    if (N == 0) {
+        if (o.hist_counts) {              // the histogram of nothing: zero counts, as pn_histogram writes them
+            const size_t hb = sizeof(unsigned long long) * 3 * (size_t)o.hist_bins, sb = sizeof(unsigned long long) * 3;
+            if (o.host_buffers) { memset(o.hist_counts, 0, hb); if (o.hist_skipped) memset(o.hist_skipped, 0, sb); }
+            else {
+                CK(cudaMemsetAsync(o.hist_counts, 0, hb, (cudaStream_t)o.stream));
+                if (o.hist_skipped) CK(cudaMemsetAsync(o.hist_skipped, 0, sb, (cudaStream_t)o.stream));
+                if (!o.async) CK(cudaStreamSynchronize((cudaStream_t)o.stream));
+            }
+        }
+        return PN_OK;
+    }
     if (!init_states || !masses || !out_final || !out_steps) return PN_EINVAL;
     if (precision != PN_FP64 && precision != PN_FP32 && precision != PN_MIXED) return PN_EINVAL;
     const bool fixed = o.fixed_steps > 0;
@@ -224,6 +236,18 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
     CK(cudaEventRecord(c.ev[2], s));
     if (o.layout == 0) CK(pn_launch_soa_to_aos((const double*)c.soa_out.p, d_final, n, 10, s));
     CK(cudaEventRecord(c.ev[3], s));
+    // optional: the histograms of the final states while they are on the device (pn_options.hist_counts)
+    unsigned long long* d_hc = o.hist_counts;
+    unsigned long long* d_hs = o.hist_skipped;
+    if (o.hist_counts) {
+        if (o.host_buffers) {
+            if ((rc = c.h_counts.ensure(sizeof(unsigned long long) * (3 * (size_t)o.hist_bins + 3))) != PN_OK) return rc;
+            d_hc = (unsigned long long*)c.h_counts.p;
+            d_hs = d_hc + 3 * (size_t)o.hist_bins;
+        }
+        CK(pn_launch_histogram(d_final, o.layout, N, o.hist_bins, d_hc, d_hs, s));
+        CK(cudaEventRecord(c.ev[4], s));
+    }
 
     if (o.async) {
         // the call's status is folded into the stream's sticky word, which pn_stream_status() reads and clears
@@ -238,12 +262,15 @@ extern "C" int pn_integrate_ex(const double* init_states, const double* masses, 
         CK(cudaMemcpyAsync(out_steps, d_steps, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, s));
         if (o.out_time) CK(cudaMemcpyAsync(o.out_time, d_time, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, s));
         if (o.out_rejected) CK(cudaMemcpyAsync(o.out_rejected, d_rej, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost, s));
+        if (o.hist_counts) CK(cudaMemcpyAsync(o.hist_counts, d_hc, sizeof(unsigned long long) * 3 * (size_t)o.hist_bins, cudaMemcpyDeviceToHost, s));
+        if (o.hist_counts && o.hist_skipped) CK(cudaMemcpyAsync(o.hist_skipped, d_hs, sizeof(unsigned long long) * 3, cudaMemcpyDeviceToHost, s));
     }
     Small hs;
     CK(cudaMemcpyAsync(&hs, small, sizeof hs, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     CK(cudaGetLastError());
     for (int i = 0; i < 3; ++i) CK(cudaEventElapsedTime(&g_ms[i], c.ev[i], c.ev[i + 1]));
+    if (o.hist_counts) CK(cudaEventElapsedTime(&g_ms[3], c.ev[3], c.ev[4]));
     memcpy(g_counters, hs.counters, sizeof g_counters);
     g_redo_count = hs.redo_count;
     return hs.status;

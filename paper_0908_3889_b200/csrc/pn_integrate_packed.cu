@@ -4,7 +4,8 @@
 // The plain FP32 kernel (pn_integrate.cu, real = float) is issue-bound: ~965 warp instructions per trial step at one
 // per cycle and scheduler (r1: 0.46 of the FP32 FMA peak at 77 % issue utilisation).  Two things changed here.
 //  (1) Packing WITHIN a system.  Blackwell's FFMA2 does two FP32 FMAs per lane in one issue slot (measured 74.3 TFLOP/s
-//      against 70.9 with FFMA, profiles/r2_microbenchmarks.md).  Everything that treats the ten components alike --
+//      against 70.9 with FFMA: pn_measure_fma_peak(3) and (PN_FP32), in the bench line as roofline.peak_measured_ffma2 /
+//      peak_measured_fma, profiles/r2_bench_lines.md).  Everything that treats the ten components alike --
 //      the Dormand-Prince stage sums, the error vector, the state update: 270 of the ~780 FP32 operations of a trial
 //      step -- and the x / y halves of the RHS's vector operations are packed (pn_rhs.cuh, pair layout), which removes
 //      ~190 issue slots per trial step at an unchanged register count (16 resident warps per SM as before).

@@ -47,12 +47,13 @@ def test_options_struct_matches_header(tmp_path):
     src = tmp_path / "sz.c"
     src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "pn.h"\nint main(){printf("%zu %zu %zu %zu %zu",'
                    "sizeof(pn_options), offsetof(pn_options,tau_land), offsetof(pn_options,out_time),"
-                   "offsetof(pn_options,stream), offsetof(pn_options,variant));return 0;}\n")
+                   "offsetof(pn_options,stream), offsetof(pn_options,variant));"
+                   'printf(" %zu %zu", offsetof(pn_options,hist_bins), offsetof(pn_options,hist_skipped));return 0;}\n')
     exe = tmp_path / "sz"
     subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
     got = [int(t) for t in subprocess.check_output([str(exe)]).split()]
     assert got == [C.sizeof(PnOptions), PnOptions.tau_land.offset, PnOptions.out_time.offset,
-                   PnOptions.stream.offset, PnOptions.variant.offset]
+                   PnOptions.stream.offset, PnOptions.variant.offset, PnOptions.hist_bins.offset, PnOptions.hist_skipped.offset]
 
 
 def test_new_structs_match_header(tmp_path):

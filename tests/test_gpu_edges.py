@@ -335,6 +335,43 @@ def test_async_calls_keep_their_status_and_scratch(pn):
     assert again["status"] == 0 and np.array_equal(again["final"], ref3["final"])
 
 
+def test_integrate_with_the_histogram_in_the_same_call(pn):
+    """pn_options.hist_counts (include/pn.h): pn_integrate_ex bins the final states it has just written while they are on
+    the device, so a host-buffer caller uploads 96 bytes per system, not 176.  Ragged size; host buffers,
+    device buffers and the SoA layout: states bit-identical to a call without the option, counts equal to pn_histogram
+    of those states."""
+    cfg = W.with_size(W.CONFIGS["C3"], 3001)
+    y0, m = W.generate(cfg)
+    ref = gpu_integrate(pn, y0, m, cfg)
+    c_ref = torch.zeros(3, cfg.bins, dtype=torch.int64, device="cuda:0"); s_ref = torch.zeros(3, dtype=torch.int64, device="cuda:0")
+    pn.pn_histogram(ref["d_final"], cfg.bins, c_ref, s_ref)
+    c_ref, s_ref = c_ref.cpu().numpy(), s_ref.cpu().numpy()
+    assert c_ref.sum() + s_ref.sum() == 3 * cfg.n
+    # host buffers
+    h_yf = np.full((cfg.n, 10), np.nan); h_steps = np.zeros(cfg.n, dtype=np.int32)
+    h_c = np.full((3, cfg.bins), -1, dtype=np.int64); h_s = np.full(3, -1, dtype=np.int64)
+    assert pn.pn_integrate(y0, m, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, h_yf, h_steps, hist_bins=cfg.bins, hist_counts=h_c, hist_skipped=h_s) == 0
+    assert np.array_equal(h_yf, ref["final"]) and np.array_equal(h_steps, ref["steps"])
+    assert np.array_equal(h_c, c_ref) and np.array_equal(h_s, s_ref)
+    assert pn.pn_last_kernel_ms()["histogram"] > 0
+    # device buffers, AoS and SoA
+    for layout in (0, 1):
+        t = (lambda a: torch.from_numpy(np.ascontiguousarray(a.T if layout else a)).cuda())
+        d_yf = torch.empty((10, cfg.n) if layout else (cfg.n, 10), dtype=torch.float64, device="cuda:0")
+        d_steps = torch.zeros(cfg.n, dtype=torch.int32, device="cuda:0")
+        d_c = torch.full((3, cfg.bins), -1, dtype=torch.int64, device="cuda:0")
+        assert pn.pn_integrate(t(y0), t(m), 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, d_yf, d_steps, layout=layout, hist_bins=cfg.bins, hist_counts=d_c) == 0
+        got = d_yf.cpu().numpy()
+        assert np.array_equal(got.T if layout else got, ref["final"]) and np.array_equal(d_c.cpu().numpy(), c_ref)
+    # N = 0: zero counts; a bad bin count is refused
+    e10 = torch.zeros(0, 10, dtype=torch.float64, device="cuda:0"); e2 = torch.zeros(0, 2, dtype=torch.float64, device="cuda:0")
+    d_c = torch.full((3, 7), -1, dtype=torch.int64, device="cuda:0")
+    assert pn.pn_integrate(e10, e2, 0.0, 0.05, 1e-10, 1e-12, 0, e10, torch.zeros(0, dtype=torch.int32, device="cuda:0"), hist_bins=7, hist_counts=d_c) == 0
+    assert d_c.sum().item() == 0
+    with pytest.raises(pn.PnError):
+        pn.pn_integrate(y0, m, 0.0, cfg.omegaf, cfg.rtol, cfg.atol, 0, h_yf, h_steps, hist_bins=0, hist_counts=h_c)
+
+
 def test_stream_release_recycles_contexts_and_table_rows(pn):
     """pn_stream_release (include/pn.h): a device has 4 rows in the uniform-mass constant table, one per live stream
     context.  A 5th live stream runs the generic kernel (rounding differs); releasing a stream returns its row, so any
